@@ -1,0 +1,290 @@
+"""Pins of the fp64 oracle against what the paper and the mathematics fix.
+
+The paper prints no worked numeric example (PAPER.md has formulas :79, :100-118 and a timing table
+only), so the pins are closed forms, invariants, brute force on tiny inputs and a library
+cross-check.  Each is chosen so that a plausible mistake in oracle/mvd_oracle.c fails it:
+  dropped/extra term .......... P5 (dense matrix), P8 (FFT)
+  conv <-> correlation swapped . P2 (off-centre delta closed form), P5, P8
+  wrong centre / axis order .... P2 (dz != dx), P5 (H != W), P8
+  simultaneous instead of sequential view update ... P6 (sum conservation), P5
+  wrong view order ............. P5
+  boundary not periodic ........ P3, P10, P5 (K > H aliasing)
+  eps guard misplaced .......... P1 with zeros in phi, test_eps_guard
+None of these tests touches the CUDA path.
+"""
+import numpy as np
+import pytest
+
+from oracle import mvd_oracle as orc
+from paper_1503_07998_b200 import synth
+
+
+def rand_psfs(V, K, seed):
+    rng = np.random.default_rng(seed)
+    return np.stack([synth.random_psf(K, rng) for _ in range(V)])
+
+
+# ---------------------------------------------------------------------------------------------
+# literal definition == fast (wrap-padded) implementation, bit for bit
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("W,H,K,V,T", [(8, 8, 3, 2, 3), (12, 8, 5, 3, 2), (8, 12, 7, 2, 2),
+                                        (6, 5, 9, 2, 2), (17, 9, 5, 1, 3)])
+def test_literal_equals_padded_bitwise(W, H, K, V, T):
+    views = synth.random_views(V, 2, W, H, seed=W * 100 + H)
+    psfs = rand_psfs(V, K, 5)
+    a = orc.deconvolve(views, psfs, T, literal=True, n_threads=1)
+    b = orc.deconvolve(views, psfs, T, literal=False, n_threads=2)
+    assert np.array_equal(a, b)
+
+
+# ---------------------------------------------------------------------------------------------
+# P1: centred delta PSF, one view: psi == phi after any number of iterations, exactly
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("T", [0, 1, 7])
+def test_P1_centred_delta_is_identity(T):
+    views = synth.random_views(1, 3, 16, 10, seed=1, lo=0, hi=65536)
+    views[0, 0, :2, :3] = 0          # zeros exercise the eps guard: 0 / max(0, eps) = 0
+    views[0, 1, 4, 5] = 65535
+    out = orc.deconvolve(views, synth.delta_psf(5)[None], T)
+    assert np.array_equal(out, views[0].astype(np.float64))
+
+
+# ---------------------------------------------------------------------------------------------
+# P2: off-centre delta at offset d: psi_T(x) = phi(x + d) for T >= 1 (closed form).
+# b(x) = phi(x-d); r(x) = phi(x)/phi(x-d); q(x) = r(x+d); psi_1(x) = phi(x+d); then r == 1.
+# With convolution and correlation swapped the result would be phi(x - d).
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dz,dx", [(1, -2), (-3, 1), (0, 2), (2, 0)])
+@pytest.mark.parametrize("T", [1, 4])
+def test_P2_offcentre_delta_shifts_by_plus_d(dz, dx, T):
+    views = synth.random_views(1, 2, 14, 9, seed=2, lo=5, hi=3000)
+    out = orc.deconvolve(views, synth.delta_psf(7, dz, dx)[None], T)
+    phi = views[0].astype(np.float64)
+    expect = np.roll(phi, shift=(-dz, -dx), axis=(1, 2))        # expect[y, x] = phi[y+dz, x+dx]
+    np.testing.assert_allclose(out, expect, rtol=1e-12, atol=0)
+    wrong = np.roll(phi, shift=(dz, dx), axis=(1, 2))
+    assert not np.allclose(out, wrong, rtol=1e-3)
+
+
+# ---------------------------------------------------------------------------------------------
+# P3: constant images with normalised PSFs stay constant (normalisation + periodic boundary)
+# ---------------------------------------------------------------------------------------------
+def test_P3_constant_is_fixed_point():
+    V, K = 3, 5
+    views = np.full((V, 2, 9, 11), 1234, dtype=np.uint16)
+    psfs = rand_psfs(V, K, 3)
+    out = orc.deconvolve(views, psfs, 6)
+    # fp32 PSFs sum to 1 within ~1e-7, compounded over 2*V*T convolutions
+    np.testing.assert_allclose(out, 1234.0, rtol=5e-6)
+
+
+# ---------------------------------------------------------------------------------------------
+# P4: psi stays non-negative and finite
+# ---------------------------------------------------------------------------------------------
+def test_P4_nonnegative_and_finite():
+    views = synth.random_views(2, 2, 16, 12, seed=4, lo=0, hi=500)
+    views[:, :, 3:6, 2:9] = 0
+    out = orc.deconvolve(views, rand_psfs(2, 5, 4), 8)
+    assert np.isfinite(out).all() and (out >= 0).all()
+
+
+# ---------------------------------------------------------------------------------------------
+# P5: brute force with dense matrices.  A_v[(y,x),(y',x')] += P_v[j][i] for
+# (y',x') = ((y-(j-c)) mod H, (x-(i-c)) mod W);  psi <- psi . A_v^T (phi_v / max(A_v psi, eps)).
+# Written with explicit matrices so that "correlation" is literally the transpose.
+# ---------------------------------------------------------------------------------------------
+def dense_operator(P, H, W):
+    K = P.shape[0]
+    c = (K - 1) // 2
+    A = np.zeros((H * W, H * W))
+    for y in range(H):
+        for x in range(W):
+            for j in range(K):
+                for i in range(K):
+                    A[y * W + x, ((y - (j - c)) % H) * W + ((x - (i - c)) % W)] += float(P[j, i])
+    return A
+
+
+def dense_rl(views_plane, psfs, T, eps):
+    V, H, W = views_plane.shape
+    phi = views_plane.reshape(V, -1).astype(np.float64)
+    psi = phi.sum(0) / V
+    ops = [dense_operator(psfs[v], H, W) for v in range(V)]
+    for _ in range(T):
+        for v in range(V):
+            b = ops[v] @ psi
+            r = phi[v] / np.maximum(b, eps)
+            psi = psi * (ops[v].T @ r)
+    return psi.reshape(H, W)
+
+
+@pytest.mark.parametrize("W,H,K", [(8, 8, 3), (8, 8, 5), (8, 8, 7), (12, 8, 5), (8, 12, 7),
+                                    (8, 8, 9),      # K > W: taps alias around the plane
+                                    (6, 5, 9)])
+def test_P5_dense_matrix_brute_force(W, H, K):
+    V, T = 3, 4
+    views = synth.random_views(V, 2, W, H, seed=50 + K)
+    psfs = rand_psfs(V, K, 60 + W)
+    out = orc.deconvolve(views, psfs, T)
+    for p in range(2):
+        ref = dense_rl(views[:, p], psfs, T, float(np.float32(1e-6)))
+        np.testing.assert_allclose(out[p], ref, rtol=1e-11, atol=1e-11)
+
+
+def test_P5_detects_view_order_and_simultaneous_form():
+    """The pin has teeth: reversed view order or the product (simultaneous) form differ by percent."""
+    V, T, W, H, K = 3, 4, 8, 8, 5
+    views = synth.random_views(V, 1, W, H, seed=77)
+    psfs = rand_psfs(V, K, 78)
+    out = orc.deconvolve(views, psfs, T)[0]
+    rev = dense_rl(views[::-1, 0], psfs[::-1], T, 1e-6)
+    assert np.linalg.norm(out - rev) / np.linalg.norm(out) > 1e-3
+    # simultaneous: every factor from the same psi^t
+    phi = views[:, 0].reshape(V, -1).astype(np.float64)
+    psi = phi.sum(0) / V
+    ops = [dense_operator(psfs[v], H, W) for v in range(V)]
+    for _ in range(T):
+        f = np.ones_like(psi)
+        for v in range(V):
+            f *= ops[v].T @ (phi[v] / np.maximum(ops[v] @ psi, 1e-6))
+        psi = psi * f
+    assert np.linalg.norm(out.ravel() - psi) / np.linalg.norm(out) > 1e-3
+
+
+# ---------------------------------------------------------------------------------------------
+# P6: sum conservation after EVERY view update: sum(psi) == sum(phi_v)   (sequential form only)
+# ---------------------------------------------------------------------------------------------
+def test_P6_sum_conservation_per_view_update():
+    V, T, K = 3, 5, 7
+    views = synth.random_views(V, 1, 20, 14, seed=6, lo=20, hi=900)
+    psfs64 = [p.astype(np.float64) for p in rand_psfs(V, K, 6)]
+    tr = orc.trace(views[:, 0], np.stack(psfs64), T)
+    assert tr.shape == (T * V, 14, 20)
+    for t in range(T):
+        for v in range(V):
+            s_psf = float(np.stack(psfs64)[v].astype(np.float32).astype(np.float64).sum())
+            got = tr[t * V + v].sum()
+            want = views[v, 0].astype(np.float64).sum()
+            # exact identity is sum(psi') = sum_y r(y) * (P^T-sum-weighted b) ; with sum(P)=1+-1e-7
+            assert abs(got / want - 1.0) < 5e-7 + abs(s_psf - 1.0) * 2
+
+
+# ---------------------------------------------------------------------------------------------
+# P7: single view: the I-divergence  sum[ phi log(phi/b) - phi + b ],  b = psi * P,  never increases
+# ---------------------------------------------------------------------------------------------
+def test_P7_idivergence_non_increasing():
+    T, K = 25, 7
+    prob = synth.make_problem(1, 1, 24, 18, K, T, seed=7, psf="random")
+    tr = orc.trace(prob.views[:, 0], prob.psfs, T)
+    phi = prob.views[0, 0].astype(np.float64)
+
+    def idiv(psi):
+        b = orc.blur(psi, prob.psfs[0])
+        with np.errstate(divide="ignore", invalid="ignore"):
+            t = np.where(phi > 0, phi * np.log(phi / b), 0.0)
+        return float((t - phi + b).sum())
+
+    d = [idiv(phi)] + [idiv(tr[t]) for t in range(T)]
+    assert all(d[k + 1] <= d[k] * (1 + 1e-12) + 1e-9 for k in range(T)), d
+    assert d[-1] < 0.9 * d[0]
+
+
+# ---------------------------------------------------------------------------------------------
+# P8: both convolutions against numpy's FFT (a library routine): blur = ifft(fft(psi) fft(h)),
+# back-projection = ifft(fft(r) conj(fft(h))), h = PSF placed at ((j-c) mod H, (i-c) mod W)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("W,H,K", [(16, 12, 5), (15, 20, 9), (32, 8, 7), (8, 6, 11)])
+def test_P8_convolutions_match_numpy_fft(W, H, K):
+    rng = np.random.default_rng(8)
+    img = rng.random((H, W)) * 100.0
+    P = synth.random_psf(K, rng)
+    c = (K - 1) // 2
+    h = np.zeros((H, W))
+    for j in range(K):
+        for i in range(K):
+            h[(j - c) % H, (i - c) % W] += float(P[j, i])
+    Fh = np.fft.fft2(h)
+    conv = np.fft.ifft2(np.fft.fft2(img) * Fh).real
+    corr = np.fft.ifft2(np.fft.fft2(img) * np.conj(Fh)).real
+    for literal in (False, True):
+        np.testing.assert_allclose(orc.blur(img, P, literal), conv, rtol=1e-11, atol=1e-11)
+        np.testing.assert_allclose(orc.backproject(img, P, literal), corr, rtol=1e-11, atol=1e-11)
+    # the two differ for an asymmetric PSF, so a swap cannot hide
+    assert np.abs(conv - corr).max() > 1e-3 * np.abs(conv).max()
+
+
+def test_P8_backproject_is_adjoint_of_blur():
+    rng = np.random.default_rng(81)
+    a, b = rng.random((10, 14)), rng.random((10, 14))
+    P = synth.random_psf(5, rng)
+    lhs = (orc.blur(a, P) * b).sum()
+    rhs = (a * orc.backproject(b, P)).sum()
+    assert abs(lhs - rhs) < 1e-12 * abs(lhs)
+
+
+# ---------------------------------------------------------------------------------------------
+# P9: a duplicated view: (phi, P) twice for T iterations == once for 2T iterations, bit-identical
+# ---------------------------------------------------------------------------------------------
+def test_P9_duplicated_view():
+    views1 = synth.random_views(1, 2, 12, 10, seed=9)
+    psf = rand_psfs(1, 5, 9)
+    views2 = np.concatenate([views1, views1], axis=0)
+    a = orc.deconvolve(views2, np.concatenate([psf, psf]), 3)
+    b = orc.deconvolve(views1, psf, 6)
+    assert np.array_equal(a, b)
+
+
+# ---------------------------------------------------------------------------------------------
+# P10: shift equivariance: circularly shifting every phi_v shifts the output identically
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("sy,sx", [(1, 0), (0, 1), (3, 5), (-2, 7)])
+def test_P10_shift_equivariance(sy, sx):
+    views = synth.random_views(2, 1, 13, 9, seed=10)
+    psfs = rand_psfs(2, 5, 10)
+    a = orc.deconvolve(views, psfs, 3)
+    b = orc.deconvolve(np.roll(views, (sy, sx), axis=(2, 3)), psfs, 3)
+    assert np.array_equal(np.roll(a, (sy, sx), axis=(1, 2)), b)
+
+
+# ---------------------------------------------------------------------------------------------
+# P11: zero iterations returns the mean of the views
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("V", [1, 2, 3, 6])
+def test_P11_zero_iterations_is_mean(V):
+    views = synth.random_views(V, 2, 8, 8, seed=11, lo=0, hi=65536)
+    out = orc.deconvolve(views, rand_psfs(V, 3, 11), 0)
+    assert np.array_equal(out, views.astype(np.float64).sum(0) / V)
+
+
+# ---------------------------------------------------------------------------------------------
+# eps guard (reading A6): r = phi / max(b, eps), eps taken at fp32 precision
+# ---------------------------------------------------------------------------------------------
+def test_eps_guard_value():
+    # one view, centred delta, phi == 0 everywhere except one pixel: psi stays phi, no NaN/Inf
+    views = np.zeros((1, 1, 6, 6), dtype=np.uint16)
+    views[0, 0, 2, 3] = 9
+    out = orc.deconvolve(views, synth.delta_psf(3)[None], 3)
+    assert np.array_equal(out[0], views[0, 0].astype(np.float64))
+    # blur below eps: psi = 0 region, phi > 0 there -> ratio = phi/eps lands only where psi == 0
+    v2 = np.zeros((2, 1, 6, 6), dtype=np.uint16)
+    v2[1, 0, 0, 0] = 7
+    out = orc.deconvolve(v2, np.stack([synth.delta_psf(3), synth.delta_psf(3)]), 1)
+    # psi0 = 3.5 at (0,0); view 0: r = 0/3.5 = 0 -> psi = 0 everywhere; view 1: r = 7/eps, psi*q = 0
+    assert np.array_equal(out, np.zeros_like(out))
+
+
+def test_argument_validation():
+    views = synth.random_views(1, 1, 8, 8, seed=12)
+    with pytest.raises(ValueError):
+        orc.deconvolve(views, np.ones((1, 4, 4), np.float32) / 16, 1)      # even K
+    with pytest.raises(ValueError):
+        orc.deconvolve(views, synth.delta_psf(3)[None], -1)                # negative T
+    with pytest.raises(ValueError):
+        orc.deconvolve(views, synth.delta_psf(3)[None], 1, eps=0.0)        # eps <= 0
+
+
+def test_threads_do_not_change_results():
+    prob = synth.make_problem(2, 5, 16, 12, 5, 2, seed=13)
+    a = orc.deconvolve(prob.views, prob.psfs, prob.T, n_threads=1)
+    b = orc.deconvolve(prob.views, prob.psfs, prob.T, n_threads=4)
+    assert np.array_equal(a, b)
