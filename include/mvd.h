@@ -1,0 +1,158 @@
+/*
+ * mvd.h -- C ABI of libmvd: plane-wise multi-view Richardson-Lucy deconvolution on one B200.
+ *
+ * The operation (arXiv 1503.07998, Schmid & Huisken, "Real-time multi-view deconvolution"):
+ *   PAPER.md:79      (Supp. Note 1)  psi^{t+1} = psi^t  prod_v  ( phi_v / (psi^t * P_v) ) * P_v^*
+ *   PAPER.md:100-104 (Supp. Note 2 s.1) "Independent" back-projector X = P_v^*
+ *   PAPER.md:118     P_v^* is the flipped PSF of view v
+ *   PAPER.md:31      the 3D transfer function is approximated by a 2D PSF, so every plane orthogonal
+ *                    to the rotation axis (an x-z plane) is an independent 2D problem
+ *   PAPER.md:87-89   phi_v is uint16 camera data, the estimate psi is float
+ *   PAPER.md:126-152 (Supp. Note 2 s.3, Algorithm 1) three CUDA streams overlap H2D, the RL steps and D2H
+ *
+ * Per plane, with the readings of DESIGN.md (the paper is silent on most of them; BASELINE.json's
+ * north_star fixes them): psi_0 = mean_v phi_v; then for t = 0..iterations-1, for v = 0..n_views-1 IN TURN
+ *   b   = psi (*) P_v                      periodic convolution   b(x) = sum_u P_v(u) psi(x - u)
+ *   r   = phi_v / max(b, eps)
+ *   q   = r (*) P_v^*                      periodic correlation   q(x) = sum_u P_v(u) r(x + u)
+ *   psi = psi . q
+ * PSF array index (j, i) <-> offset u = (j - c, i - c), c = (psf_size - 1) / 2, j along z (rows), i along x.
+ *
+ * Layouts (x fastest everywhere):
+ *   psfs   float    [n_views][psf_size][psf_size]
+ *   views  uint16_t [n_views][n_planes][plane_h][plane_w]      ("view-major": each view is one stack)
+ *   out    float    [n_planes][plane_h][plane_w]
+ *
+ * All functions return MVD_OK (0) or a negative code; nothing throws, aborts or prints.  The library
+ * never falls back to the CPU: without a CUDA device every compute call fails with MVD_ERR_CUDA.
+ */
+#ifndef MVD_H_
+#define MVD_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#if defined(__GNUC__)
+#define MVD_API __attribute__((visibility("default")))
+#else
+#define MVD_API
+#endif
+
+typedef struct mvd_handle mvd_handle; /* opaque; owned by the library; one device, not thread-safe */
+
+enum {
+    MVD_OK = 0,
+    MVD_ERR_INVALID = -1,     /* null pointer, non-positive size, even psf_size, bad eps, bad PSF value */
+    MVD_ERR_UNSUPPORTED = -2, /* a forced path cannot handle this shape (e.g. FFT on a non-smooth size)  */
+    MVD_ERR_CUDA = -3,        /* a CUDA call failed; mvd_last_cuda_error() has the cudaError_t           */
+    MVD_ERR_NOMEM = -4,       /* device or pinned-staging allocation failed                              */
+    MVD_ERR_BUSY = -5         /* reserved                                                                */
+};
+
+/* Convolution engine used for steps a1 and a3 (both engines fuse a2 and a4 into their kernels). */
+enum {
+    MVD_PATH_AUTO = 0,   /* chosen in mvd_create from the measured crossover table            */
+    MVD_PATH_DIRECT = 1, /* shared-memory halo tiles + register-blocked FP32 FMA; any shape               */
+    MVD_PATH_FFT = 2     /* hand-written batched 2D FFT with the pointwise steps fused into the passes;
+                            plane_w and plane_h must factor into 2, 3 and 5 and stay within the kernel's
+                            shared-memory limit (see mvd_path_supported)                                  */
+};
+
+/*
+ * mvd_create -- build a plan for planes of plane_w x plane_h pixels seen by n_views views.
+ *   psfs        HOST pointer, float [n_views][psf_size][psf_size]; copied, may be freed on return.
+ *               Used as given (not renormalised); values must be finite and >= 0.
+ *   psf_size    odd, >= 1.  psf_size > plane_w or plane_h is allowed (taps alias around the plane).
+ *   iterations  >= 0; 0 returns the mean of the views (the count is the user's choice).
+ *   eps         division guard of step a2, finite and > 0 (north_star: 1e-6).
+ *   out         receives the handle.
+ * The path is MVD_PATH_AUTO unless the environment variable MVD_FORCE_PATH is "direct" or "fft"
+ * (measurement only).  Errors: MVD_ERR_INVALID, MVD_ERR_UNSUPPORTED (forced path), MVD_ERR_CUDA, MVD_ERR_NOMEM.
+ */
+MVD_API int mvd_create(int plane_w, int plane_h, int n_views, const float* psfs, int psf_size,
+               int iterations, float eps, mvd_handle** out);
+
+/* Same, with the path given explicitly (MVD_PATH_*); MVD_FORCE_PATH is ignored. */
+MVD_API int mvd_create_path(int plane_w, int plane_h, int n_views, const float* psfs, int psf_size,
+                    int iterations, float eps, int path, mvd_handle** out);
+
+/*
+ * mvd_deconvolve_planes -- steps a0..a5 on n_planes device-resident planes.
+ *   dev_views_u16  DEVICE, uint16 [n_views][n_planes][plane_h][plane_w]; read-only.
+ *   dev_out_f32    DEVICE, float  [n_planes][plane_h][plane_w]; fully overwritten; must not alias the input.
+ *   stream         a cudaStream_t (NULL = legacy default stream).  The call ENQUEUES and returns; it does
+ *                  not synchronise.  Calls on one handle must all be ordered on one stream (scratch is
+ *                  per handle, grown at first use and kept until mvd_destroy).
+ * n_planes == 0 is a no-op.  Errors: MVD_ERR_INVALID, MVD_ERR_CUDA, MVD_ERR_NOMEM.
+ */
+MVD_API int mvd_deconvolve_planes(mvd_handle* h, const uint16_t* dev_views_u16, float* dev_out_f32,
+                          int n_planes, void* stream);
+
+/*
+ * mvd_deconvolve_host -- the same result for host-resident stacks, streamed through the GPU in batches
+ * of planes on three CUDA streams so that H2D copies, the RL iterations and D2H copies of different
+ * batches overlap (Algorithm 1, with pinned host buffers standing in for disk IO).
+ *   host_views_u16  HOST (pinned for overlap; pageable memory works but serialises), same layout as above.
+ *   host_out_f32    HOST, float [n_planes][plane_h][plane_w].
+ * Blocks until host_out_f32 is complete.  Bit-identical to mvd_deconvolve_planes on the same data.
+ */
+MVD_API int mvd_deconvolve_host(mvd_handle* h, const uint16_t* host_views_u16, float* host_out_f32,
+                        int n_planes);
+
+/* Frees the plan, its scratch, its streams and staging buffers.  NULL is a no-op. */
+MVD_API void mvd_destroy(mvd_handle* h);
+
+/* Static, never-NULL description of a return code. */
+MVD_API const char* mvd_strerror(int code);
+
+/* The raw cudaError_t behind the last MVD_ERR_CUDA / MVD_ERR_NOMEM of this handle (0 if none). */
+MVD_API int mvd_last_cuda_error(const mvd_handle* h);
+
+/* MVD_PATH_DIRECT or MVD_PATH_FFT: what this handle runs. */
+MVD_API int mvd_get_path(const mvd_handle* h);
+
+/* 1 if `path` can run planes of this shape, else 0 (no device needed). */
+MVD_API int mvd_path_supported(int path, int plane_w, int plane_h, int psf_size);
+
+/*
+ * Tuning knobs (measurement; defaults are chosen in mvd_create).
+ *   mvd_set_chunk_planes  planes processed per internal pass of mvd_deconvolve_planes (0 = default)
+ *   mvd_set_batch_planes  planes per pipeline batch of mvd_deconvolve_host (0 = default)
+ */
+MVD_API int mvd_set_chunk_planes(mvd_handle* h, int planes);
+MVD_API int mvd_set_batch_planes(mvd_handle* h, int planes);
+
+/*
+ * Instrumentation for bench.py's roofline line.
+ *   mvd_launch_count      kernels launched by this handle since creation (or since the last reset).
+ *   mvd_profile_enable    when on, every kernel launch is bracketed by CUDA events on the launching stream.
+ *   mvd_profile_read      synchronises the recorded events and returns, per kernel class k in
+ *                         [0, MVD_N_KERNEL_CLASSES), the summed device time ms[k] and launch count n[k]
+ *                         since the last read; both arrays are HOST, length MVD_N_KERNEL_CLASSES.
+ *   mvd_kernel_class_name static name of class k (NULL if out of range).
+ */
+enum { MVD_N_KERNEL_CLASSES = 8 };
+MVD_API long long mvd_launch_count(const mvd_handle* h);
+MVD_API void mvd_launch_count_reset(mvd_handle* h);
+MVD_API int mvd_profile_enable(mvd_handle* h, int on);
+MVD_API int mvd_profile_read(mvd_handle* h, float* ms, long long* n);
+MVD_API const char* mvd_kernel_class_name(int k);
+
+/*
+ * FP32 FMA peak of the current device, measured with a register-only FFMA micro-kernel: *tflops
+ * (2 flop per FMA) and the SM clock in MHz seen while it ran.  Denominator of the direct engine's
+ * roofline fraction (the driver-measured peaks file has no FP32 figure).
+ */
+MVD_API int mvd_measure_fp32_peak(double* tflops, double* sm_mhz);
+
+/* Library version string, e.g. "mvd 0.1 sm_100a". */
+MVD_API const char* mvd_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MVD_H_ */

@@ -1,0 +1,231 @@
+"""Thin ctypes binding of libmvd (include/mvd.h).  Argument marshalling only.
+
+Every step of the hot path runs in the CUDA library; PyTorch is used for device memory, pinned
+memory and streams.  There is no CPU fallback: if `libmvd.so` is missing, or no CUDA device is
+present, the compute calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libmvd.so")
+
+MVD_OK, MVD_ERR_INVALID, MVD_ERR_UNSUPPORTED, MVD_ERR_CUDA, MVD_ERR_NOMEM, MVD_ERR_BUSY = 0, -1, -2, -3, -4, -5
+PATH_AUTO, PATH_DIRECT, PATH_FFT = 0, 1, 2
+N_KERNEL_CLASSES = 8
+PATH_NAMES = {PATH_AUTO: "auto", PATH_DIRECT: "direct", PATH_FFT: "fft"}
+
+# name -> (restype, argtypes): the symbols include/mvd.h declares (tests check the two agree)
+_i, _f, _vp, _ll = ctypes.c_int, ctypes.c_float, ctypes.c_void_p, ctypes.c_longlong
+_fp = ctypes.POINTER(ctypes.c_float)
+SIGNATURES = {
+    "mvd_create": (_i, [_i, _i, _i, _fp, _i, _i, _f, ctypes.POINTER(_vp)]),
+    "mvd_create_path": (_i, [_i, _i, _i, _fp, _i, _i, _f, _i, ctypes.POINTER(_vp)]),
+    "mvd_deconvolve_planes": (_i, [_vp, _vp, _vp, _i, _vp]),
+    "mvd_deconvolve_host": (_i, [_vp, _vp, _vp, _i]),
+    "mvd_destroy": (None, [_vp]),
+    "mvd_strerror": (ctypes.c_char_p, [_i]),
+    "mvd_last_cuda_error": (_i, [_vp]),
+    "mvd_get_path": (_i, [_vp]),
+    "mvd_path_supported": (_i, [_i, _i, _i, _i]),
+    "mvd_set_chunk_planes": (_i, [_vp, _i]),
+    "mvd_set_batch_planes": (_i, [_vp, _i]),
+    "mvd_launch_count": (_ll, [_vp]),
+    "mvd_launch_count_reset": (None, [_vp]),
+    "mvd_profile_enable": (_i, [_vp, _i]),
+    "mvd_profile_read": (_i, [_vp, _fp, ctypes.POINTER(_ll)]),
+    "mvd_kernel_class_name": (ctypes.c_char_p, [_i]),
+    "mvd_version": (ctypes.c_char_p, []),
+    "mvd_measure_fp32_peak": (_i, [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]),
+}
+
+_lib: Optional[ctypes.CDLL] = None
+
+
+class MvdError(RuntimeError):
+    def __init__(self, code: int, what: str, cuda: int = 0):
+        self.code, self.cuda = code, cuda
+        msg = f"{what}: {strerror(code)} (mvd {code}" + (f", cudaError {cuda})" if cuda else ")")
+        super().__init__(msg)
+
+
+def lib() -> ctypes.CDLL:
+    """Load libmvd.so.  Fails loudly if it has not been built (python -m paper_1503_07998_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} is missing: build it with `python -m paper_1503_07998_b200.build` "
+                              "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+def strerror(code: int) -> str:
+    return lib().mvd_strerror(int(code)).decode()
+
+
+def version() -> str:
+    return lib().mvd_version().decode()
+
+
+def path_supported(path: int, plane_w: int, plane_h: int, psf_size: int) -> bool:
+    return bool(lib().mvd_path_supported(path, plane_w, plane_h, psf_size))
+
+
+def kernel_class_names():
+    return [lib().mvd_kernel_class_name(k).decode() for k in range(N_KERNEL_CLASSES)]
+
+
+def measure_fp32_peak() -> Tuple[float, float]:
+    """(TFLOP/s of an FFMA-saturating micro-kernel, its SM clock estimate in MHz) on the current device."""
+    tf, mhz = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    rc = lib().mvd_measure_fp32_peak(ctypes.byref(tf), ctypes.byref(mhz))
+    if rc != MVD_OK:
+        raise MvdError(rc, "mvd_measure_fp32_peak")
+    return tf.value, mhz.value
+
+
+class Mvd:
+    """One plan (mvd_create ... mvd_destroy).  Same names and argument order as the C ABI."""
+
+    def __init__(self, plane_w: int, plane_h: int, n_views: int, psfs: np.ndarray, psf_size: int,
+                 iterations: int, eps: float = 1e-6, path: Optional[int] = None):
+        psfs = np.ascontiguousarray(psfs, dtype=np.float32)
+        if psfs.size != n_views * psf_size * psf_size:
+            raise ValueError("psfs must hold n_views * psf_size * psf_size floats")
+        self._h = _vp()
+        self.plane_w, self.plane_h, self.n_views = plane_w, plane_h, n_views
+        self.psf_size, self.iterations = psf_size, iterations
+        p = psfs.ctypes.data_as(_fp)
+        if path is None:
+            rc = lib().mvd_create(plane_w, plane_h, n_views, p, psf_size, iterations, eps, ctypes.byref(self._h))
+        else:
+            rc = lib().mvd_create_path(plane_w, plane_h, n_views, p, psf_size, iterations, eps, path,
+                                       ctypes.byref(self._h))
+        if rc != MVD_OK:
+            self._h = _vp()
+            raise MvdError(rc, "mvd_create")
+
+    # -- C ABI, one to one ---------------------------------------------------------------------
+    def deconvolve_planes(self, dev_views_u16, dev_out_f32, n_planes: int, stream=None) -> None:
+        """dev_views_u16 / dev_out_f32: CUDA torch tensors (uint16 bits in an int16/uint16 tensor; float32)
+        or raw device pointers (int).  Enqueues on `stream` (torch stream, raw handle or None = current)."""
+        rc = lib().mvd_deconvolve_planes(self._h, _ptr(dev_views_u16), _ptr(dev_out_f32), n_planes,
+                                         _stream(stream))
+        self._raise(rc, "mvd_deconvolve_planes")
+
+    def deconvolve_host(self, host_views_u16, host_out_f32, n_planes: int) -> None:
+        """host buffers: pinned torch tensors, numpy arrays or raw host pointers.  Blocks."""
+        rc = lib().mvd_deconvolve_host(self._h, _ptr(host_views_u16), _ptr(host_out_f32), n_planes)
+        self._raise(rc, "mvd_deconvolve_host")
+
+    def destroy(self) -> None:
+        if getattr(self, "_h", None) is not None and self._h.value:
+            lib().mvd_destroy(self._h)
+            self._h = _vp()
+
+    @property
+    def path(self) -> int:
+        return lib().mvd_get_path(self._h)
+
+    def set_chunk_planes(self, planes: int) -> None:
+        self._raise(lib().mvd_set_chunk_planes(self._h, planes), "mvd_set_chunk_planes")
+
+    def set_batch_planes(self, planes: int) -> None:
+        self._raise(lib().mvd_set_batch_planes(self._h, planes), "mvd_set_batch_planes")
+
+    def launch_count(self) -> int:
+        return int(lib().mvd_launch_count(self._h))
+
+    def launch_count_reset(self) -> None:
+        lib().mvd_launch_count_reset(self._h)
+
+    def profile_enable(self, on: bool) -> None:
+        self._raise(lib().mvd_profile_enable(self._h, int(on)), "mvd_profile_enable")
+
+    def profile_read(self):
+        """{kernel class name: (summed ms, launches)} since the last read (synchronises)."""
+        ms = (ctypes.c_float * N_KERNEL_CLASSES)()
+        n = (_ll * N_KERNEL_CLASSES)()
+        self._raise(lib().mvd_profile_read(self._h, ms, n), "mvd_profile_read")
+        return {name: (float(ms[k]), int(n[k])) for k, name in enumerate(kernel_class_names())}
+
+    # -- plumbing ----------------------------------------------------------------------------------
+    def _raise(self, rc: int, what: str) -> None:
+        if rc != MVD_OK:
+            raise MvdError(rc, what, lib().mvd_last_cuda_error(self._h))
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.destroy()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def _ptr(x) -> _vp:
+    if x is None:
+        return _vp(0)
+    if isinstance(x, int):
+        return _vp(x)
+    if isinstance(x, np.ndarray):
+        if not x.flags["C_CONTIGUOUS"]:
+            raise ValueError("numpy buffer must be C-contiguous")
+        return _vp(x.ctypes.data)
+    if hasattr(x, "data_ptr"):
+        if not x.is_contiguous():
+            raise ValueError("tensor must be contiguous")
+        return _vp(x.data_ptr())
+    raise TypeError(type(x))
+
+
+def _stream(s) -> _vp:
+    if s is None:
+        import torch
+        return _vp(torch.cuda.current_stream().cuda_stream)
+    if isinstance(s, int):
+        return _vp(s)
+    return _vp(s.cuda_stream)
+
+
+def deconvolve(views: np.ndarray, psfs: np.ndarray, iterations: int, eps: float = 1e-6,
+               path: Optional[int] = None, host: bool = False, chunk_planes: int = 0,
+               batch_planes: int = 0) -> np.ndarray:
+    """Convenience for tests: numpy uint16 `[V][N][H][W]` in, numpy float32 `[N][H][W]` out, through
+    mvd_deconvolve_planes (host=False) or mvd_deconvolve_host (host=True, pinned buffers)."""
+    import torch
+    if not torch.cuda.is_available():
+        raise RuntimeError("no CUDA device: libmvd has no CPU fallback")
+    views = np.ascontiguousarray(views, dtype=np.uint16)
+    V, N, H, W = views.shape
+    K = psfs.shape[-1]
+    with Mvd(W, H, V, psfs, K, iterations, eps, path) as m:
+        if chunk_planes:
+            m.set_chunk_planes(chunk_planes)
+        if batch_planes:
+            m.set_batch_planes(batch_planes)
+        tv = torch.from_numpy(views.view(np.int16))
+        if host:
+            hv = tv.pin_memory()
+            ho = torch.empty((N, H, W), dtype=torch.float32).pin_memory()
+            m.deconvolve_host(hv, ho, N)
+            return ho.numpy().copy()
+        dv = tv.cuda()
+        do = torch.empty((N, H, W), dtype=torch.float32, device="cuda")
+        m.deconvolve_planes(dv, do, N)
+        torch.cuda.synchronize()
+        return do.cpu().numpy()

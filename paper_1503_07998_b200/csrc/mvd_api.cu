@@ -1,0 +1,321 @@
+// mvd_api.cu -- the C ABI of libmvd (include/mvd.h): plan creation, the device-resident entry
+// point, and the three-stream host pipeline (Algorithm 1).
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <algorithm>
+#include <new>
+
+#include "mvd_internal.cuh"
+
+// ---------------------------------------------------------------------------------------------
+// helpers
+// ---------------------------------------------------------------------------------------------
+int mvd_check(mvd_handle* h, cudaError_t e) {
+    if (e == cudaSuccess) return MVD_OK;
+    if (h) h->last_cuda = (int)e;
+    (void)cudaGetLastError();   // clear the sticky-less error state
+    return e == cudaErrorMemoryAllocation ? MVD_ERR_NOMEM : MVD_ERR_CUDA;
+}
+
+LaunchScope::LaunchScope(mvd_handle* h_, int kc, cudaStream_t s) : h(h_), stream(s) {
+    h->launches++;
+    if (!h->profiling) return;
+    cudaEvent_t ev[2] = {nullptr, nullptr};
+    for (int k = 0; k < 2; ++k) {
+        if (!h->event_pool.empty()) {
+            ev[k] = h->event_pool.back();
+            h->event_pool.pop_back();
+        } else if (cudaEventCreate(&ev[k]) != cudaSuccess) {
+            ev[k] = nullptr;
+        }
+    }
+    if (!ev[0] || !ev[1]) return;
+    cudaEventRecord(ev[0], stream);
+    e1 = ev[1];
+    h->prof.push_back(ProfRecord{kc, ev[0], ev[1]});
+}
+
+LaunchScope::~LaunchScope() {
+    if (e1) cudaEventRecord(e1, stream);
+}
+
+static int grow(mvd_handle* h, float** p, size_t* have, size_t want) {
+    if (want <= *have) return MVD_OK;
+    if (*p) {
+        // the buffer may still be in use by work enqueued earlier on this handle's stream
+        MVD_TRY(h, cudaDeviceSynchronize());
+        MVD_TRY(h, cudaFree(*p));
+        *p = nullptr;
+        *have = 0;
+    }
+    MVD_TRY(h, cudaMalloc((void**)p, want));
+    *have = want;
+    return MVD_OK;
+}
+
+int ws_reserve(mvd_handle* h, Workspace& ws, size_t a_bytes, size_t b_bytes) {
+    int rc = grow(h, &ws.a, &ws.a_bytes, a_bytes);
+    if (rc != MVD_OK) return rc;
+    return grow(h, &ws.b, &ws.b_bytes, b_bytes);
+}
+
+static void ws_free(Workspace& ws) {
+    if (ws.a) cudaFree(ws.a);
+    if (ws.b) cudaFree(ws.b);
+    ws = Workspace();
+}
+
+// ---------------------------------------------------------------------------------------------
+// plan
+// ---------------------------------------------------------------------------------------------
+int mvd_path_supported(int path, int plane_w, int plane_h, int psf_size) {
+    if (plane_w < 1 || plane_h < 1 || psf_size < 1 || (psf_size % 2) == 0) return 0;
+    if (path == MVD_PATH_DIRECT) {
+        int JC, Kp;
+        direct_choose_chunk(psf_size, &JC, &Kp);
+        const size_t smem = sizeof(float) * ((size_t)psf_size * Kp + (size_t)(64 + Kp - 1) * (psf_size + 64 - 1));
+        return smem <= 227u * 1024u ? 1 : 0;
+    }
+    if (path == MVD_PATH_FFT) return fft_supported(plane_w, plane_h);
+    if (path == MVD_PATH_AUTO)
+        return mvd_path_supported(MVD_PATH_DIRECT, plane_w, plane_h, psf_size) ||
+               mvd_path_supported(MVD_PATH_FFT, plane_w, plane_h, psf_size);
+    return 0;
+}
+
+// Measured crossover: the FFT engine moves a fixed number of bytes per
+// voxel-view-iteration whatever K is, the direct engine does 4 K^2 flop.
+static int choose_path(int W, int H, int K) {
+    const bool fft_ok = mvd_path_supported(MVD_PATH_FFT, W, H, K) != 0;
+    const bool dir_ok = mvd_path_supported(MVD_PATH_DIRECT, W, H, K) != 0;
+    if (fft_ok && (!dir_ok || K >= 7)) return MVD_PATH_FFT;
+    if (dir_ok) return MVD_PATH_DIRECT;
+    return -1;
+}
+
+int mvd_create_path(int plane_w, int plane_h, int n_views, const float* psfs, int psf_size,
+                    int iterations, float eps, int path, mvd_handle** out) {
+    if (!out) return MVD_ERR_INVALID;
+    *out = nullptr;
+    if (!psfs || plane_w < 1 || plane_h < 1 || n_views < 1 || n_views > 255 || iterations < 0)
+        return MVD_ERR_INVALID;
+    if (psf_size < 1 || (psf_size % 2) == 0) return MVD_ERR_INVALID;
+    if (!(eps > 0.f) || !isfinite(eps)) return MVD_ERR_INVALID;
+    if ((long long)plane_w * plane_h > (1LL << 30)) return MVD_ERR_INVALID;
+    const size_t ncoef = (size_t)n_views * psf_size * psf_size;
+    for (size_t k = 0; k < ncoef; ++k)
+        if (!isfinite(psfs[k]) || psfs[k] < 0.f) return MVD_ERR_INVALID;
+    if (path != MVD_PATH_AUTO && path != MVD_PATH_DIRECT && path != MVD_PATH_FFT) return MVD_ERR_INVALID;
+    if (path == MVD_PATH_AUTO) {
+        path = choose_path(plane_w, plane_h, psf_size);
+        if (path < 0) return MVD_ERR_UNSUPPORTED;
+    } else if (!mvd_path_supported(path, plane_w, plane_h, psf_size)) {
+        return MVD_ERR_UNSUPPORTED;
+    }
+
+    mvd_handle* h = new (std::nothrow) mvd_handle();
+    if (!h) return MVD_ERR_NOMEM;
+    h->W = plane_w; h->H = plane_h; h->V = n_views; h->K = psf_size; h->T = iterations;
+    h->eps = eps; h->path = path;
+    int rc = mvd_check(h, cudaGetDevice(&h->device));
+    if (rc == MVD_OK) rc = mvd_check(h, cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device));
+    if (rc == MVD_OK) rc = path == MVD_PATH_FFT ? fft_setup(h, psfs) : direct_setup(h, psfs);
+    if (rc != MVD_OK) {
+        // keep the cuda error visible to the caller through the return code only
+        mvd_destroy(h);
+        return rc;
+    }
+    *out = h;
+    return MVD_OK;
+}
+
+int mvd_create(int plane_w, int plane_h, int n_views, const float* psfs, int psf_size,
+               int iterations, float eps, mvd_handle** out) {
+    int path = MVD_PATH_AUTO;
+    const char* f = getenv("MVD_FORCE_PATH");
+    if (f && !strcmp(f, "direct")) path = MVD_PATH_DIRECT;
+    else if (f && !strcmp(f, "fft")) path = MVD_PATH_FFT;
+    return mvd_create_path(plane_w, plane_h, n_views, psfs, psf_size, iterations, eps, path, out);
+}
+
+void mvd_destroy(mvd_handle* h) {
+    if (!h) return;
+    cudaDeviceSynchronize();
+    for (auto& r : h->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
+    for (auto& e : h->event_pool) cudaEventDestroy(e);
+    ws_free(h->ws_main);
+    for (int s = 0; s < mvd_handle::kSlots; ++s) {
+        ws_free(h->ws_slot[s]);
+        if (h->d_in[s]) cudaFree(h->d_in[s]);
+        if (h->d_out[s]) cudaFree(h->d_out[s]);
+        if (h->streams[s]) cudaStreamDestroy(h->streams[s]);
+    }
+    if (h->d_coef) cudaFree(h->d_coef);
+    if (h->d_otf) cudaFree(h->d_otf);
+    (void)cudaGetLastError();
+    delete h;
+}
+
+// ---------------------------------------------------------------------------------------------
+// compute
+// ---------------------------------------------------------------------------------------------
+static int default_chunk(const mvd_handle* h) {
+    if (h->chunk_planes > 0) return h->chunk_planes;
+    if (h->path == MVD_PATH_FFT) return fft_default_chunk(h);
+    // direct: bound the scratch (one fp32 plane per plane) to ~1 GiB
+    const size_t npx = (size_t)h->W * h->H;
+    size_t c = ((size_t)1 << 30) / (npx * sizeof(float));
+    return (int)std::max<size_t>(1, std::min<size_t>(c, 1 << 20));
+}
+
+// All T iterations on planes [0, n) of `views`, in chunks (each chunk runs to completion).
+static int run_core(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_stride,
+                    float* out, int n_planes, cudaStream_t stream) {
+    const size_t npx = (size_t)h->W * h->H;
+    const int chunk = default_chunk(h);
+    for (int p0 = 0; p0 < n_planes; p0 += chunk) {
+        const int n = std::min(chunk, n_planes - p0);
+        int rc = h->path == MVD_PATH_FFT
+                     ? fft_run(h, ws, views + (size_t)p0 * npx, view_stride, out + (size_t)p0 * npx, n, stream)
+                     : direct_run(h, ws, views + (size_t)p0 * npx, view_stride, out + (size_t)p0 * npx, n, stream);
+        if (rc != MVD_OK) return rc;
+    }
+    return MVD_OK;
+}
+
+int mvd_deconvolve_planes(mvd_handle* h, const uint16_t* dev_views_u16, float* dev_out_f32,
+                          int n_planes, void* stream) {
+    if (!h || n_planes < 0) return MVD_ERR_INVALID;
+    if (n_planes == 0) return MVD_OK;
+    if (!dev_views_u16 || !dev_out_f32) return MVD_ERR_INVALID;
+    const size_t npx = (size_t)h->W * h->H;
+    return run_core(h, h->ws_main, dev_views_u16, (size_t)n_planes * npx, dev_out_f32, n_planes,
+                    (cudaStream_t)stream);
+}
+
+static int default_batch(const mvd_handle* h, int n_planes) {
+    if (h->batch_planes > 0) return std::min(h->batch_planes, n_planes);
+    // ~64 MiB of uint16 input per batch, at least 12 batches when the stack allows it so that the
+    // pipeline's fill and drain (one H2D and one D2H that overlap nothing) stay a few percent
+    const size_t per_plane = (size_t)h->W * h->H * sizeof(uint16_t) * h->V;
+    size_t b = std::max<size_t>(1, ((size_t)64 << 20) / per_plane);
+    b = std::min<size_t>(b, std::max(1, n_planes / 12));
+    if (h->path == MVD_PATH_FFT && b > 1) b &= ~(size_t)1;   // plane pairs
+    return (int)std::max<size_t>(1, std::min<size_t>(b, (size_t)n_planes));
+}
+
+int mvd_deconvolve_host(mvd_handle* h, const uint16_t* host_views_u16, float* host_out_f32,
+                        int n_planes) {
+    if (!h || n_planes < 0) return MVD_ERR_INVALID;
+    if (n_planes == 0) return MVD_OK;
+    if (!host_views_u16 || !host_out_f32) return MVD_ERR_INVALID;
+    const size_t npx = (size_t)h->W * h->H;
+    const int B = default_batch(h, n_planes);
+
+    for (int s = 0; s < mvd_handle::kSlots; ++s)
+        if (!h->streams[s]) MVD_TRY(h, cudaStreamCreateWithFlags(&h->streams[s], cudaStreamNonBlocking));
+    if ((size_t)B > h->slot_planes) {
+        MVD_TRY(h, cudaDeviceSynchronize());
+        for (int s = 0; s < mvd_handle::kSlots; ++s) {
+            if (h->d_in[s]) { cudaFree(h->d_in[s]); h->d_in[s] = nullptr; }
+            if (h->d_out[s]) { cudaFree(h->d_out[s]); h->d_out[s] = nullptr; }
+        }
+        h->slot_planes = 0;
+        for (int s = 0; s < mvd_handle::kSlots; ++s) {
+            MVD_TRY(h, cudaMalloc((void**)&h->d_in[s], sizeof(uint16_t) * npx * B * h->V));
+            MVD_TRY(h, cudaMalloc((void**)&h->d_out[s], sizeof(float) * npx * B));
+        }
+        h->slot_planes = (size_t)B;
+    }
+
+    // Algorithm 1 with batches of planes instead of single planes and pinned
+    // host memory instead of disk: batch k goes to stream k mod 3; within a stream H2D, the RL
+    // steps and D2H are ordered, across streams they overlap.  Nothing blocks until the end.
+    int rc = MVD_OK;
+    int k = 0;
+    for (int p0 = 0; p0 < n_planes && rc == MVD_OK; p0 += B, ++k) {
+        const int s = k % mvd_handle::kSlots;
+        const int n = std::min(B, n_planes - p0);
+        cudaStream_t st = h->streams[s];
+        for (int v = 0; v < h->V && rc == MVD_OK; ++v)
+            rc = mvd_check(h, cudaMemcpyAsync(h->d_in[s] + (size_t)v * B * npx,
+                                             host_views_u16 + ((size_t)v * n_planes + p0) * npx,
+                                             sizeof(uint16_t) * npx * n, cudaMemcpyHostToDevice, st));
+        if (rc == MVD_OK) rc = run_core(h, h->ws_slot[s], h->d_in[s], (size_t)B * npx, h->d_out[s], n, st);
+        if (rc == MVD_OK)
+            rc = mvd_check(h, cudaMemcpyAsync(host_out_f32 + (size_t)p0 * npx, h->d_out[s],
+                                             sizeof(float) * npx * n, cudaMemcpyDeviceToHost, st));
+    }
+    for (int s = 0; s < mvd_handle::kSlots; ++s) {
+        int rs = mvd_check(h, cudaStreamSynchronize(h->streams[s]));
+        if (rc == MVD_OK) rc = rs;
+    }
+    return rc;
+}
+
+// ---------------------------------------------------------------------------------------------
+// small accessors
+// ---------------------------------------------------------------------------------------------
+const char* mvd_strerror(int code) {
+    switch (code) {
+        case MVD_OK: return "ok";
+        case MVD_ERR_INVALID: return "invalid argument";
+        case MVD_ERR_UNSUPPORTED: return "shape not supported by the requested path";
+        case MVD_ERR_CUDA: return "CUDA error (see mvd_last_cuda_error)";
+        case MVD_ERR_NOMEM: return "out of device or pinned memory";
+        case MVD_ERR_BUSY: return "handle busy";
+        default: return "unknown mvd error code";
+    }
+}
+
+int mvd_last_cuda_error(const mvd_handle* h) { return h ? h->last_cuda : 0; }
+int mvd_get_path(const mvd_handle* h) { return h ? h->path : MVD_ERR_INVALID; }
+
+int mvd_set_chunk_planes(mvd_handle* h, int planes) {
+    if (!h || planes < 0) return MVD_ERR_INVALID;
+    h->chunk_planes = planes;
+    return MVD_OK;
+}
+
+int mvd_set_batch_planes(mvd_handle* h, int planes) {
+    if (!h || planes < 0) return MVD_ERR_INVALID;
+    h->batch_planes = planes;
+    return MVD_OK;
+}
+
+long long mvd_launch_count(const mvd_handle* h) { return h ? h->launches : 0; }
+void mvd_launch_count_reset(mvd_handle* h) { if (h) h->launches = 0; }
+
+int mvd_profile_enable(mvd_handle* h, int on) {
+    if (!h) return MVD_ERR_INVALID;
+    h->profiling = on != 0;
+    return MVD_OK;
+}
+
+int mvd_profile_read(mvd_handle* h, float* ms, long long* n) {
+    if (!h || !ms || !n) return MVD_ERR_INVALID;
+    for (int k = 0; k < MVD_N_KERNEL_CLASSES; ++k) { ms[k] = 0.f; n[k] = 0; }
+    int rc = MVD_OK;
+    for (auto& r : h->prof) {
+        float t = 0.f;
+        cudaError_t e = cudaEventSynchronize(r.e1);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&t, r.e0, r.e1);
+        if (e != cudaSuccess) rc = mvd_check(h, e);
+        else if (r.kc >= 0 && r.kc < MVD_N_KERNEL_CLASSES) { ms[r.kc] += t; n[r.kc]++; }
+        h->event_pool.push_back(r.e0);
+        h->event_pool.push_back(r.e1);
+    }
+    h->prof.clear();
+    return rc;
+}
+
+const char* mvd_kernel_class_name(int k) {
+    static const char* names[MVD_N_KERNEL_CLASSES] = {
+        "init_mean", "direct_blur_ratio", "direct_backproject_update", "fft_rows_first",
+        "fft_cols_otf", "fft_rows_ratio", "fft_rows_update", "setup"};
+    return (k >= 0 && k < MVD_N_KERNEL_CLASSES) ? names[k] : nullptr;
+}
+
+const char* mvd_version(void) { return "mvd 0.1 sm_100a"; }

@@ -1,0 +1,103 @@
+// mvd_internal.cuh -- shared declarations of libmvd's translation units (not part of the C ABI).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <vector>
+
+#include "../../include/mvd.h"
+
+// Kernel classes for mvd_profile_read / bench.py's roofline line.
+enum KernelClass {
+    KC_INIT_MEAN = 0,        // a0: psi_0 = mean of the views (direct path)
+    KC_DIRECT_BLUR_RATIO,    // a1+a2: b = psi (*) P_v, r = phi_v / max(b, eps)
+    KC_DIRECT_BACK_UPDATE,   // a3+a4: q = r (*) P_v^*, psi *= q
+    KC_FFT_ROWS_FIRST,       // a0 + forward row FFT of psi_0
+    KC_FFT_COLS,             // column FFT . OTF . inverse column FFT (a1 / a3 middle part)
+    KC_FFT_ROWS_RATIO,       // inverse row FFT -> b, a2 ratio, forward row FFT of r
+    KC_FFT_ROWS_UPDATE,      // inverse row FFT -> q, a4 update, forward row FFT of the new psi
+    KC_SETUP                 // mvd_create-time kernels (OTF construction)
+};
+static_assert(KC_SETUP + 1 == MVD_N_KERNEL_CLASSES, "kernel class table and mvd.h disagree");
+
+struct ProfRecord {
+    int kc;
+    cudaEvent_t e0, e1;
+};
+
+// Per-stream working memory.  Grown on demand, freed in mvd_destroy.
+struct Workspace {
+    float* a = nullptr;      // direct: r [chunk][H][W];   fft: Z (psi pairs, float2 [pairs][H][W])
+    float* b = nullptr;      // direct: unused;            fft: S (spectrum, float2 [pairs][H][W])
+    size_t a_bytes = 0, b_bytes = 0;
+};
+
+struct mvd_handle {
+    int W = 0, H = 0, V = 0, K = 0, T = 0;
+    float eps = 0.f;
+    int path = MVD_PATH_DIRECT;
+    int device = 0;
+    int n_sm = 148;
+
+    // direct path: per view two coefficient arrays, transposed and row-padded: G[v][which][K][Kp]
+    // which = 0: blur (flipped PSF), 1: back-projection (PSF as given)
+    float* d_coef = nullptr;
+    int Kp = 0;   // padded number of PSF rows (multiple of the kernel's row chunk)
+    int JC = 0;   // row chunk of the direct kernel chosen for K
+
+    // fft path: optical transfer functions, float2 [V][H][W], pre-scaled by 1/(W*H)
+    float2* d_otf = nullptr;
+
+    Workspace ws_main;
+    // host pipeline (mvd_deconvolve_host): three slots, one stream each
+    static constexpr int kSlots = 3;
+    cudaStream_t streams[kSlots] = {nullptr, nullptr, nullptr};
+    Workspace ws_slot[kSlots];
+    uint16_t* d_in[kSlots] = {nullptr, nullptr, nullptr};
+    float* d_out[kSlots] = {nullptr, nullptr, nullptr};
+    size_t slot_planes = 0;
+
+    int chunk_planes = 0;   // 0 = default
+    int batch_planes = 0;   // 0 = default
+
+    int last_cuda = 0;
+    long long launches = 0;
+    bool profiling = false;
+    std::vector<ProfRecord> prof;
+    std::vector<cudaEvent_t> event_pool;
+};
+
+// Bracket a kernel launch: counts it and, when profiling, records events on `stream`.
+struct LaunchScope {
+    mvd_handle* h;
+    cudaStream_t stream;
+    cudaEvent_t e1 = nullptr;
+    LaunchScope(mvd_handle* h_, int kc, cudaStream_t s);
+    ~LaunchScope();
+};
+
+// Returns MVD_OK or records the CUDA error in h and returns MVD_ERR_CUDA / MVD_ERR_NOMEM.
+int mvd_check(mvd_handle* h, cudaError_t e);
+#define MVD_TRY(h, expr)                        \
+    do {                                        \
+        int rc__ = mvd_check((h), (expr));      \
+        if (rc__ != MVD_OK) return rc__;        \
+    } while (0)
+
+int ws_reserve(mvd_handle* h, Workspace& ws, size_t a_bytes, size_t b_bytes);
+
+// ---- direct path (mvd_direct.cu) ------------------------------------------------------------
+int direct_choose_chunk(int K, int* JC, int* Kp);
+int direct_setup(mvd_handle* h, const float* host_psfs);
+size_t direct_scratch_bytes(const mvd_handle* h, int n_planes);
+// views: view v of plane p at views + (v * view_stride + p * H * W); out: [n][H][W]
+int direct_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_stride, float* out,
+               int n_planes, cudaStream_t stream);
+
+// ---- fft path (mvd_fft.cu) --------------------------------------------------------------------
+int fft_supported(int W, int H);
+int fft_setup(mvd_handle* h, const float* host_psfs);
+int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_stride, float* out,
+            int n_planes, cudaStream_t stream);
+int fft_default_chunk(const mvd_handle* h);

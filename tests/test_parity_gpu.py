@@ -1,0 +1,226 @@
+"""GPU-vs-oracle parity, through the C ABI (binding -> libmvd.so).  Run with -m gpu on the B200 box.
+
+Element-by-element comparison on the same seeded inputs; tolerance per north_star (parity_util).
+Integer / exact work (uint16 ingest, iterations = 0, delta PSFs, chunking, host pipeline) is bit-exact.
+Every case runs on both engines where the engine supports the shape.
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+from oracle import mvd_oracle
+from paper_1503_07998_b200 import binding, build, synth
+from parity_util import assert_parity
+
+pytestmark = pytest.mark.gpu
+
+PATHS = [binding.PATH_DIRECT, binding.PATH_FFT]
+GOLDEN = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+
+
+@pytest.fixture(scope="module", autouse=True)
+def _lib():
+    build.build()
+    return binding.lib()
+
+
+def _need(path, W, H, K):
+    if not binding.path_supported(path, W, H, K):
+        pytest.skip(f"{binding.PATH_NAMES[path]} engine does not take {W}x{H} K={K}")
+
+
+def _run(views, psfs, T, path, **kw):
+    return binding.deconvolve(views, psfs, T, float(synth.EPS), path=path, **kw)
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE.json configs
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("path", PATHS)
+def test_config1_full_volume(path):
+    cfg = synth.config(1)
+    _need(path, cfg.W, cfg.H, cfg.K)
+    psfs, views = synth.config_psfs(1), synth.views(cfg)
+    ref = mvd_oracle.deconvolve(views, psfs, cfg.T, cfg.eps)
+    out = _run(views, psfs, cfg.T, path)
+    assert_parity(out, ref, f"config1 {binding.PATH_NAMES[path]}")
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_config2_plane_subset_full_size(path):
+    """Full-size 512x256 planes, K = 21, T = 10 (the bench workload's shape), oracle computed live."""
+    cfg = synth.config(2)
+    _need(path, cfg.W, cfg.H, cfg.K)
+    planes = [0, 255, 256, 511, 100, 37]
+    psfs, views = synth.config_psfs(2), synth.views(cfg, planes)
+    ref = mvd_oracle.deconvolve(views, psfs, cfg.T, cfg.eps)
+    out = _run(views, psfs, cfg.T, path)
+    assert_parity(out, ref, f"config2 {binding.PATH_NAMES[path]}")
+
+
+@pytest.mark.parametrize("cid", [3, 4, 5])
+def test_large_configs_against_stored_oracle_planes(cid):
+    """Configs 3-5 at full plane size against oracle planes stored by tests/golden/make_golden.py."""
+    fn = os.path.join(GOLDEN, f"config{cid}_samples.json")
+    if not os.path.exists(fn):
+        pytest.skip(f"{fn} not generated yet")
+    with open(fn) as f:
+        g = json.load(f)
+    cfg = synth.config(cid)
+    psfs = synth.config_psfs(cid)
+    planes = [rec["plane"] for rec in g["planes"]]
+    views = synth.views(cfg, planes, psfs)
+    for k, rec in enumerate(g["planes"]):   # the stored planes belong to exactly these inputs
+        assert [int(views[v, k].astype(np.int64).sum()) for v in range(cfg.V)] == rec["view_sums"]
+    out = binding.deconvolve(views, psfs, cfg.T, cfg.eps)   # the path mvd_create picks
+    for k, rec in enumerate(g["planes"]):
+        flat = out[k].astype(np.float64).ravel()
+        pos, val = np.array(rec["pos"]), np.array(rec["val"])
+        d = flat[pos] - val
+        rel_l2 = np.sqrt((d ** 2).sum() / (val ** 2).sum())
+        bright = val > 0.01 * rec["max"]
+        max_rel = (np.abs(d[bright]) / val[bright]).max()
+        assert rel_l2 <= 1e-4 and max_rel <= 1e-3, (cid, rec["plane"], rel_l2, max_rel)
+        assert abs(flat.sum() - rec["sum"]) <= 2e-5 * rec["sum"]
+        assert abs((flat ** 2).sum() - rec["sumsq"]) <= 2e-4 * rec["sumsq"]
+
+
+# ---------------------------------------------------------------------------------------------
+# Cases the configs lack: asymmetric PSFs (conv vs corr, flip, centre), ragged shapes, aliasing
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("V,N,W,H,K,T,psf", [
+    (3, 3, 96, 80, 7, 4, "random"),      # asymmetric, smooth sizes (both engines)
+    (2, 5, 160, 100, 13, 3, "random"),   # odd plane count; 100 = 2^2 5^2
+    (1, 2, 128, 64, 21, 5, "sparse"),    # templated K, single view
+    (2, 2, 200, 150, 31, 2, "random"),   # several tiles + ragged tail, 2-chunk PSF rows
+    (2, 1, 70, 50, 5, 6, "random"),      # W, H not multiples of anything useful
+    (4, 2, 60, 36, 9, 3, "gauss"),
+    (2, 2, 37, 23, 5, 3, "random"),      # primes: direct only
+    (2, 2, 192, 320, 51, 1, "random"),   # largest templated K, 3-chunk rows
+])
+def test_asymmetric_and_ragged(path, V, N, W, H, K, T, psf):
+    _need(path, W, H, K)
+    pr = synth.make_problem(V, N, W, H, K, T, seed=K * 1000 + W, psf=psf)
+    ref = mvd_oracle.deconvolve(pr.views, pr.psfs, T, pr.eps)
+    out = _run(pr.views, pr.psfs, T, path)
+    assert_parity(out, ref, f"{binding.PATH_NAMES[path]} {V}v {N}x{W}x{H} K{K} {psf}")
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_psf_larger_than_plane_aliases(path):
+    """K > W: taps alias around the plane (oracle pin P5 covers the same case against brute force)."""
+    V, N, W, H, K, T = 2, 2, 8, 12, 9, 3
+    _need(path, W, H, K)
+    rng = np.random.default_rng(5)
+    psfs = np.stack([synth.random_psf(K, rng) for _ in range(V)])
+    views = synth.random_views(V, N, W, H, seed=3, lo=50, hi=3000)
+    ref = mvd_oracle.deconvolve(views, psfs, T)
+    assert_parity(_run(views, psfs, T, path), ref, "aliasing")
+
+
+# ---------------------------------------------------------------------------------------------
+# Exact work
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("V", [1, 2, 4, 6])
+def test_zero_iterations_is_mean_of_views(path, V):
+    """A17 / P11: uint16 ingest is exact; the mean is bit-exact for V in {1,2,4}, 1 ulp for V = 6."""
+    W, H, N = 64, 32, 3
+    _need(path, W, H, 3)
+    views = synth.random_views(V, N, W, H, seed=V, lo=0, hi=65536)
+    psfs = np.stack([synth.delta_psf(3)] * V)
+    out = _run(views, psfs, 0, path)
+    want = (views.astype(np.float64).sum(axis=0) / V)
+    if V in (1, 2, 4):
+        assert np.array_equal(out, want.astype(np.float32))
+    else:
+        np.testing.assert_allclose(out, want, rtol=1.2e-7)
+    if V == 1:
+        assert np.array_equal(out.astype(np.uint16), views[0])   # ingest round-trips every uint16 value
+
+
+@pytest.mark.parametrize("T", [1, 3])
+def test_centred_delta_is_identity_direct(T):
+    """P1 on the direct engine: x/x = 1 and x*1 are exact in fp32, so psi == phi bit for bit."""
+    W, H, N, K = 64, 48, 2, 5
+    views = synth.random_views(1, N, W, H, seed=11, lo=1, hi=60000)
+    out = _run(views, synth.delta_psf(K)[None], T, binding.PATH_DIRECT)
+    assert np.array_equal(out, views[0].astype(np.float32))
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("dz,dx", [(1, -2), (-2, 1)])
+def test_offcentre_delta_shifts_by_plus_d(path, dz, dx):
+    """P2 closed form: psi(x) = phi(x + d).  Swapping convolution and correlation gives phi(x - d)."""
+    W, H, N, K, T = 64, 32, 2, 5, 2
+    _need(path, W, H, K)
+    views = synth.random_views(1, N, W, H, seed=21, lo=100, hi=5000)
+    out = _run(views, synth.delta_psf(K, dz, dx)[None], T, path)
+    want = np.roll(views[0].astype(np.float64), shift=(-dz, -dx), axis=(1, 2))
+    np.testing.assert_allclose(out, want, rtol=2e-5)
+    assert not np.allclose(out, np.roll(views[0].astype(np.float64), shift=(dz, dx), axis=(1, 2)), rtol=1e-2)
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_chunking_and_host_pipeline_are_bit_identical(path):
+    """P12: planes are independent, so chunk size, batch size and the 3-stream pipeline change nothing."""
+    V, N, W, H, K, T = 2, 11, 96, 64, 7, 3
+    _need(path, W, H, K)
+    pr = synth.make_problem(V, N, W, H, K, T, seed=77)
+    base = _run(pr.views, pr.psfs, T, path)
+    assert np.array_equal(base, _run(pr.views, pr.psfs, T, path, chunk_planes=4))
+    assert np.array_equal(base, _run(pr.views, pr.psfs, T, path, host=True))
+    assert np.array_equal(base, _run(pr.views, pr.psfs, T, path, host=True, batch_planes=2, chunk_planes=2))
+    assert np.array_equal(base, _run(pr.views, pr.psfs, T, path, host=True, batch_planes=5))
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_sum_conservation_and_nonnegativity(path):
+    """P6 / P4 on the GPU output: sum(psi) = sum(phi_{V-1}) per plane, psi >= 0."""
+    cfg = synth.config(2).with_planes(4)
+    _need(path, cfg.W, cfg.H, cfg.K)
+    psfs, views = synth.config_psfs(2), synth.views(cfg, [3, 4, 5, 6])
+    out = _run(views, psfs, 3, path).astype(np.float64)
+    assert (out >= 0).all()
+    np.testing.assert_allclose(out.sum(axis=(1, 2)), views[-1].astype(np.float64).sum(axis=(1, 2)), rtol=2e-5)
+
+
+def test_single_plane_and_repeated_calls_on_one_handle():
+    import torch
+    pr = synth.make_problem(2, 3, 64, 64, 9, 2, seed=5)
+    ref = mvd_oracle.deconvolve(pr.views, pr.psfs, 2)
+    with binding.Mvd(64, 64, 2, pr.psfs, 9, 2) as m:
+        st = torch.cuda.Stream()
+        for n in (1, 3, 2, 3):     # scratch grows, shrinks, is reused
+            dv = torch.from_numpy(np.ascontiguousarray(pr.views[:, :n]).view(np.int16)).cuda()
+            do = torch.empty((n, 64, 64), dtype=torch.float32, device="cuda")
+            torch.cuda.synchronize()
+            m.deconvolve_planes(dv, do, n, st)
+            st.synchronize()
+            assert_parity(do.cpu().numpy(), ref[:n], f"n={n}")
+        assert m.launch_count() > 0
+        m.deconvolve_planes(dv, do, 0, st)       # no-op
+        with pytest.raises(binding.MvdError):
+            m.deconvolve_planes(None, do, 1, st)
+
+
+def test_profile_hooks_report_every_launch():
+    pr = synth.make_problem(2, 2, 64, 64, 9, 2, seed=6)
+    import torch
+    with binding.Mvd(64, 64, 2, pr.psfs, 9, 2) as m:
+        dv = torch.from_numpy(pr.views.view(np.int16)).cuda()
+        do = torch.empty((2, 64, 64), dtype=torch.float32, device="cuda")
+        m.profile_enable(True)
+        m.launch_count_reset()
+        m.deconvolve_planes(dv, do, 2)
+        prof = m.profile_read()
+        assert sum(n for _, n in prof.values()) == m.launch_count() > 0
+        assert all(ms >= 0 for ms, _ in prof.values())
+
+
+def test_fp32_peak_microbenchmark_is_plausible():
+    tf, mhz = binding.measure_fp32_peak()
+    assert 20.0 < tf < 120.0 and 500.0 < mhz < 3000.0
