@@ -154,6 +154,7 @@ void mvd_destroy(mvd_handle* h) {
     }
     if (h->d_coef) cudaFree(h->d_coef);
     if (h->d_otf) cudaFree(h->d_otf);
+    fft_teardown(h);
     (void)cudaGetLastError();
     delete h;
 }
@@ -161,8 +162,12 @@ void mvd_destroy(mvd_handle* h) {
 // ---------------------------------------------------------------------------------------------
 // compute
 // ---------------------------------------------------------------------------------------------
+// The FFT engine packs planes (2m, 2m+1) into one complex plane; chunks and batches start on even
+// planes so that the pairing -- and with it every output bit -- does not depend on the chunking.
+static int even_up(int n) { return n + (n & 1); }
+
 static int default_chunk(const mvd_handle* h) {
-    if (h->chunk_planes > 0) return h->chunk_planes;
+    if (h->chunk_planes > 0) return h->path == MVD_PATH_FFT ? even_up(h->chunk_planes) : h->chunk_planes;
     if (h->path == MVD_PATH_FFT) return fft_default_chunk(h);
     // direct: bound the scratch (one fp32 plane per plane) to ~1 GiB
     const size_t npx = (size_t)h->W * h->H;
@@ -196,14 +201,15 @@ int mvd_deconvolve_planes(mvd_handle* h, const uint16_t* dev_views_u16, float* d
 }
 
 static int default_batch(const mvd_handle* h, int n_planes) {
-    if (h->batch_planes > 0) return std::min(h->batch_planes, n_planes);
+    if (h->batch_planes > 0)
+        return h->path == MVD_PATH_FFT ? even_up(h->batch_planes) : std::min(h->batch_planes, n_planes);
     // ~64 MiB of uint16 input per batch, at least 12 batches when the stack allows it so that the
     // pipeline's fill and drain (one H2D and one D2H that overlap nothing) stay a few percent
     const size_t per_plane = (size_t)h->W * h->H * sizeof(uint16_t) * h->V;
     size_t b = std::max<size_t>(1, ((size_t)64 << 20) / per_plane);
     b = std::min<size_t>(b, std::max(1, n_planes / 12));
-    if (h->path == MVD_PATH_FFT && b > 1) b &= ~(size_t)1;   // plane pairs
-    return (int)std::max<size_t>(1, std::min<size_t>(b, (size_t)n_planes));
+    b = std::max<size_t>(1, std::min<size_t>(b, (size_t)n_planes));
+    return h->path == MVD_PATH_FFT ? even_up((int)b) : (int)b;
 }
 
 int mvd_deconvolve_host(mvd_handle* h, const uint16_t* host_views_u16, float* host_out_f32,

@@ -1,7 +1,236 @@
-// mvd_fft.cu -- FFT engine of libmvd (placeholder until the kernels land).
+// mvd_fft.cu -- host side of the FFT engine: supported lengths, twiddle tables, optical transfer
+// functions, and the launch sequence of one chunk of planes (see mvd_fft_kernels.cuh for the kernels).
+#include <math.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "mvd_fft_kernels.cuh"
 #include "mvd_internal.cuh"
 
-int fft_supported(int, int) { return 0; }
-int fft_setup(mvd_handle*, const float*) { return MVD_ERR_UNSUPPORTED; }
-int fft_run(mvd_handle*, Workspace&, const uint16_t*, size_t, float*, int, cudaStream_t) { return MVD_ERR_UNSUPPORTED; }
-int fft_default_chunk(const mvd_handle*) { return 1; }
+using mvdfft::PlanInfo;
+using mvdfft::RowArgs;
+using mvdfft::SizeOps;
+
+namespace {
+
+const SizeOps* find_ops(int N) {
+    if (const SizeOps* o = mvd_fft_ops_small(N)) return o;
+    if (const SizeOps* o = mvd_fft_ops_mid(N)) return o;
+    return mvd_fft_ops_large(N);
+}
+
+// Per-thread twiddles of a plan, [(s-1) E + e][TPF], s >= 1:
+//   element e of thread t in stage s belongs to butterfly j = t + u TPF, input m  (e = u + m E/R),
+//   and is multiplied by exp(-2 pi i m k / (Ns R)),  k = j mod Ns  (inverse transforms conjugate it).
+std::vector<float2> make_twiddles(int N, const PlanInfo& p) {
+    std::vector<float2> tw((size_t)std::max(p.S - 1, 0) * p.E * p.TPF);
+    int Ns = p.radices[0];
+    for (int s = 1; s < p.S; ++s) {
+        const int R = p.radices[s], NB = p.E / R;
+        for (int e = 0; e < p.E; ++e) {
+            const int u = e % NB, m = e / NB;
+            for (int t = 0; t < p.TPF; ++t) {
+                const int j = t + u * p.TPF, k = j % Ns;
+                const double ang = -2.0 * M_PI * (double)((long long)m * k) / (double)((long long)Ns * R);
+                tw[((size_t)(s - 1) * p.E + e) * p.TPF + t] = make_float2((float)cos(ang), (float)sin(ang));
+            }
+        }
+        Ns *= R;
+    }
+    (void)N;
+    return tw;
+}
+
+// OTF, phase 1: G[j][kx] = sum_i P[j][i] exp(-2 pi i kx (i - c) / W)        (fp64)
+__global__ void otf_rows_kernel(const float* __restrict__ P, int K, int W, double2* __restrict__ G) {
+    const int kx = blockIdx.x * blockDim.x + threadIdx.x, j = blockIdx.y;
+    if (kx >= W) return;
+    const int c = (K - 1) / 2;
+    double re = 0.0, im = 0.0;
+    for (int i = 0; i < K; ++i) {
+        long long ph = ((long long)kx * (i - c)) % W;
+        if (ph < 0) ph += W;
+        double s, co;
+        sincospi(-2.0 * (double)ph / (double)W, &s, &co);
+        const double p = (double)P[j * K + i];
+        re += p * co;
+        im += p * s;
+    }
+    G[(size_t)j * W + kx] = make_double2(re, im);
+}
+
+// OTF, phase 2: O[ky][kx] = (1 / (W H)) sum_j G[j][kx] exp(-2 pi i ky (j - c) / H)   -> fp32
+__global__ void otf_cols_kernel(const double2* __restrict__ G, int K, int W, int H, float2* __restrict__ O) {
+    const int kx = blockIdx.x * blockDim.x + threadIdx.x, ky = blockIdx.y;
+    if (kx >= W) return;
+    const int c = (K - 1) / 2;
+    double re = 0.0, im = 0.0;
+    for (int j = 0; j < K; ++j) {
+        long long ph = ((long long)ky * (j - c)) % H;
+        if (ph < 0) ph += H;
+        double s, co;
+        sincospi(-2.0 * (double)ph / (double)H, &s, &co);
+        const double2 g = G[(size_t)j * W + kx];
+        re += g.x * co - g.y * s;
+        im += g.x * s + g.y * co;
+    }
+    const double sc = 1.0 / ((double)W * (double)H);
+    O[(size_t)ky * W + kx] = make_float2((float)(re * sc), (float)(im * sc));
+}
+
+struct FftState {
+    const SizeOps* row = nullptr;   // length W
+    const SizeOps* col = nullptr;   // length H
+    float2* tw_row = nullptr;
+    float2* tw_col = nullptr;
+};
+
+FftState* state_of(const mvd_handle* h) { return static_cast<FftState*>(h->fft); }
+
+}  // namespace
+
+int fft_supported(int W, int H) {
+    const SizeOps* r = find_ops(W);
+    const SizeOps* c = find_ops(H);
+    if (!r || !c) return 0;
+    if (W % c->col_tc != 0) return 0;
+    return 1;
+}
+
+void fft_teardown(mvd_handle* h) {
+    FftState* st = state_of(h);
+    if (!st) return;
+    if (st->tw_row) cudaFree(st->tw_row);
+    if (st->tw_col) cudaFree(st->tw_col);
+    delete st;
+    h->fft = nullptr;
+}
+
+int fft_setup(mvd_handle* h, const float* host_psfs) {
+    if (!fft_supported(h->W, h->H)) return MVD_ERR_UNSUPPORTED;
+    FftState st;
+    st.row = find_ops(h->W);
+    st.col = find_ops(h->H);
+    MVD_TRY(h, st.row->prepare());
+    MVD_TRY(h, st.col->prepare());
+
+    auto upload = [&](const std::vector<float2>& v, float2** d) -> int {
+        const size_t bytes = std::max<size_t>(v.size(), 1) * sizeof(float2);
+        MVD_TRY(h, cudaMalloc((void**)d, bytes));
+        if (!v.empty()) MVD_TRY(h, cudaMemcpy(*d, v.data(), v.size() * sizeof(float2), cudaMemcpyHostToDevice));
+        return MVD_OK;
+    };
+    int rc = upload(make_twiddles(h->W, st.row->row), &st.tw_row);
+    if (rc == MVD_OK) rc = upload(make_twiddles(h->H, st.col->col), &st.tw_col);
+    if (rc != MVD_OK) {
+        if (st.tw_row) cudaFree(st.tw_row);
+        if (st.tw_col) cudaFree(st.tw_col);
+        return rc;
+    }
+    h->fft = new FftState(st);
+
+    // optical transfer functions
+    const int K = h->K, W = h->W, H = h->H;
+    const size_t npx = (size_t)W * H;
+    float* d_psf = nullptr;
+    double2* d_G = nullptr;
+    MVD_TRY(h, cudaMalloc((void**)&h->d_otf, sizeof(float2) * npx * h->V));
+    MVD_TRY(h, cudaMalloc((void**)&d_psf, sizeof(float) * (size_t)h->V * K * K));
+    rc = mvd_check(h, cudaMalloc((void**)&d_G, sizeof(double2) * (size_t)K * W));
+    if (rc == MVD_OK)
+        rc = mvd_check(h, cudaMemcpy(d_psf, host_psfs, sizeof(float) * (size_t)h->V * K * K, cudaMemcpyHostToDevice));
+    for (int v = 0; v < h->V && rc == MVD_OK; ++v) {
+        const dim3 block(128), g1((W + 127) / 128, K), g2((W + 127) / 128, H);
+        {
+            LaunchScope ls(h, KC_SETUP, 0);
+            otf_rows_kernel<<<g1, block>>>(d_psf + (size_t)v * K * K, K, W, d_G);
+        }
+        {
+            LaunchScope ls(h, KC_SETUP, 0);
+            otf_cols_kernel<<<g2, block>>>(d_G, K, W, H, h->d_otf + (size_t)v * npx);
+        }
+        rc = mvd_check(h, cudaGetLastError());
+    }
+    if (rc == MVD_OK) rc = mvd_check(h, cudaDeviceSynchronize());
+    if (d_psf) cudaFree(d_psf);
+    if (d_G) cudaFree(d_G);
+    h->launches = 0;
+    return rc;
+}
+
+// Planes per internal pass: bound the two scratch buffers (8 B per voxel) to about 1 GiB.
+int fft_default_chunk(const mvd_handle* h) {
+    const size_t npx = (size_t)h->W * h->H;
+    size_t c = ((size_t)1 << 30) / (npx * 8);
+    c = std::max<size_t>(2, std::min<size_t>(c, 1 << 20));
+    return (int)(c & ~(size_t)1);
+}
+
+int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_stride, float* out,
+            int n_planes, cudaStream_t stream) {
+    FftState* st = state_of(h);
+    if (!st) return MVD_ERR_INVALID;
+    const int W = h->W, H = h->H;
+    const int pairs = (n_planes + 1) / 2;
+    const size_t bytes = sizeof(float2) * (size_t)pairs * H * W;
+    int rc = ws_reserve(h, ws, bytes, bytes);
+    if (rc != MVD_OK) return rc;
+
+    RowArgs a;
+    a.Z = (float2*)ws.a;
+    a.S = (float2*)ws.b;
+    a.views = views;
+    a.view_stride = view_stride;
+    a.out = out;
+    a.n_planes = n_planes;
+    a.H = H;
+    a.V = h->V;
+    a.v = 0;
+    a.eps = h->eps;
+    a.final = 0;
+    a.total_rows = pairs * H;
+
+    const int rp = st->row->row_threads / st->row->row.TPF;          // rows per CTA pass
+    const int row_ctas = (a.total_rows + rp - 1) / rp;
+    const int row_grid = std::max(1, std::min(row_ctas, h->n_sm * 16));
+    const int tiles = W / st->col->col_tc;
+    const int per_tile = std::max(1, (h->n_sm * 8 + tiles - 1) / tiles);
+    const dim3 col_grid(tiles, std::min(pairs, per_tile));
+    const size_t npx = (size_t)W * H;
+
+    {
+        LaunchScope ls(h, KC_FFT_ROWS_FIRST, stream);
+        a.final = h->T == 0;
+        rc = mvd_check(h, st->row->rows(mvdfft::ROWS_FIRST, a, st->tw_row, row_grid, stream));
+    }
+    if (rc != MVD_OK) return rc;
+    for (int t = 0; t < h->T; ++t)
+        for (int v = 0; v < h->V; ++v) {
+            const float2* otf = h->d_otf + (size_t)v * npx;
+            {
+                LaunchScope ls(h, KC_FFT_COLS, stream);
+                rc = mvd_check(h, st->col->cols(a.S, otf, 0, pairs, W, st->tw_col, col_grid, stream));   // a1
+            }
+            if (rc != MVD_OK) return rc;
+            {
+                LaunchScope ls(h, KC_FFT_ROWS_RATIO, stream);
+                a.v = v;
+                a.final = 0;
+                rc = mvd_check(h, st->row->rows(mvdfft::ROWS_RATIO, a, st->tw_row, row_grid, stream));   // a2
+            }
+            if (rc != MVD_OK) return rc;
+            {
+                LaunchScope ls(h, KC_FFT_COLS, stream);
+                rc = mvd_check(h, st->col->cols(a.S, otf, 1, pairs, W, st->tw_col, col_grid, stream));   // a3
+            }
+            if (rc != MVD_OK) return rc;
+            {
+                LaunchScope ls(h, KC_FFT_ROWS_UPDATE, stream);
+                a.final = (t == h->T - 1 && v == h->V - 1);
+                rc = mvd_check(h, st->row->rows(mvdfft::ROWS_UPDATE, a, st->tw_row, row_grid, stream));  // a4
+            }
+            if (rc != MVD_OK) return rc;
+        }
+    return MVD_OK;
+}

@@ -1,0 +1,513 @@
+// mvd_fft_kernels.cuh -- hand-written batched FFT convolution kernels of libmvd's FFT engine (sm_100a).
+//
+// Two planes are packed into one complex plane, z = psi_a + i psi_b.  Convolution with a REAL kernel
+// is linear and real, so  z (*) P = (psi_a (*) P) + i (psi_b (*) P):  one complex 2D FFT serves two
+// planes, no real-FFT post-processing, no Hermitian bookkeeping.  With X = FFT2(z) and the optical
+// transfer function O_v = FFT2(P_v embedded with its centre at the origin) / (W H):
+//     a1  b = IFFT2(X . O_v)              (periodic convolution,  PAPER.md:79  "psi * P_v")
+//     a3  q = IFFT2(FFT2(r) . conj O_v)   (periodic correlation,  PAPER.md:79, :118  "* P_v^*", P real)
+// The 2D transforms are split into row passes (x, contiguous) and column passes (z, strided), and the
+// pointwise steps are fused into them:
+//     rows_first   a0: psi_0 = mean_v phi_v -> Z;  row FFT -> S
+//     cols         column FFT, . O_v (or conj O_v), inverse column FFT          S -> S   (twice per view update)
+//     rows_ratio   inverse row FFT -> b;  a2: r = phi_v / max(b, eps);  row FFT  S -> S
+//     rows_update  inverse row FFT -> q;  a4: psi <- psi . q  (Z, or the output after the last update);
+//                  row FFT of the new psi -> S
+//
+// One FFT of length N = R0 R1 ... is a Stockham autosort: every thread keeps E elements in registers,
+// element e of thread t being position t + TPF e (TPF = N / E threads per FFT) -- the layout every
+// stage reads, and the layout the last stage leaves its results in, so global loads, the pointwise
+// steps and global stores all use it directly and only S-1 exchanges per FFT go through shared memory.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace mvdfft {
+
+// ---------------------------------------------------------------------------------------------
+// complex arithmetic on packed f32x2 (SASS FADD2 / FMUL2 / FFMA2 on sm_100a)
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float2 add2(float2 a, float2 b) {
+    float2 r;
+    asm("{ .reg .b64 ra, rb, rc; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; add.rn.f32x2 rc, ra, rb; "
+        "mov.b64 {%0,%1}, rc; }" : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+__device__ __forceinline__ float2 sub2(float2 a, float2 b) {
+    float2 r;
+    asm("{ .reg .b64 ra, rb, rc; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; sub.rn.f32x2 rc, ra, rb; "
+        "mov.b64 {%0,%1}, rc; }" : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+__device__ __forceinline__ float2 mul2(float2 a, float2 b) {
+    float2 r;
+    asm("{ .reg .b64 ra, rb, rc; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; mul.rn.f32x2 rc, ra, rb; "
+        "mov.b64 {%0,%1}, rc; }" : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y));
+    return r;
+}
+__device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
+    float2 r;
+    asm("{ .reg .b64 ra, rb, rc, rd; mov.b64 ra, {%2,%3}; mov.b64 rb, {%4,%5}; mov.b64 rc, {%6,%7}; "
+        "fma.rn.f32x2 rd, ra, rb, rc; mov.b64 {%0,%1}, rd; }"
+        : "=f"(r.x), "=f"(r.y) : "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y), "f"(c.x), "f"(c.y));
+    return r;
+}
+__device__ __forceinline__ float2 scale2(float2 a, float s) { return mul2(a, make_float2(s, s)); }
+// a * w
+__device__ __forceinline__ float2 cmul(float2 a, float2 w) {
+    return fma2(make_float2(a.y, a.y), make_float2(-w.y, w.x), mul2(make_float2(a.x, a.x), w));
+}
+// a * conj(w)
+__device__ __forceinline__ float2 cmulc(float2 a, float2 w) {
+    return fma2(make_float2(a.y, a.y), make_float2(w.y, w.x), mul2(make_float2(a.x, a.x), make_float2(w.x, -w.y)));
+}
+// a * (-i) for the forward transform (DIR < 0), a * (+i) for the inverse
+template <int DIR>
+__device__ __forceinline__ float2 rot90(float2 a) {
+    return DIR < 0 ? make_float2(a.y, -a.x) : make_float2(-a.y, a.x);
+}
+
+// ---------------------------------------------------------------------------------------------
+// in-register DFTs, natural order in and out: v[q] <- sum_m v[m] exp(DIR 2 pi i m q / R)
+// ---------------------------------------------------------------------------------------------
+template <int R, int DIR>
+struct Bfly;
+
+template <int DIR>
+struct Bfly<2, DIR> {
+    static __device__ __forceinline__ void run(float2* v) {
+        const float2 a = v[0];
+        v[0] = add2(a, v[1]);
+        v[1] = sub2(a, v[1]);
+    }
+};
+
+template <int DIR>
+struct Bfly<3, DIR> {
+    static __device__ __forceinline__ void run(float2* v) {
+        const float2 t1 = add2(v[1], v[2]);
+        const float2 m = fma2(t1, make_float2(-0.5f, -0.5f), v[0]);
+        const float2 s = rot90<DIR>(scale2(sub2(v[1], v[2]), 0.86602540378443864676f));
+        v[0] = add2(v[0], t1);
+        v[1] = add2(m, s);
+        v[2] = sub2(m, s);
+    }
+};
+
+template <int DIR>
+struct Bfly<4, DIR> {
+    static __device__ __forceinline__ void run(float2* v) {
+        const float2 a0 = add2(v[0], v[2]), a1 = sub2(v[0], v[2]);
+        const float2 a2 = add2(v[1], v[3]), a3 = rot90<DIR>(sub2(v[1], v[3]));
+        v[0] = add2(a0, a2);
+        v[2] = sub2(a0, a2);
+        v[1] = add2(a1, a3);
+        v[3] = sub2(a1, a3);
+    }
+};
+
+template <int DIR>
+struct Bfly<5, DIR> {
+    static __device__ __forceinline__ void run(float2* v) {
+        constexpr float c1 = 0.30901699437494742410f, c2 = -0.80901699437494742410f;   // cos 72, cos 144
+        constexpr float s1 = 0.95105651629515357212f, s2 = 0.58778525229247312917f;    // sin 72, sin 144
+        const float2 a1 = add2(v[1], v[4]), a2 = add2(v[2], v[3]);
+        const float2 b1 = sub2(v[1], v[4]), b2 = sub2(v[2], v[3]);
+        const float2 x0 = v[0];
+        v[0] = add2(x0, add2(a1, a2));
+        const float2 e1 = fma2(a2, make_float2(c2, c2), fma2(a1, make_float2(c1, c1), x0));
+        const float2 e2 = fma2(a2, make_float2(c1, c1), fma2(a1, make_float2(c2, c2), x0));
+        const float2 d1 = rot90<DIR>(fma2(b2, make_float2(s2, s2), scale2(b1, s1)));
+        const float2 d2 = rot90<DIR>(fma2(b2, make_float2(-s1, -s1), scale2(b1, s2)));
+        v[1] = add2(e1, d1);
+        v[4] = sub2(e1, d1);
+        v[2] = add2(e2, d2);
+        v[3] = sub2(e2, d2);
+    }
+};
+
+// a * exp(DIR i pi / 4) and a * exp(DIR 3 i pi / 4)
+template <int DIR>
+__device__ __forceinline__ float2 rot45(float2 a) {
+    constexpr float h = 0.70710678118654752440f;
+    return scale2(add2(a, rot90<DIR>(a)), h);
+}
+template <int DIR>
+__device__ __forceinline__ float2 rot135(float2 a) {
+    constexpr float h = 0.70710678118654752440f;
+    return scale2(sub2(rot90<DIR>(a), a), h);
+}
+
+template <int DIR>
+struct Bfly<8, DIR> {
+    static __device__ __forceinline__ void run(float2* v) {
+        // radix-2 split (decimation in frequency), then two radix-4 transforms
+        float2 a[4], b[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            a[k] = add2(v[k], v[k + 4]);
+            b[k] = sub2(v[k], v[k + 4]);
+        }
+        b[1] = rot45<DIR>(b[1]);
+        b[2] = rot90<DIR>(b[2]);
+        b[3] = rot135<DIR>(b[3]);
+        Bfly<4, DIR>::run(a);
+        Bfly<4, DIR>::run(b);
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            v[2 * q] = a[q];
+            v[2 * q + 1] = b[q];
+        }
+    }
+};
+
+template <int DIR>
+struct Bfly<16, DIR> {
+    static __device__ __forceinline__ void run(float2* v) {
+        // 16 = 4 x 4: n = n1 + 4 n2, f = f2 + 4 f1
+        constexpr float c1 = 0.92387953251128675613f, s1 = 0.38268343236508977173f;   // cos, sin of pi/8
+        constexpr float h = 0.70710678118654752440f;
+        float2 a[4][4];
+#pragma unroll
+        for (int n1 = 0; n1 < 4; ++n1) {
+            float2 t[4] = {v[n1], v[n1 + 4], v[n1 + 8], v[n1 + 12]};
+            Bfly<4, DIR>::run(t);
+#pragma unroll
+            for (int f2 = 0; f2 < 4; ++f2) a[n1][f2] = t[f2];
+        }
+        // twiddles w16^(n1 f2), w16 = exp(DIR 2 pi i / 16)
+        const float sg = DIR < 0 ? -1.f : 1.f;
+        const float2 w1 = make_float2(c1, sg * s1), w2 = make_float2(h, sg * h), w3 = make_float2(s1, sg * c1);
+        const float2 w6 = make_float2(-h, sg * h), w9 = make_float2(-c1, -sg * s1);
+        a[1][1] = cmul(a[1][1], w1);
+        a[1][2] = cmul(a[1][2], w2);
+        a[1][3] = cmul(a[1][3], w3);
+        a[2][1] = cmul(a[2][1], w2);
+        a[2][2] = rot90<DIR>(a[2][2]);
+        a[2][3] = cmul(a[2][3], w6);
+        a[3][1] = cmul(a[3][1], w3);
+        a[3][2] = cmul(a[3][2], w6);
+        a[3][3] = cmul(a[3][3], w9);
+#pragma unroll
+        for (int f2 = 0; f2 < 4; ++f2) {
+            float2 t[4] = {a[0][f2], a[1][f2], a[2][f2], a[3][f2]};
+            Bfly<4, DIR>::run(t);
+#pragma unroll
+            for (int f1 = 0; f1 < 4; ++f1) v[f2 + 4 * f1] = t[f1];
+        }
+    }
+};
+
+// ---------------------------------------------------------------------------------------------
+// plans
+// ---------------------------------------------------------------------------------------------
+template <int N_, int E_, int R0, int R1 = 1, int R2 = 1, int R3 = 1, int R4 = 1>
+struct Plan {
+    static constexpr int N = N_, E = E_, TPF = N_ / E_;
+    static constexpr int S = 1 + (R1 > 1) + (R2 > 1) + (R3 > 1) + (R4 > 1);
+    static constexpr int PAD_DIV = R0;   // row layout: pos -> pos + pos / R0 (conflict-free strided stores)
+    static constexpr int NPAD = N_ + N_ / R0;
+    __host__ __device__ static constexpr int radix(int s) {
+        return s == 0 ? R0 : s == 1 ? R1 : s == 2 ? R2 : s == 3 ? R3 : R4;
+    }
+    __host__ __device__ static constexpr int ns(int s) {   // product of the radices before stage s
+        int p = 1;
+        for (int k = 0; k < s; ++k) p *= radix(k);
+        return p;
+    }
+    static_assert(R0 * R1 * R2 * R3 * R4 == N_, "radices must multiply to N");
+    static_assert(N_ % E_ == 0 && E_ % R0 == 0 && E_ % R1 == 0 && E_ % R2 == 0 && E_ % R3 == 0 && E_ % R4 == 0,
+                  "every radix must divide the per-thread element count");
+};
+
+// Row layout: one FFT per TPF threads, exchange region of NPAD float2 per FFT, padded against the
+// stride-R0 stores of stage 0.
+template <class P>
+struct RowAddr {
+    int base;
+    __device__ __forceinline__ int operator()(int pos) const { return base + pos + pos / P::PAD_DIV; }
+};
+// Column layout: TC FFTs side by side, position-major: [pos][TC].  With TC = 16 a half-warp touches
+// one 128-byte line; narrower tiles shift every group of R0 positions by one slot so that the
+// stride-R0 stores of stage 0 from two neighbouring threads land in different bank halves.
+template <class P, int TC>
+struct ColAddr {
+    static constexpr int NPOS = TC < 16 ? P::NPAD : P::N;
+    int c;
+    __device__ __forceinline__ int operator()(int pos) const {
+        return (TC < 16 ? pos + pos / P::PAD_DIV : pos) * TC + c;
+    }
+};
+
+// tw: shared memory, [(s-1) * E + e][TPF] for stages s >= 1: exp(-2 pi i m k / (Ns R)) of the element
+template <class P, int s, int DIR, class Addr>
+__device__ __forceinline__ void fft_stage(float2 (&x)[P::E], float2* buf, const float2* tw, int t, const Addr& addr) {
+    constexpr int R = P::radix(s), NB = P::E / R, NS = P::ns(s), TPF = P::TPF;
+    constexpr bool last = (s == P::S - 1);
+#pragma unroll
+    for (int u = 0; u < NB; ++u) {
+        float2 v[R];
+#pragma unroll
+        for (int m = 0; m < R; ++m) v[m] = x[u + m * NB];
+        if (s > 0) {
+#pragma unroll
+            for (int m = 1; m < R; ++m) {
+                const float2 w = tw[((s - 1) * P::E + u + m * NB) * TPF + t];
+                v[m] = DIR < 0 ? cmul(v[m], w) : cmulc(v[m], w);
+            }
+        }
+        Bfly<R, DIR>::run(v);
+        if (last) {
+#pragma unroll
+            for (int m = 0; m < R; ++m) x[u + m * NB] = v[m];
+        } else {
+            const int j = t + u * TPF;
+            const int k = j % NS;
+            const int base = (j - k) * R + k;
+#pragma unroll
+            for (int m = 0; m < R; ++m) buf[addr(base + m * NS)] = v[m];
+        }
+    }
+    if (!last) {
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < P::E; ++e) x[e] = buf[addr(t + TPF * e)];
+        __syncthreads();
+    }
+}
+
+template <class P, int DIR, class Addr>
+__device__ __forceinline__ void fft_run(float2 (&x)[P::E], float2* buf, const float2* tw, int t, const Addr& addr) {
+    fft_stage<P, 0, DIR>(x, buf, tw, t, addr);
+    if constexpr (P::S > 1) fft_stage<P, 1, DIR>(x, buf, tw, t, addr);
+    if constexpr (P::S > 2) fft_stage<P, 2, DIR>(x, buf, tw, t, addr);
+    if constexpr (P::S > 3) fft_stage<P, 3, DIR>(x, buf, tw, t, addr);
+    if constexpr (P::S > 4) fft_stage<P, 4, DIR>(x, buf, tw, t, addr);
+}
+
+// ---------------------------------------------------------------------------------------------
+// kernels
+// ---------------------------------------------------------------------------------------------
+enum RowMode { ROWS_FIRST = 0, ROWS_RATIO = 1, ROWS_UPDATE = 2 };
+
+struct RowArgs {
+    float2* S;               // [pairs][H][W] spectrum (row pass in / out)
+    float2* Z;               // [pairs][H][W] psi pairs
+    const uint16_t* views;   // view 0 of plane 0 of this chunk
+    size_t view_stride;      // elements between views
+    float* out;              // [n_planes][H][W]; written when `final`
+    int n_planes, H, V, v;   // v: the view of this update (ROWS_RATIO)
+    float eps;
+    int final;               // ROWS_UPDATE: last update -> write `out`, skip the forward FFT
+                             // ROWS_FIRST : iterations == 0 -> write `out` only
+    int total_rows;          // pairs * H
+};
+
+template <class P, int MODE, int NT>
+__global__ void __launch_bounds__(NT) fft_rows_kernel(RowArgs a, const float2* __restrict__ tw_g) {
+    constexpr int E = P::E, TPF = P::TPF, W = P::N, RP = NT / TPF;
+    static_assert(NT % TPF == 0 && RP >= 1, "block must hold whole FFTs");
+    extern __shared__ float2 smem_rows[];
+    float2* tw = smem_rows;                                   // [(S-1) E][TPF]
+    float2* buf = smem_rows + (P::S - 1) * E * TPF;           // [RP][NPAD]
+    for (int k = threadIdx.x; k < (P::S - 1) * E * TPF; k += NT) tw[k] = tw_g[k];
+    __syncthreads();
+    const int r = threadIdx.x / TPF, t = threadIdx.x % TPF;
+    const RowAddr<P> addr{r * P::NPAD};
+    const size_t npx = (size_t)a.H * W;
+
+    for (int row0 = blockIdx.x * RP; row0 < a.total_rows; row0 += gridDim.x * RP) {
+        const int row = row0 + r;
+        const bool valid = row < a.total_rows;
+        const int pair = valid ? row / a.H : 0, y = valid ? row % a.H : 0;
+        const int pa = 2 * pair, pb = 2 * pair + 1;
+        const bool has_b = pb < a.n_planes;
+        const size_t rowoff = (size_t)row * W;          // into S / Z
+        const size_t pxa = (size_t)pa * npx + (size_t)y * W, pxb = pxa + npx;   // into views / out
+        float2 x[E];
+
+        if (MODE == ROWS_FIRST) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const int pos = t + TPF * e;
+                float sa = 0.f, sb = 0.f;
+                if (valid)
+                    for (int v = 0; v < a.V; ++v) {
+                        const uint16_t* vp = a.views + (size_t)v * a.view_stride;
+                        sa += (float)__ldg(vp + pxa + pos);
+                        if (has_b) sb += (float)__ldg(vp + pxb + pos);
+                    }
+                x[e] = make_float2(sa / (float)a.V, sb / (float)a.V);       // a0
+                if (valid) {
+                    if (a.final) {
+                        a.out[pxa + pos] = x[e].x;
+                        if (has_b) a.out[pxb + pos] = x[e].y;
+                    } else {
+                        a.Z[rowoff + pos] = x[e];
+                    }
+                }
+            }
+            if (a.final) continue;   // uniform over the block
+        } else {
+            uint32_t ph[E];          // phi_a | phi_b << 16, fetched before the inverse transform
+            if (MODE == ROWS_RATIO) {
+                const uint16_t* vp = a.views + (size_t)a.v * a.view_stride;
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    const int pos = t + TPF * e;
+                    uint32_t lo = 0, hi = 0;
+                    if (valid) {
+                        lo = __ldg(vp + pxa + pos);
+                        if (has_b) hi = __ldg(vp + pxb + pos);
+                    }
+                    ph[e] = lo | (hi << 16);
+                }
+            }
+#pragma unroll
+            for (int e = 0; e < E; ++e) x[e] = valid ? a.S[rowoff + t + TPF * e] : make_float2(0.f, 0.f);
+            fft_run<P, +1>(x, buf, tw, t, addr);
+            if (MODE == ROWS_RATIO) {
+#pragma unroll
+                for (int e = 0; e < E; ++e) {                                 // a2
+                    x[e].x = (float)(ph[e] & 0xffffu) / fmaxf(x[e].x, a.eps);
+                    x[e].y = (float)(ph[e] >> 16) / fmaxf(x[e].y, a.eps);
+                }
+            } else {
+#pragma unroll
+                for (int e = 0; e < E; ++e) {                                 // a4
+                    const int pos = t + TPF * e;
+                    const float2 z = valid ? a.Z[rowoff + pos] : make_float2(0.f, 0.f);
+                    x[e] = make_float2(z.x * x[e].x, z.y * x[e].y);
+                    if (valid) {
+                        if (a.final) {
+                            a.out[pxa + pos] = x[e].x;
+                            if (has_b) a.out[pxb + pos] = x[e].y;
+                        } else {
+                            a.Z[rowoff + pos] = x[e];
+                        }
+                    }
+                }
+                if (a.final) continue;
+            }
+        }
+        fft_run<P, -1>(x, buf, tw, t, addr);
+        if (valid) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) a.S[rowoff + t + TPF * e] = x[e];
+        }
+    }
+}
+
+// Column pass over a tile of TC columns: forward FFT along z, multiply by the OTF (conjugated for
+// the back-projection), inverse FFT, in place.  The CTA keeps its OTF tile in registers and walks
+// over the plane pairs assigned to it.
+template <class P, int TC, bool OTF_REGS>
+__global__ void __launch_bounds__(TC* P::TPF)
+fft_cols_kernel(float2* __restrict__ S, const float2* __restrict__ otf, int conj_otf, int pairs, int W,
+                const float2* __restrict__ tw_g) {
+    constexpr int E = P::E, TPF = P::TPF, H = P::N, NT = TC * TPF;
+    extern __shared__ float2 smem_cols[];
+    float2* tw = smem_cols;                                   // [(S-1) E][TPF]
+    float2* buf = smem_cols + (P::S - 1) * E * TPF;           // [H][TC]
+    for (int k = threadIdx.x; k < (P::S - 1) * E * TPF; k += NT) tw[k] = tw_g[k];
+    __syncthreads();
+    const int c = threadIdx.x % TC, t = threadIdx.x / TC;
+    const ColAddr<P, TC> addr{c};
+    const int xg = blockIdx.x * TC + c;
+    const float sgn = conj_otf ? -1.f : 1.f;
+
+    float2 o[OTF_REGS ? E : 1];
+    if (OTF_REGS) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            o[e] = __ldg(otf + (size_t)(t + TPF * e) * W + xg);
+            o[e].y *= sgn;
+        }
+    }
+    for (int p = blockIdx.y; p < pairs; p += gridDim.y) {
+        float2* Sp = S + (size_t)p * H * W + xg;
+        float2 x[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) x[e] = Sp[(size_t)(t + TPF * e) * W];
+        fft_run<P, -1>(x, buf, tw, t, addr);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            float2 w;
+            if (OTF_REGS) {
+                w = o[e];
+            } else {
+                w = __ldg(otf + (size_t)(t + TPF * e) * W + xg);
+                w.y *= sgn;
+            }
+            x[e] = cmul(x[e], w);
+        }
+        fft_run<P, +1>(x, buf, tw, t, addr);
+#pragma unroll
+        for (int e = 0; e < E; ++e) Sp[(size_t)(t + TPF * e) * W] = x[e];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host-side descriptors (one per supported length)
+// ---------------------------------------------------------------------------------------------
+struct PlanInfo {
+    int E, TPF, S;
+    int radices[5];
+};
+struct SizeOps {
+    int N;
+    PlanInfo row, col;               // the length's plan when it is the row (x) / column (z) length
+    int row_threads;                 // NT of the row kernels
+    size_t row_smem, col_smem;       // dynamic shared memory (bytes)
+    int col_tc;                      // TC of the column kernel
+    cudaError_t (*rows)(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st);
+    cudaError_t (*cols)(float2* S, const float2* otf, int conj_otf, int pairs, int W, const float2* tw,
+                        dim3 grid, cudaStream_t st);
+    cudaError_t (*prepare)();        // opt in to > 48 KB dynamic shared memory
+};
+
+template <class P, int NT, class PC, int TC, bool OTF_REGS>
+struct OpsFor {
+    static_assert(P::N == PC::N, "row and column plan of one entry describe the same length");
+    static constexpr size_t kRowSmem = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * P::NPAD);
+    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)ColAddr<PC, TC>::NPOS * TC);
+
+    static cudaError_t rows(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st) {
+        if (mode == ROWS_FIRST) fft_rows_kernel<P, ROWS_FIRST, NT><<<grid, NT, kRowSmem, st>>>(a, tw);
+        else if (mode == ROWS_RATIO) fft_rows_kernel<P, ROWS_RATIO, NT><<<grid, NT, kRowSmem, st>>>(a, tw);
+        else fft_rows_kernel<P, ROWS_UPDATE, NT><<<grid, NT, kRowSmem, st>>>(a, tw);
+        return cudaGetLastError();
+    }
+    static cudaError_t cols(float2* S, const float2* otf, int conj_otf, int pairs, int W, const float2* tw,
+                            dim3 grid, cudaStream_t st) {
+        fft_cols_kernel<PC, TC, OTF_REGS><<<grid, TC * PC::TPF, kColSmem, st>>>(S, otf, conj_otf, pairs, W, tw);
+        return cudaGetLastError();
+    }
+    static cudaError_t prepare() {
+        cudaError_t e;
+        e = cudaFuncSetAttribute(fft_rows_kernel<P, ROWS_FIRST, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(fft_rows_kernel<P, ROWS_RATIO, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(fft_rows_kernel<P, ROWS_UPDATE, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
+        if (e != cudaSuccess) return e;
+        return cudaFuncSetAttribute(fft_cols_kernel<PC, TC, OTF_REGS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
+    }
+    static SizeOps make() {
+        SizeOps o;
+        o.N = P::N;
+        o.row = PlanInfo{P::E, P::TPF, P::S, {P::radix(0), P::radix(1), P::radix(2), P::radix(3), P::radix(4)}};
+        o.col = PlanInfo{PC::E, PC::TPF, PC::S, {PC::radix(0), PC::radix(1), PC::radix(2), PC::radix(3), PC::radix(4)}};
+        o.row_threads = NT; o.row_smem = kRowSmem; o.col_smem = kColSmem; o.col_tc = TC;
+        o.rows = &rows; o.cols = &cols; o.prepare = &prepare;
+        return o;
+    }
+};
+
+}  // namespace mvdfft
+
+// one translation unit per group of sizes (parallel compilation); each returns nullptr for other N
+const mvdfft::SizeOps* mvd_fft_ops_small(int N);
+const mvdfft::SizeOps* mvd_fft_ops_mid(int N);
+const mvdfft::SizeOps* mvd_fft_ops_large(int N);

@@ -48,6 +48,7 @@ struct mvd_handle {
 
     // fft path: optical transfer functions, float2 [V][H][W], pre-scaled by 1/(W*H)
     float2* d_otf = nullptr;
+    void* fft = nullptr;   // FftState (mvd_fft.cu)
 
     Workspace ws_main;
     // host pipeline (mvd_deconvolve_host): three slots, one stream each
@@ -101,3 +102,4 @@ int fft_setup(mvd_handle* h, const float* host_psfs);
 int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_stride, float* out,
             int n_planes, cudaStream_t stream);
 int fft_default_chunk(const mvd_handle* h);
+void fft_teardown(mvd_handle* h);

@@ -93,13 +93,18 @@ def test_large_configs_against_stored_oracle_planes(cid):
 @pytest.mark.parametrize("path", PATHS)
 @pytest.mark.parametrize("V,N,W,H,K,T,psf", [
     (3, 3, 96, 80, 7, 4, "random"),      # asymmetric, smooth sizes (both engines)
-    (2, 5, 160, 100, 13, 3, "random"),   # odd plane count; 100 = 2^2 5^2
+    (2, 5, 160, 80, 13, 3, "random"),    # odd plane count; radix-5 lengths
     (1, 2, 128, 64, 21, 5, "sparse"),    # templated K, single view
     (2, 2, 200, 150, 31, 2, "random"),   # several tiles + ragged tail, 2-chunk PSF rows
     (2, 1, 70, 50, 5, 6, "random"),      # W, H not multiples of anything useful
     (4, 2, 60, 36, 9, 3, "gauss"),
     (2, 2, 37, 23, 5, 3, "random"),      # primes: direct only
     (2, 2, 192, 320, 51, 1, "random"),   # largest templated K, 3-chunk rows
+    (2, 2, 256, 800, 9, 2, "random"),    # config 4's column length (800 = 2^5 5^2)
+    (1, 3, 2048, 64, 7, 2, "random"),    # config 4's row length
+    (2, 2, 64, 1024, 5, 2, "random"),    # config 5's column length
+    (2, 2, 1024, 512, 5, 1, "sparse"),   # config 3's plane
+    (2, 2, 32, 2048, 5, 1, "random"),    # longest column transform
 ])
 def test_asymmetric_and_ragged(path, V, N, W, H, K, T, psf):
     _need(path, W, H, K)
