@@ -79,12 +79,34 @@ __global__ void otf_cols_kernel(const double2* __restrict__ G, int K, int W, int
     O[(size_t)ky * W + kx] = make_float2((float)(re * sc), (float)(im * sc));
 }
 
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
 struct FftState {
     const SizeOps* row = nullptr;   // length W
     const SizeOps* col = nullptr;   // length H
     float2* tw_row = nullptr;
     float2* tw_col = nullptr;
+    EncodeTiledFn encode = nullptr; // cuTensorMapEncodeTiled, resolved through the runtime (no -lcuda)
 };
+
+// Tensor map of the spectrum buffer S = float [pairs * H][2 W] with a box of one column tile:
+// 2 TC floats (TC complex columns) by box_h rows.
+int make_col_tensor_map(mvd_handle* h, const FftState* st, float2* S, int pairs, CUtensorMap* map) {
+    const cuuint64_t dims[2] = {(cuuint64_t)2 * h->W, (cuuint64_t)pairs * h->H};
+    const cuuint64_t strides[1] = {(cuuint64_t)h->W * sizeof(float2)};
+    const cuuint32_t box[2] = {(cuuint32_t)(2 * st->col->col_tc), (cuuint32_t)st->col->col_box_h};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = st->encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, S, dims, strides, box, estr,
+                                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                  CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        h->last_cuda = (int)cudaErrorInvalidValue;
+        return MVD_ERR_CUDA;
+    }
+    return MVD_OK;
+}
 
 FftState* state_of(const mvd_handle* h) { return static_cast<FftState*>(h->fft); }
 
@@ -95,6 +117,8 @@ int fft_supported(int W, int H) {
     const SizeOps* c = find_ops(H);
     if (!r || !c) return 0;
     if (W % c->col_tc != 0) return 0;
+    const size_t limit = 227u * 1024u;   // dynamic shared memory per CTA on sm_100
+    if (r->row_smem > limit || c->col_smem > limit) return 0;
     return 1;
 }
 
@@ -112,8 +136,18 @@ int fft_setup(mvd_handle* h, const float* host_psfs) {
     FftState st;
     st.row = find_ops(h->W);
     st.col = find_ops(h->H);
-    MVD_TRY(h, st.row->prepare());
-    MVD_TRY(h, st.col->prepare());
+    MVD_TRY(h, st.row->prepare_rows());
+    MVD_TRY(h, st.col->prepare_cols());
+    {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        MVD_TRY(h, cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &q));
+        if (!fn || q != cudaDriverEntryPointSuccess) {
+            h->last_cuda = (int)cudaErrorNotSupported;
+            return MVD_ERR_CUDA;
+        }
+        st.encode = (EncodeTiledFn)fn;
+    }
 
     auto upload = [&](const std::vector<float2>& v, float2** d) -> int {
         const size_t bytes = std::max<size_t>(v.size(), 1) * sizeof(float2);
@@ -174,7 +208,12 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_str
     const int W = h->W, H = h->H;
     const int pairs = (n_planes + 1) / 2;
     const size_t bytes = sizeof(float2) * (size_t)pairs * H * W;
+    // the bulk copies of the row kernels need 16-byte aligned rows
+    if (((uintptr_t)views & 15u) != 0 || ((view_stride * sizeof(uint16_t)) & 15u) != 0) return MVD_ERR_INVALID;
     int rc = ws_reserve(h, ws, bytes, bytes);
+    if (rc != MVD_OK) return rc;
+    CUtensorMap tmap;
+    rc = make_col_tensor_map(h, st, (float2*)ws.b, pairs, &tmap);
     if (rc != MVD_OK) return rc;
 
     RowArgs a;
@@ -210,7 +249,7 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_str
             const float2* otf = h->d_otf + (size_t)v * npx;
             {
                 LaunchScope ls(h, KC_FFT_COLS, stream);
-                rc = mvd_check(h, st->col->cols(a.S, otf, 0, pairs, W, st->tw_col, col_grid, stream));   // a1
+                rc = mvd_check(h, st->col->cols(tmap, a.S, otf, 0, pairs, W, st->tw_col, col_grid, stream));   // a1
             }
             if (rc != MVD_OK) return rc;
             {
@@ -222,7 +261,7 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_str
             if (rc != MVD_OK) return rc;
             {
                 LaunchScope ls(h, KC_FFT_COLS, stream);
-                rc = mvd_check(h, st->col->cols(a.S, otf, 1, pairs, W, st->tw_col, col_grid, stream));   // a3
+                rc = mvd_check(h, st->col->cols(tmap, a.S, otf, 1, pairs, W, st->tw_col, col_grid, stream));   // a3
             }
             if (rc != MVD_OK) return rc;
             {

@@ -20,10 +20,47 @@
 // steps and global stores all use it directly and only S-1 exchanges per FFT go through shared memory.
 #pragma once
 
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 namespace mvdfft {
+
+// ---------------------------------------------------------------------------------------------
+// TMA (cp.async.bulk) + mbarrier plumbing: inputs of the next work item stream into shared memory
+// while the current one is transformed
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t* bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() {
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t done;
+    do {
+        asm volatile("{ .reg .pred p; mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2; selp.u32 %0, 1, 0, p; }"
+                     : "=r"(done) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    } while (!done);
+}
+// 1D bulk copy global -> shared (16-byte aligned, size a multiple of 16); SASS UBLKCP
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+// 2D tiled tensor copy global -> shared; SASS UTMALDG
+__device__ __forceinline__ void tma_2d_g2s(void* dst, const CUtensorMap* map, int x, int y, uint64_t* bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
+                 ::"r"(smem_u32(dst)), "l"(map), "r"(x), "r"(y), "r"(smem_u32(bar)) : "memory");
+}
+__host__ __device__ constexpr size_t align_up(size_t n, size_t a) { return (n + a - 1) / a * a; }
 
 // ---------------------------------------------------------------------------------------------
 // complex arithmetic on packed f32x2 (SASS FADD2 / FMUL2 / FFMA2 on sm_100a)
@@ -399,23 +436,179 @@ __global__ void __launch_bounds__(NT) fft_rows_kernel(RowArgs a, const float2* _
     }
 }
 
-// Column pass over a tile of TC columns: forward FFT along z, multiply by the OTF (conjugated for
-// the back-projection), inverse FFT, in place.  The CTA keeps its OTF tile in registers and walks
-// over the plane pairs assigned to it.
-template <class P, int TC, bool OTF_REGS>
-__global__ void __launch_bounds__(TC* P::TPF)
-fft_cols_kernel(float2* __restrict__ S, const float2* __restrict__ otf, int conj_otf, int pairs, int W,
-                const float2* __restrict__ tw_g) {
-    constexpr int E = P::E, TPF = P::TPF, H = P::N, NT = TC * TPF;
-    extern __shared__ float2 smem_cols[];
-    float2* tw = smem_cols;                                   // [(S-1) E][TPF]
-    float2* buf = smem_cols + (P::S - 1) * E * TPF;           // [H][TC]
+// Shared-memory map of the streamed row kernels (bytes from the 128-byte aligned base).
+template <class P, int MODE, int NT>
+struct RowSmem {
+    static constexpr int RP = NT / P::TPF;
+    static constexpr size_t kTw = 0;
+    static constexpr size_t kBuf = align_up(sizeof(float2) * (P::S - 1) * P::E * P::TPF, 128);
+    static constexpr size_t kStage = kBuf + align_up(sizeof(float2) * RP * P::NPAD, 128);
+    static constexpr size_t kStageBytes = align_up(sizeof(float2) * RP * P::N, 128);
+    static constexpr size_t kAux = kStage + 2 * kStageBytes;
+    // ROWS_RATIO: two uint16 rows (plane a, plane b) per row;  ROWS_UPDATE: the psi row (float2)
+    static constexpr size_t kAuxRow = MODE == ROWS_RATIO ? 2 * sizeof(uint16_t) * P::N : sizeof(float2) * P::N;
+    static constexpr size_t kAuxBytes = align_up(kAuxRow * RP, 128);
+    static constexpr size_t kBar = kAux + 2 * kAuxBytes;
+    static constexpr size_t kTotal = kBar + 2 * sizeof(uint64_t);
+};
+
+// rows_ratio / rows_update with the inputs of the NEXT pass streamed into shared memory by bulk
+// copies (one spectrum row + the uint16 rows of the two planes, or the psi row) while the current
+// pass is transformed.  Each row's first thread issues that row's copies.
+template <class P, int MODE, int NT>
+__global__ void __launch_bounds__(NT) fft_rows_tma_kernel(RowArgs a, const float2* __restrict__ tw_g) {
+    using L = RowSmem<P, MODE, NT>;
+    constexpr int E = P::E, TPF = P::TPF, W = P::N, RP = NT / TPF;
+    static_assert(MODE == ROWS_RATIO || MODE == ROWS_UPDATE, "ROWS_FIRST has its own kernel");
+    static_assert(NT % TPF == 0 && RP >= 1, "block must hold whole FFTs");
+    static_assert(P::S >= 2, "the stage-buffer reuse relies on the barriers of a multi-stage FFT");
+    extern __shared__ __align__(128) unsigned char smem_rows_tma[];
+    float2* tw = reinterpret_cast<float2*>(smem_rows_tma + L::kTw);
+    float2* buf = reinterpret_cast<float2*>(smem_rows_tma + L::kBuf);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_rows_tma + L::kBar);
+    const int r = threadIdx.x / TPF, t = threadIdx.x % TPF;
+    const RowAddr<P> addr{r * P::NPAD};
+    const size_t npx = (size_t)a.H * W;
+    const uint16_t* vp = a.views + (size_t)a.v * a.view_stride;
+
+    if (threadIdx.x == 0) {
+        mbar_init(&bar[0], RP);
+        mbar_init(&bar[1], RP);
+        fence_mbar_init();
+    }
     for (int k = threadIdx.x; k < (P::S - 1) * E * TPF; k += NT) tw[k] = tw_g[k];
     __syncthreads();
+
+    // the row's first thread fetches the row's inputs of pass `row0` into stage `s`
+    auto issue = [&](int row0, int s) {
+        if (t != 0) return;
+        const int row = row0 + r;
+        if (row >= a.total_rows) { mbar_arrive(&bar[s]); return; }
+        const int pair = row / a.H, y = row % a.H;
+        const bool has_b = 2 * pair + 1 < a.n_planes;
+        const size_t pxa = (size_t)(2 * pair) * npx + (size_t)y * W;
+        unsigned char* st = smem_rows_tma + L::kStage + (size_t)s * L::kStageBytes + sizeof(float2) * W * r;
+        unsigned char* ax = smem_rows_tma + L::kAux + (size_t)s * L::kAuxBytes + L::kAuxRow * r;
+        const uint32_t row_bytes = sizeof(float2) * W;
+        if (MODE == ROWS_RATIO) {
+            const uint32_t pb = sizeof(uint16_t) * W;
+            mbar_arrive_expect_tx(&bar[s], row_bytes + (has_b ? 2 * pb : pb));
+            bulk_g2s(st, a.S + (size_t)row * W, row_bytes, &bar[s]);
+            bulk_g2s(ax, vp + pxa, pb, &bar[s]);
+            if (has_b) bulk_g2s(ax + pb, vp + pxa + npx, pb, &bar[s]);
+        } else {
+            mbar_arrive_expect_tx(&bar[s], 2 * row_bytes);
+            bulk_g2s(st, a.S + (size_t)row * W, row_bytes, &bar[s]);
+            bulk_g2s(ax, a.Z + (size_t)row * W, row_bytes, &bar[s]);
+        }
+    };
+
+    const int stride = gridDim.x * RP;
+    int row0 = blockIdx.x * RP;
+    if (row0 < a.total_rows) issue(row0, 0);
+    for (int i = 0; row0 < a.total_rows; row0 += stride, ++i) {
+        const int s = i & 1;
+        if (row0 + stride < a.total_rows) issue(row0 + stride, s ^ 1);
+        const int row = row0 + r;
+        const bool valid = row < a.total_rows;
+        const int pair = valid ? row / a.H : 0, y = valid ? row % a.H : 0;
+        const bool has_b = 2 * pair + 1 < a.n_planes;
+        const size_t rowoff = (size_t)row * W;
+        const size_t pxa = (size_t)(2 * pair) * npx + (size_t)y * W, pxb = pxa + npx;
+        const float2* st = reinterpret_cast<const float2*>(smem_rows_tma + L::kStage + (size_t)s * L::kStageBytes) + (size_t)W * r;
+        const unsigned char* ax = smem_rows_tma + L::kAux + (size_t)s * L::kAuxBytes + L::kAuxRow * r;
+
+        mbar_wait(&bar[s], (i >> 1) & 1);
+        float2 x[E];
+#pragma unroll
+        for (int e = 0; e < E; ++e) x[e] = valid ? st[t + TPF * e] : make_float2(0.f, 0.f);
+        fft_run<P, +1>(x, buf, tw, t, addr);
+        if (MODE == ROWS_RATIO) {
+            const uint16_t* pa = reinterpret_cast<const uint16_t*>(ax);
+#pragma unroll
+            for (int e = 0; e < E; ++e) {                                 // a2
+                const int pos = t + TPF * e;
+                const float fa = valid ? (float)pa[pos] : 0.f;
+                const float fb = (valid && has_b) ? (float)pa[W + pos] : 0.f;
+                x[e].x = __fdividef(fa, fmaxf(x[e].x, a.eps));
+                x[e].y = __fdividef(fb, fmaxf(x[e].y, a.eps));
+            }
+        } else {
+            const float2* zr = reinterpret_cast<const float2*>(ax);
+#pragma unroll
+            for (int e = 0; e < E; ++e) {                                 // a4
+                const int pos = t + TPF * e;
+                const float2 z = valid ? zr[pos] : make_float2(0.f, 0.f);
+                x[e] = make_float2(z.x * x[e].x, z.y * x[e].y);
+                if (valid) {
+                    if (a.final) {
+                        a.out[pxa + pos] = x[e].x;
+                        if (has_b) a.out[pxb + pos] = x[e].y;
+                    } else {
+                        a.Z[rowoff + pos] = x[e];
+                    }
+                }
+            }
+            if (a.final) {
+                __syncthreads();   // every thread is done with this stage's psi row before it is refilled
+                continue;
+            }
+        }
+        fft_run<P, -1>(x, buf, tw, t, addr);
+        if (valid) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) a.S[rowoff + t + TPF * e] = x[e];
+        }
+    }
+}
+
+// Column pass with the next pair's tile streamed in by a 2D tiled TMA copy.  Two tile buffers: the
+// one the tile arrived in becomes the exchange buffer of its own transforms once the registers are
+// loaded, the other one receives the next tile meanwhile.
+template <class P, int TC>
+struct ColSmem {
+    static constexpr int BOXH = P::N <= 256 ? P::N : (P::N % 256 == 0 ? 256 : (P::N % 200 == 0 ? 200 : (P::N % 160 == 0 ? 160 : 128)));
+    static_assert(P::N % BOXH == 0, "tile rows must split into whole TMA boxes");
+    static constexpr size_t kTw = 0;
+    static constexpr size_t kTile = align_up(sizeof(float2) * (P::S - 1) * P::E * P::TPF, 128);
+    static constexpr size_t kTileBytes = align_up(sizeof(float2) * ColAddr<P, TC>::NPOS * TC, 128);
+    static constexpr size_t kBar = kTile + 2 * kTileBytes;
+    static constexpr size_t kTotal = kBar + 2 * sizeof(uint64_t);
+};
+
+template <class P, int TC, bool OTF_REGS>
+__global__ void __launch_bounds__(TC* P::TPF)
+fft_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, float2* __restrict__ S,
+                    const float2* __restrict__ otf, int conj_otf, int pairs, int W,
+                    const float2* __restrict__ tw_g) {
+    using L = ColSmem<P, TC>;
+    constexpr int E = P::E, TPF = P::TPF, H = P::N, NT = TC * TPF;
+    static_assert(P::S >= 2, "the tile-buffer reuse relies on the barriers of a multi-stage FFT");
+    extern __shared__ __align__(128) unsigned char smem_cols_tma[];
+    float2* tw = reinterpret_cast<float2*>(smem_cols_tma + L::kTw);
+    uint64_t* bar = reinterpret_cast<uint64_t*>(smem_cols_tma + L::kBar);
     const int c = threadIdx.x % TC, t = threadIdx.x / TC;
     const ColAddr<P, TC> addr{c};
     const int xg = blockIdx.x * TC + c;
     const float sgn = conj_otf ? -1.f : 1.f;
+
+    if (threadIdx.x == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        fence_mbar_init();
+    }
+    for (int k = threadIdx.x; k < (P::S - 1) * E * TPF; k += NT) tw[k] = tw_g[k];
+    __syncthreads();
+
+    auto issue = [&](int p, int s) {
+        if (threadIdx.x != 0) return;
+        unsigned char* dst = smem_cols_tma + L::kTile + (size_t)s * L::kTileBytes;
+        mbar_arrive_expect_tx(&bar[s], (uint32_t)(sizeof(float2) * H * TC));
+#pragma unroll
+        for (int b = 0; b < H / L::BOXH; ++b)
+            tma_2d_g2s(dst + sizeof(float2) * TC * L::BOXH * b, &tmap, 2 * (int)(blockIdx.x * TC),
+                       p * H + b * L::BOXH, &bar[s]);
+    };
 
     float2 o[OTF_REGS ? E : 1];
     if (OTF_REGS) {
@@ -425,12 +618,19 @@ fft_cols_kernel(float2* __restrict__ S, const float2* __restrict__ otf, int conj
             o[e].y *= sgn;
         }
     }
-    for (int p = blockIdx.y; p < pairs; p += gridDim.y) {
+    int p = blockIdx.y;
+    if (p < pairs) issue(p, 0);
+    for (int i = 0; p < pairs; p += gridDim.y, ++i) {
+        const int s = i & 1;
+        if (p + (int)gridDim.y < pairs) issue(p + gridDim.y, s ^ 1);
+        float2* tile = reinterpret_cast<float2*>(smem_cols_tma + L::kTile + (size_t)s * L::kTileBytes);
         float2* Sp = S + (size_t)p * H * W + xg;
+        mbar_wait(&bar[s], (i >> 1) & 1);
         float2 x[E];
 #pragma unroll
-        for (int e = 0; e < E; ++e) x[e] = Sp[(size_t)(t + TPF * e) * W];
-        fft_run<P, -1>(x, buf, tw, t, addr);
+        for (int e = 0; e < E; ++e) x[e] = tile[(t + TPF * e) * TC + c];
+        __syncthreads();   // the tile buffer turns into the exchange buffer
+        fft_run<P, -1>(x, tile, tw, t, addr);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             float2 w;
@@ -442,7 +642,7 @@ fft_cols_kernel(float2* __restrict__ S, const float2* __restrict__ otf, int conj
             }
             x[e] = cmul(x[e], w);
         }
-        fft_run<P, +1>(x, buf, tw, t, addr);
+        fft_run<P, +1>(x, tile, tw, t, addr);
 #pragma unroll
         for (int e = 0; e < E; ++e) Sp[(size_t)(t + TPF * e) * W] = x[e];
     }
@@ -462,45 +662,52 @@ struct SizeOps {
     size_t row_smem, col_smem;       // dynamic shared memory (bytes)
     int col_tc;                      // TC of the column kernel
     cudaError_t (*rows)(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st);
-    cudaError_t (*cols)(float2* S, const float2* otf, int conj_otf, int pairs, int W, const float2* tw,
-                        dim3 grid, cudaStream_t st);
-    cudaError_t (*prepare)();        // opt in to > 48 KB dynamic shared memory
+    int col_box_h;                   // rows per TMA box of the column kernel's tile
+    cudaError_t (*cols)(const CUtensorMap& tmap, float2* S, const float2* otf, int conj_otf, int pairs, int W,
+                        const float2* tw, dim3 grid, cudaStream_t st);
+    cudaError_t (*prepare_rows)();   // opt in to > 48 KB dynamic shared memory (length used as W)
+    cudaError_t (*prepare_cols)();   // same (length used as H)
 };
 
 template <class P, int NT, class PC, int TC, bool OTF_REGS>
 struct OpsFor {
     static_assert(P::N == PC::N, "row and column plan of one entry describe the same length");
-    static constexpr size_t kRowSmem = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * P::NPAD);
-    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)ColAddr<PC, TC>::NPOS * TC);
+    static constexpr size_t kFirstSmem = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * P::NPAD);
+    static constexpr size_t kRatioSmem = RowSmem<P, ROWS_RATIO, NT>::kTotal;
+    static constexpr size_t kUpdateSmem = RowSmem<P, ROWS_UPDATE, NT>::kTotal;
+    static constexpr size_t kColSmem = ColSmem<PC, TC>::kTotal;
 
     static cudaError_t rows(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st) {
-        if (mode == ROWS_FIRST) fft_rows_kernel<P, ROWS_FIRST, NT><<<grid, NT, kRowSmem, st>>>(a, tw);
-        else if (mode == ROWS_RATIO) fft_rows_kernel<P, ROWS_RATIO, NT><<<grid, NT, kRowSmem, st>>>(a, tw);
-        else fft_rows_kernel<P, ROWS_UPDATE, NT><<<grid, NT, kRowSmem, st>>>(a, tw);
+        if (mode == ROWS_FIRST) fft_rows_kernel<P, ROWS_FIRST, NT><<<grid, NT, kFirstSmem, st>>>(a, tw);
+        else if (mode == ROWS_RATIO) fft_rows_tma_kernel<P, ROWS_RATIO, NT><<<grid, NT, kRatioSmem, st>>>(a, tw);
+        else fft_rows_tma_kernel<P, ROWS_UPDATE, NT><<<grid, NT, kUpdateSmem, st>>>(a, tw);
         return cudaGetLastError();
     }
-    static cudaError_t cols(float2* S, const float2* otf, int conj_otf, int pairs, int W, const float2* tw,
-                            dim3 grid, cudaStream_t st) {
-        fft_cols_kernel<PC, TC, OTF_REGS><<<grid, TC * PC::TPF, kColSmem, st>>>(S, otf, conj_otf, pairs, W, tw);
+    static cudaError_t cols(const CUtensorMap& tmap, float2* S, const float2* otf, int conj_otf, int pairs, int W,
+                            const float2* tw, dim3 grid, cudaStream_t st) {
+        fft_cols_tma_kernel<PC, TC, OTF_REGS><<<grid, TC * PC::TPF, kColSmem, st>>>(tmap, S, otf, conj_otf, pairs, W, tw);
         return cudaGetLastError();
     }
-    static cudaError_t prepare() {
+    static cudaError_t prepare_rows() {
         cudaError_t e;
-        e = cudaFuncSetAttribute(fft_rows_kernel<P, ROWS_FIRST, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
+        e = cudaFuncSetAttribute(fft_rows_kernel<P, ROWS_FIRST, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kFirstSmem);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(fft_rows_kernel<P, ROWS_RATIO, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
+        e = cudaFuncSetAttribute(fft_rows_tma_kernel<P, ROWS_RATIO, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRatioSmem);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(fft_rows_kernel<P, ROWS_UPDATE, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
-        if (e != cudaSuccess) return e;
-        return cudaFuncSetAttribute(fft_cols_kernel<PC, TC, OTF_REGS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
+        return cudaFuncSetAttribute(fft_rows_tma_kernel<P, ROWS_UPDATE, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kUpdateSmem);
+    }
+    static cudaError_t prepare_cols() {
+        return cudaFuncSetAttribute(fft_cols_tma_kernel<PC, TC, OTF_REGS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
     }
     static SizeOps make() {
         SizeOps o;
         o.N = P::N;
         o.row = PlanInfo{P::E, P::TPF, P::S, {P::radix(0), P::radix(1), P::radix(2), P::radix(3), P::radix(4)}};
         o.col = PlanInfo{PC::E, PC::TPF, PC::S, {PC::radix(0), PC::radix(1), PC::radix(2), PC::radix(3), PC::radix(4)}};
-        o.row_threads = NT; o.row_smem = kRowSmem; o.col_smem = kColSmem; o.col_tc = TC;
-        o.rows = &rows; o.cols = &cols; o.prepare = &prepare;
+        o.row_threads = NT;
+        o.row_smem = kRatioSmem > kUpdateSmem ? kRatioSmem : kUpdateSmem;
+        o.col_smem = kColSmem; o.col_tc = TC; o.col_box_h = ColSmem<PC, TC>::BOXH;
+        o.rows = &rows; o.cols = &cols; o.prepare_rows = &prepare_rows; o.prepare_cols = &prepare_cols;
         return o;
     }
 };
