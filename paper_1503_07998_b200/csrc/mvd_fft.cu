@@ -1,6 +1,8 @@
 // mvd_fft.cu -- host side of the FFT engine: supported lengths, twiddle tables, optical transfer
 // functions, and the launch sequence of one chunk of planes (see mvd_fft_kernels.cuh for the kernels).
 #include <math.h>
+#include <stdlib.h>
+#include <string.h>
 
 #include <algorithm>
 #include <vector>
@@ -14,11 +16,22 @@ using mvdfft::SizeOps;
 
 namespace {
 
-const SizeOps* find_ops(int N) {
+// MVD_FFT_GEN=1 keeps the first-generation kernels for every length (measurement only)
+bool want_v2() {
+    const char* g = getenv("MVD_FFT_GEN");
+    return !(g && g[0] == '1');
+}
+
+// The two generations lay the spectrum out differently (v2: tile-major), so a plane uses v2 kernels
+// only when BOTH of its lengths have them.
+const SizeOps* find_ops_v1(int N) {
     if (const SizeOps* o = mvd_fft_ops_small(N)) return o;
     if (const SizeOps* o = mvd_fft_ops_mid(N)) return o;
     return mvd_fft_ops_large(N);
 }
+bool use_v2(int W, int H) { return want_v2() && mvd_fft_ops_v2(W) && mvd_fft_ops_v2(H); }
+const SizeOps* find_row_ops(int W, int H) { return use_v2(W, H) ? mvd_fft_ops_v2(W) : find_ops_v1(W); }
+const SizeOps* find_col_ops(int W, int H) { return use_v2(W, H) ? mvd_fft_ops_v2(H) : find_ops_v1(H); }
 
 // Per-thread twiddles of a plan, [(s-1) E + e][TPF], s >= 1:
 //   element e of thread t in stage s belongs to butterfly j = t + u TPF, input m  (e = u + m E/R),
@@ -61,7 +74,8 @@ __global__ void otf_rows_kernel(const float* __restrict__ P, int K, int W, doubl
 }
 
 // OTF, phase 2: O[ky][kx] = (1 / (W H)) sum_j G[j][kx] exp(-2 pi i ky (j - c) / H)   -> fp32
-__global__ void otf_cols_kernel(const double2* __restrict__ G, int K, int W, int H, float2* __restrict__ O) {
+__global__ void otf_cols_kernel(const double2* __restrict__ G, int K, int W, int H, float2* __restrict__ O,
+                                int tile_major) {
     const int kx = blockIdx.x * blockDim.x + threadIdx.x, ky = blockIdx.y;
     if (kx >= W) return;
     const int c = (K - 1) / 2;
@@ -76,7 +90,8 @@ __global__ void otf_cols_kernel(const double2* __restrict__ G, int K, int W, int
         im += g.x * s + g.y * co;
     }
     const double sc = 1.0 / ((double)W * (double)H);
-    O[(size_t)ky * W + kx] = make_float2((float)(re * sc), (float)(im * sc));
+    const size_t idx = tile_major ? ((size_t)(kx >> 4) * H + ky) * 16 + (kx & 15) : (size_t)ky * W + kx;
+    O[idx] = make_float2((float)(re * sc), (float)(im * sc));
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -113,8 +128,8 @@ FftState* state_of(const mvd_handle* h) { return static_cast<FftState*>(h->fft);
 }  // namespace
 
 int fft_supported(int W, int H) {
-    const SizeOps* r = find_ops(W);
-    const SizeOps* c = find_ops(H);
+    const SizeOps* r = find_row_ops(W, H);
+    const SizeOps* c = find_col_ops(W, H);
     if (!r || !c) return 0;
     if (W % c->col_tc != 0) return 0;
     const size_t limit = 227u * 1024u;   // dynamic shared memory per CTA on sm_100
@@ -134,8 +149,8 @@ void fft_teardown(mvd_handle* h) {
 int fft_setup(mvd_handle* h, const float* host_psfs) {
     if (!fft_supported(h->W, h->H)) return MVD_ERR_UNSUPPORTED;
     FftState st;
-    st.row = find_ops(h->W);
-    st.col = find_ops(h->H);
+    st.row = find_row_ops(h->W, h->H);
+    st.col = find_col_ops(h->W, h->H);
     MVD_TRY(h, st.row->prepare_rows());
     MVD_TRY(h, st.col->prepare_cols());
     {
@@ -182,7 +197,7 @@ int fft_setup(mvd_handle* h, const float* host_psfs) {
         }
         {
             LaunchScope ls(h, KC_SETUP, 0);
-            otf_cols_kernel<<<g2, block>>>(d_G, K, W, H, h->d_otf + (size_t)v * npx);
+            otf_cols_kernel<<<g2, block>>>(d_G, K, W, H, h->d_otf + (size_t)v * npx, st.row->generation == 2);
         }
         rc = mvd_check(h, cudaGetLastError());
     }
@@ -213,8 +228,11 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_str
     int rc = ws_reserve(h, ws, bytes, bytes);
     if (rc != MVD_OK) return rc;
     CUtensorMap tmap;
-    rc = make_col_tensor_map(h, st, (float2*)ws.b, pairs, &tmap);
-    if (rc != MVD_OK) return rc;
+    memset(&tmap, 0, sizeof(tmap));
+    if (st->col->generation == 1) {
+        rc = make_col_tensor_map(h, st, (float2*)ws.b, pairs, &tmap);
+        if (rc != MVD_OK) return rc;
+    }
 
     RowArgs a;
     a.Z = (float2*)ws.a;
@@ -232,10 +250,21 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_str
 
     const int rp = st->row->row_threads / st->row->row.TPF;          // rows per CTA pass
     const int row_ctas = (a.total_rows + rp - 1) / rp;
-    const int row_grid = std::max(1, std::min(row_ctas, h->n_sm * 16));
+    // v1: many short-lived CTAs; v2: persistent, two CTAs per SM
+    const int row_grid = std::max(1, std::min(row_ctas, h->n_sm * (st->row->generation == 2 ? st->row->row_cps : 16)));
     const int tiles = W / st->col->col_tc;
-    const int per_tile = std::max(1, (h->n_sm * 8 + tiles - 1) / tiles);
-    const dim3 col_grid(tiles, std::min(pairs, per_tile));
+    dim3 col_grid;
+    if (st->col->generation == 2) {
+        // persistent 1D grid over (tile, pair) items, never more CTAs than fit at once (a second
+        // wave would double the pass); a multiple of the tile count when CTAs keep OTF registers
+        const long long items = (long long)tiles * pairs;
+        long long g = (long long)h->n_sm * st->col->col_cps;
+        if (st->col->col_otf_regs) g = std::max<long long>(tiles, g / tiles * tiles);
+        col_grid = dim3((unsigned)std::max<long long>(1, std::min(g, items)));
+    } else {
+        const int per_tile = std::max(1, (h->n_sm * 8 + tiles - 1) / tiles);
+        col_grid = dim3(tiles, std::min(pairs, per_tile));
+    }
     const size_t npx = (size_t)W * H;
 
     {

@@ -236,6 +236,53 @@ struct Bfly<16, DIR> {
     }
 };
 
+// cos / sin of 2 pi k / 32 as compile-time constants (k any integer)
+__host__ __device__ constexpr float cos32(int k) {
+    constexpr float C[9] = {1.0f, 0.98078528040323044913f, 0.92387953251128675613f, 0.83146961230254523708f,
+                            0.70710678118654752440f, 0.55557023301960222474f, 0.38268343236508977173f,
+                            0.19509032201612826785f, 0.0f};
+    k = ((k % 32) + 32) % 32;
+    if (k > 16) k = 32 - k;
+    return k > 8 ? -C[16 - k] : C[k];
+}
+__host__ __device__ constexpr float sin32(int k) { return cos32(k - 8); }
+
+template <int DIR>
+struct Bfly<32, DIR> {
+    static __device__ __forceinline__ void run(float2* v) {
+        // 32 = 8 x 4: n = n1 + 4 n2 (n1 < 4, n2 < 8), f = f2 + 8 f1 (f2 < 8, f1 < 4)
+        float2 a[4][8];
+#pragma unroll
+        for (int n1 = 0; n1 < 4; ++n1) {
+            float2 t[8];
+#pragma unroll
+            for (int n2 = 0; n2 < 8; ++n2) t[n2] = v[n1 + 4 * n2];
+            Bfly<8, DIR>::run(t);
+#pragma unroll
+            for (int f2 = 0; f2 < 8; ++f2) a[n1][f2] = t[f2];
+        }
+        // twiddles w32^(n1 f2), w32 = exp(DIR 2 pi i / 32)
+#pragma unroll
+        for (int n1 = 1; n1 < 4; ++n1) {
+#pragma unroll
+            for (int f2 = 1; f2 < 8; ++f2) {
+                const int k = n1 * f2;
+                if (k == 8) a[n1][f2] = rot90<DIR>(a[n1][f2]);
+                else if (k == 4) a[n1][f2] = rot45<DIR>(a[n1][f2]);
+                else if (k == 12) a[n1][f2] = rot135<DIR>(a[n1][f2]);
+                else a[n1][f2] = cmul(a[n1][f2], make_float2(cos32(k), (DIR < 0 ? -1.f : 1.f) * sin32(k)));
+            }
+        }
+#pragma unroll
+        for (int f2 = 0; f2 < 8; ++f2) {
+            float2 t[4] = {a[0][f2], a[1][f2], a[2][f2], a[3][f2]};
+            Bfly<4, DIR>::run(t);
+#pragma unroll
+            for (int f1 = 0; f1 < 4; ++f1) v[f2 + 8 * f1] = t[f1];
+        }
+    }
+};
+
 // ---------------------------------------------------------------------------------------------
 // plans
 // ---------------------------------------------------------------------------------------------
@@ -277,9 +324,25 @@ struct ColAddr {
     }
 };
 
+// Who has to meet at an exchange: the whole CTA (v1 kernels: an FFT's threads are spread over all
+// warps), or only the team of NTH threads that owns the FFTs in one exchange region (v2 kernels:
+// __syncwarp for teams inside a warp, a named barrier for teams of whole warps).
+struct CtaSync {
+    __device__ __forceinline__ void operator()() const { __syncthreads(); }
+};
+template <int NTH>
+struct TeamSync {
+    int id;   // team index within the CTA (named barrier id - 1); unused for NTH <= 32
+    __device__ __forceinline__ void operator()() const {
+        if constexpr (NTH <= 32) __syncwarp();
+        else asm volatile("bar.sync %0, %1;" ::"r"(id + 1), "n"(NTH) : "memory");
+    }
+};
+
 // tw: shared memory, [(s-1) * E + e][TPF] for stages s >= 1: exp(-2 pi i m k / (Ns R)) of the element
-template <class P, int s, int DIR, class Addr>
-__device__ __forceinline__ void fft_stage(float2 (&x)[P::E], float2* buf, const float2* tw, int t, const Addr& addr) {
+template <class P, int s, int DIR, class Addr, class Sync>
+__device__ __forceinline__ void fft_stage(float2 (&x)[P::E], float2* buf, const float2* tw, int t, const Addr& addr,
+                                          const Sync& sync) {
     constexpr int R = P::radix(s), NB = P::E / R, NS = P::ns(s), TPF = P::TPF;
     constexpr bool last = (s == P::S - 1);
 #pragma unroll
@@ -307,20 +370,37 @@ __device__ __forceinline__ void fft_stage(float2 (&x)[P::E], float2* buf, const 
         }
     }
     if (!last) {
-        __syncthreads();
+        sync();
 #pragma unroll
         for (int e = 0; e < P::E; ++e) x[e] = buf[addr(t + TPF * e)];
-        __syncthreads();
+        sync();
     }
 }
 
-template <class P, int DIR, class Addr>
-__device__ __forceinline__ void fft_run(float2 (&x)[P::E], float2* buf, const float2* tw, int t, const Addr& addr) {
-    fft_stage<P, 0, DIR>(x, buf, tw, t, addr);
-    if constexpr (P::S > 1) fft_stage<P, 1, DIR>(x, buf, tw, t, addr);
-    if constexpr (P::S > 2) fft_stage<P, 2, DIR>(x, buf, tw, t, addr);
-    if constexpr (P::S > 3) fft_stage<P, 3, DIR>(x, buf, tw, t, addr);
-    if constexpr (P::S > 4) fft_stage<P, 4, DIR>(x, buf, tw, t, addr);
+template <class P, int DIR, class Addr, class Sync = CtaSync>
+__device__ __forceinline__ void fft_run(float2 (&x)[P::E], float2* buf, const float2* tw, int t, const Addr& addr,
+                                        const Sync& sync = Sync()) {
+    fft_stage<P, 0, DIR>(x, buf, tw, t, addr, sync);
+    if constexpr (P::S > 1) fft_stage<P, 1, DIR>(x, buf, tw, t, addr, sync);
+    if constexpr (P::S > 2) fft_stage<P, 2, DIR>(x, buf, tw, t, addr, sync);
+    if constexpr (P::S > 3) fft_stage<P, 3, DIR>(x, buf, tw, t, addr, sync);
+    if constexpr (P::S > 4) fft_stage<P, 4, DIR>(x, buf, tw, t, addr, sync);
+}
+
+// fft_run in two parts: every stage that exchanges through shared memory, then the last stage, which
+// works on registers only -- the exchange region is free from the end of the head onwards.
+template <class P, int DIR, class Addr, class Sync>
+__device__ __forceinline__ void fft_run_head(float2 (&x)[P::E], float2* buf, const float2* tw, int t, const Addr& addr,
+                                             const Sync& sync) {
+    if constexpr (P::S > 1) fft_stage<P, 0, DIR>(x, buf, tw, t, addr, sync);
+    if constexpr (P::S > 2) fft_stage<P, 1, DIR>(x, buf, tw, t, addr, sync);
+    if constexpr (P::S > 3) fft_stage<P, 2, DIR>(x, buf, tw, t, addr, sync);
+    if constexpr (P::S > 4) fft_stage<P, 3, DIR>(x, buf, tw, t, addr, sync);
+}
+template <class P, int DIR, class Addr, class Sync>
+__device__ __forceinline__ void fft_run_tail(float2 (&x)[P::E], float2* buf, const float2* tw, int t, const Addr& addr,
+                                             const Sync& sync) {
+    fft_stage<P, P::S - 1, DIR>(x, buf, tw, t, addr, sync);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -667,6 +747,9 @@ struct SizeOps {
                         const float2* tw, dim3 grid, cudaStream_t st);
     cudaError_t (*prepare_rows)();   // opt in to > 48 KB dynamic shared memory (length used as W)
     cudaError_t (*prepare_cols)();   // same (length used as H)
+    int col_otf_regs = 0;            // generation 2: the column kernel keeps its tile's OTF in registers
+    int row_cps = 0, col_cps = 0;    // generation 2: resident CTAs per SM the persistent grids are sized for
+    int generation = 1;              // 1: CTA-synchronous TMA-staged kernels (this file); 2: team kernels (mvd_fft_v2.cuh)
 };
 
 template <class P, int NT, class PC, int TC, bool OTF_REGS>
@@ -718,3 +801,4 @@ struct OpsFor {
 const mvdfft::SizeOps* mvd_fft_ops_small(int N);
 const mvdfft::SizeOps* mvd_fft_ops_mid(int N);
 const mvdfft::SizeOps* mvd_fft_ops_large(int N);
+const mvdfft::SizeOps* mvd_fft_ops_v2(int N);      // power-of-two lengths, team kernels

@@ -1,0 +1,375 @@
+// mvd_fft_v2.cuh -- second-generation FFT-engine kernels for power-of-two lengths (sm_100a).
+//
+// Same passes and the same arithmetic as mvd_fft_kernels.cuh (rows_first, cols . OTF, rows_ratio,
+// rows_update), organised around TEAMS instead of CTAs:
+//   * a row FFT is owned by a team of TPF threads that sits inside one warp (TPF <= 32) or is made of
+//     whole warps; the team's exchange region in shared memory is private, so the only synchronisation
+//     of a transform is __syncwarp / a named barrier of the team.  Warps of a CTA drift apart and hide
+//     each other's shared-memory and HBM latency; nothing in the steady state is a CTA-wide barrier;
+//   * a column team owns FOUR adjacent columns (one 32-byte sector per image row) and 4 TPF threads, so
+//     every global load and store of the column pass moves whole sectors without a staging tile;
+//   * plans have two stages wherever E = 32 elements per thread allows it (256 = 16 x 16, 512 = 32 x 16,
+//     1024 = 32 x 32): one exchange per transform, i.e. half the shared-memory traffic of the 8 x 8 x 8
+//     plans, which matters because at HBM speed the exchanges alone need ~50 % of an SM's shared-memory
+//     bandwidth;
+//   * the spectrum S and the OTFs are stored TILE-MAJOR: plane element (y, x) lives at
+//     ((x / 16) H + y) 16 + x % 16, i.e. 16-column tiles of H rows with 128 contiguous bytes per row.  A
+//     column team then walks one contiguous tile (DRAM pages stay open) instead of touching 32 bytes in
+//     every 8 W-byte image row, and a row team still reads whole 128-byte lines;
+//   * exchange regions are XOR-swizzled (position p lives in slot p ^ ((p / R0) & 15)) so that both the
+//     stride-R0 stores of stage 0 and the unit-stride loads are bank-conflict free for 8-byte elements.
+#pragma once
+
+#include "mvd_fft_kernels.cuh"
+
+namespace mvdfft {
+
+// programmatic dependent launch: let the next kernel in the stream start its prologue early, and wait
+// for the previous kernel's memory before touching anything it wrote
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
+// L2 prefetch of a contiguous span (16-byte aligned, size a multiple of 16)
+__device__ __forceinline__ void prefetch_l2(const void* p, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
+template <class P>
+__device__ __forceinline__ int swz(int p) {
+    constexpr int R0 = P::radix(0);
+    static_assert(R0 == 16 || R0 == 32, "the XOR swizzle is derived for first radices 16 and 32");
+    return p ^ ((p / R0) & 15);
+}
+// one FFT per region of N slots
+template <class P>
+struct RowAddr2 {
+    int base;
+    __device__ __forceinline__ int operator()(int pos) const { return base + swz<P>(pos); }
+};
+// four FFTs (adjacent columns) interleaved: [slot][4]
+template <class P>
+struct ColAddr2 {
+    int base;   // team region + column within the team
+    __device__ __forceinline__ int operator()(int pos) const { return base + 4 * swz<P>(pos); }
+};
+
+// 16-byte asynchronous copy global -> shared (SASS LDGSTS), no registers in between
+__device__ __forceinline__ void cp_async16(void* dst, const void* src) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// ---------------------------------------------------------------------------------------------
+// row passes: rows_first (MODE 0), rows_ratio (1), rows_update (2)
+//
+// rows_ratio / rows_update keep a team's exchange region busy all the time: while a transform runs
+// its register-only last stage the region is the landing zone of the next input (cp.async, no
+// registers involved), so no global load latency sits on a team's critical path:
+//     [S row landed]  -> registers -> inverse FFT head | issue phi / psi row | inverse FFT tail
+//     [aux landed]    -> pointwise step               -> forward FFT head | issue next S row | tail -> store
+// ---------------------------------------------------------------------------------------------
+template <class P, int MODE, int NT>
+__global__ void __launch_bounds__(NT, 2) fft2_rows_kernel(RowArgs a, const float2* __restrict__ tw_g) {
+    constexpr int E = P::E, TPF = P::TPF, W = P::N, RP = NT / TPF;
+    static_assert(NT % TPF == 0 && (TPF <= 32 ? 32 % TPF == 0 : TPF % 32 == 0), "teams are warp-aligned");
+    static_assert(TPF % 16 == 0 && W % 16 == 0, "tile-major addressing assumes whole 16-element groups per team step");
+    static_assert(TPF <= 32 || RP <= 15, "one named barrier per team");
+    static_assert(E % 4 == 0, "the landing copies split evenly over the team");
+    extern __shared__ __align__(16) float2 smem_rows2[];
+    float2* tw = smem_rows2;                                  // [(S-1) E][TPF]
+    float2* buf = smem_rows2 + (P::S - 1) * E * TPF;          // [RP][N]
+    for (int k = threadIdx.x; k < (P::S - 1) * E * TPF; k += NT) tw[k] = tw_g[k];
+    __syncthreads();
+    pdl_launch_dependents();
+    pdl_wait();
+    const int team = threadIdx.x / TPF, t = threadIdx.x % TPF;
+    const RowAddr2<P> addr{team * W};
+    const TeamSync<TPF> sync{team};
+    const size_t npx = (size_t)a.H * W;
+    const int stride = gridDim.x * RP;
+    const uint16_t* vp = a.views + (size_t)a.v * a.view_stride;
+    float2* land = buf + team * W;                            // the team's region, used linearly as landing zone
+    const int last_row = a.total_rows - 1;
+
+    // S is tile-major: 16-byte chunk q of image row `row` (elements 2q, 2q+1)
+    auto issue_S = [&](int row) {
+        const int pair = row / a.H, y = row % a.H;
+        const float2* src = a.S + (size_t)pair * npx + (size_t)y * 16;
+#pragma unroll
+        for (int k = 0; k < E / 2; ++k) {
+            const int q = t + TPF * k;
+            cp_async16(land + 2 * q, src + (size_t)(q >> 3) * (a.H * 16) + 2 * (q & 7));
+        }
+        cp_async_commit();
+    };
+
+    if (MODE != ROWS_FIRST && (int)blockIdx.x * RP < a.total_rows) issue_S(min((int)blockIdx.x * RP + team, last_row));
+
+    for (int row0 = blockIdx.x * RP; row0 < a.total_rows; row0 += stride) {
+        // A team whose row is past the end works on the last row again and stores nothing, so the
+        // control flow (and every barrier) is uniform.
+        const bool valid = row0 + team < a.total_rows;
+        const int row = valid ? row0 + team : last_row;
+        const int pair = row / a.H, y = row % a.H;
+        const bool has_b = 2 * pair + 1 < a.n_planes;
+        const size_t rowoff = (size_t)row * W;                                      // into Z
+        const size_t pxa = (size_t)(2 * pair) * npx + (size_t)y * W;                // into views / out
+        const size_t pxb = has_b ? pxa + npx : pxa;                                 // odd tail: plane a again, discarded
+        const bool st_a = valid, st_b = valid && has_b;
+        float2* Srow = a.S + (size_t)pair * npx + (size_t)(t >> 4) * (a.H * 16) + (size_t)y * 16 + (t & 15);
+        const size_t Sstep = (size_t)TPF * a.H;       // x advances by TPF: TPF / 16 tiles of H * 16 elements
+        float2* Zrow = a.Z + rowoff + t;
+        const bool more = row0 + stride < a.total_rows;
+        const int next_row = min(row0 + stride + team, last_row);
+        float2 x[E];
+
+        if (MODE == ROWS_FIRST) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) x[e] = make_float2(0.f, 0.f);
+            for (int v = 0; v < a.V; ++v) {
+                const uint16_t* qa = a.views + (size_t)v * a.view_stride + pxa + t;
+                const uint16_t* qb = a.views + (size_t)v * a.view_stride + pxb + t;
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    x[e].x += (float)__ldg(qa + TPF * e);
+                    x[e].y += (float)__ldg(qb + TPF * e);
+                }
+            }
+            const float fv = (float)a.V;
+#pragma unroll
+            for (int e = 0; e < E; ++e) x[e] = make_float2(x[e].x / fv, x[e].y / fv);       // a0
+            if (a.final) {   // iterations == 0: the mean is the result (uniform over the grid)
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    if (st_a) a.out[pxa + t + TPF * e] = x[e].x;
+                    if (st_b) a.out[pxb + t + TPF * e] = x[e].y;
+                }
+                continue;
+            }
+            if (valid) {
+#pragma unroll
+                for (int e = 0; e < E; ++e) Zrow[TPF * e] = x[e];
+            }
+            fft_run<P, -1>(x, buf, tw, t, addr, sync);
+        } else {
+            cp_async_wait_all();
+            sync();
+#pragma unroll
+            for (int e = 0; e < E; ++e) x[e] = land[t + TPF * e];
+            sync();
+            fft_run_head<P, +1>(x, buf, tw, t, addr, sync);
+            if (MODE == ROWS_RATIO) {
+                // phi rows of the two planes: W uint16 each, [0, W) plane a, [W, 2 W) plane b
+                uint16_t* lu = reinterpret_cast<uint16_t*>(land);
+#pragma unroll
+                for (int k = 0; k < E / 4; ++k) {
+                    const int q = t + TPF * k;                   // chunk of 8 uint16; W / 8 chunks per plane
+                    const bool second = q >= W / 8;
+                    const int qq = second ? q - W / 8 : q;
+                    cp_async16(lu + 8 * q, vp + (second ? pxb : pxa) + 8 * qq);
+                }
+            } else {
+#pragma unroll
+                for (int k = 0; k < E / 2; ++k) {
+                    const int q = t + TPF * k;
+                    cp_async16(land + 2 * q, a.Z + rowoff + 2 * q);
+                }
+            }
+            cp_async_commit();
+            fft_run_tail<P, +1>(x, buf, tw, t, addr, sync);
+            cp_async_wait_all();
+            sync();
+            if (MODE == ROWS_RATIO) {
+                const uint16_t* lu = reinterpret_cast<const uint16_t*>(land);
+#pragma unroll
+                for (int e = 0; e < E; ++e) {                                 // a2
+                    const int pos = t + TPF * e;
+                    x[e].x = __fdividef((float)lu[pos], fmaxf(x[e].x, a.eps));
+                    x[e].y = __fdividef((float)lu[W + pos], fmaxf(x[e].y, a.eps));
+                }
+                sync();
+            } else {
+#pragma unroll
+                for (int e = 0; e < E; ++e) {                                 // a4
+                    const float2 z = land[t + TPF * e];
+                    x[e] = make_float2(z.x * x[e].x, z.y * x[e].y);
+                }
+                sync();
+                if (a.final) {   // last update: psi is the result (uniform over the grid)
+                    if (more) issue_S(next_row);
+#pragma unroll
+                    for (int e = 0; e < E; ++e) {
+                        if (st_a) a.out[pxa + t + TPF * e] = x[e].x;
+                        if (st_b) a.out[pxb + t + TPF * e] = x[e].y;
+                    }
+                    continue;
+                }
+                if (valid) {
+#pragma unroll
+                    for (int e = 0; e < E; ++e) Zrow[TPF * e] = x[e];
+                }
+            }
+            fft_run_head<P, -1>(x, buf, tw, t, addr, sync);
+            if (more) issue_S(next_row);
+            fft_run_tail<P, -1>(x, buf, tw, t, addr, sync);
+        }
+        if (valid) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) Srow[Sstep * e] = x[e];
+        }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// column pass: forward column FFT, . OTF (or its conjugate), inverse column FFT, in place
+// ---------------------------------------------------------------------------------------------
+// STAGE: the team's slice of the NEXT pair is copied into a staging region with cp.async while the
+// current pair is transformed (costs as much shared memory again as the exchange regions).
+template <class P, int NT, bool OTF_REGS, bool STAGE, int MINB>
+__global__ void __launch_bounds__(NT, MINB)
+fft2_cols_kernel(float2* __restrict__ S, const float2* __restrict__ otf, int conj_otf, int pairs, int W,
+                 const float2* __restrict__ tw_g) {
+    constexpr int E = P::E, TPF = P::TPF, H = P::N, TEAM = 4 * TPF, NTEAM = NT / TEAM, TC = 4 * NTEAM;
+    static_assert(NT % TEAM == 0 && TEAM % 32 == 0 && NTEAM <= 15, "column teams are whole warps");
+    static_assert((2 * H) % TEAM == 0, "the staging copy splits evenly over the team");
+    extern __shared__ __align__(16) float2 smem_cols2[];
+    float2* tw = smem_cols2;                                  // [(S-1) E][TPF]
+    float2* buf = smem_cols2 + (P::S - 1) * E * TPF;          // [NTEAM][H][4]  exchange regions
+    float2* stage = buf + NTEAM * H * 4;                      // [NTEAM][H][4]  staging regions (STAGE)
+    for (int k = threadIdx.x; k < (P::S - 1) * E * TPF; k += NT) tw[k] = tw_g[k];
+    __syncthreads();
+    pdl_launch_dependents();
+    const int team = threadIdx.x / TEAM, l = threadIdx.x % TEAM;
+    const int c4 = l & 3, t = l >> 2;
+    const ColAddr2<P> addr{team * H * 4 + c4};
+    const TeamSync<TEAM> sync{team};
+    const float sgn = conj_otf ? -1.f : 1.f;
+    float2* my_stage = stage + team * H * 4;
+    // Work items (column tile, pair), tile fastest, dealt round-robin to a persistent grid.  With
+    // OTF_REGS the host makes gridDim.x a multiple of the tile count, so a CTA keeps its tile.
+    const int tiles = W / TC;
+    const int items = tiles * pairs;
+    auto first_col = [&](int item) { return (item % tiles) * TC + team * 4; };
+    // tile-major offset of (row 0, column x) within a plane: 16-column tiles of H rows, 16 elements per row
+    auto plane_off = [&](int x) { return (size_t)(x >> 4) * (H * 16) + (x & 15); };
+
+    // chunk q of a team's slice: image row q / 2, columns x0 + 2 (q % 2) .. + 1  (16 bytes)
+    auto issue = [&](int item) {
+        const float2* src = S + (size_t)(item / tiles) * H * W + plane_off(first_col(item));
+#pragma unroll
+        for (int k = 0; k < 2 * H / TEAM; ++k) {
+            const int q = l + TEAM * k;
+            cp_async16(my_stage + 2 * q, src + (size_t)(q >> 1) * 16 + 2 * (q & 1));
+        }
+        cp_async_commit();
+    };
+
+    int item = blockIdx.x;
+    float2 o[OTF_REGS ? E : 1];
+    if (OTF_REGS && item < items) {   // the OTF is written once in mvd_create: no dependency on the previous kernel
+        const int xg = first_col(item) + c4;
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            o[e] = __ldg(otf + plane_off(xg) + (size_t)(t + TPF * e) * 16);
+            o[e].y *= sgn;
+        }
+    }
+    pdl_wait();
+    if (STAGE && item < items) issue(item);
+    for (; item < items; item += gridDim.x) {
+        const int xg = first_col(item) + c4;
+        float2* Sp = S + (size_t)(item / tiles) * H * W + plane_off(xg);
+        float2 x[E];
+        if (STAGE) {
+            cp_async_wait_all();
+            sync();
+#pragma unroll
+            for (int e = 0; e < E; ++e) x[e] = my_stage[(t + TPF * e) * 4 + c4];
+            sync();
+            if (item + (int)gridDim.x < items) issue(item + gridDim.x);
+        } else {
+#pragma unroll
+            for (int e = 0; e < E; ++e) x[e] = Sp[(size_t)(t + TPF * e) * 16];
+        }
+        fft_run<P, -1>(x, buf, tw, t, addr, sync);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            float2 w;
+            if (OTF_REGS) {
+                w = o[e];
+            } else {
+                w = __ldg(otf + plane_off(xg) + (size_t)(t + TPF * e) * 16);
+                w.y *= sgn;
+            }
+            x[e] = cmul(x[e], w);
+        }
+        fft_run<P, +1>(x, buf, tw, t, addr, sync);
+#pragma unroll
+        for (int e = 0; e < E; ++e) Sp[(size_t)(t + TPF * e) * 16] = x[e];
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host-side descriptor of a v2 length
+// ---------------------------------------------------------------------------------------------
+template <class Kern, class... Args>
+inline cudaError_t launch_pdl(Kern kern, dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kern, args...);
+}
+
+template <class P, int NT, class PC, int NTC, bool OTF_REGS, bool STAGE, int MINB>
+struct OpsFor2 {
+    static_assert(P::N == PC::N, "row and column plan of one entry describe the same length");
+    static constexpr size_t kRowSmem = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * P::N);
+    static constexpr int kTeam = 4 * PC::TPF, kNTeam = NTC / kTeam, kTC = 4 * kNTeam;
+    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)(STAGE ? 2 : 1) * kNTeam * PC::N * 4);
+
+    static cudaError_t rows(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st) {
+        if (mode == ROWS_FIRST) return launch_pdl(fft2_rows_kernel<P, ROWS_FIRST, NT>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
+        if (mode == ROWS_RATIO) return launch_pdl(fft2_rows_kernel<P, ROWS_RATIO, NT>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
+        return launch_pdl(fft2_rows_kernel<P, ROWS_UPDATE, NT>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
+    }
+    static cudaError_t cols(const CUtensorMap&, float2* S, const float2* otf, int conj_otf, int pairs, int W,
+                            const float2* tw, dim3 grid, cudaStream_t st) {
+        return launch_pdl(fft2_cols_kernel<PC, NTC, OTF_REGS, STAGE, MINB>, grid, dim3(NTC), kColSmem, st, S, otf, conj_otf, pairs, W, tw);
+    }
+    static cudaError_t prepare_rows() {
+        cudaError_t e;
+        e = cudaFuncSetAttribute(fft2_rows_kernel<P, ROWS_FIRST, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(fft2_rows_kernel<P, ROWS_RATIO, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
+        if (e != cudaSuccess) return e;
+        return cudaFuncSetAttribute(fft2_rows_kernel<P, ROWS_UPDATE, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
+    }
+    static cudaError_t prepare_cols() {
+        return cudaFuncSetAttribute(fft2_cols_kernel<PC, NTC, OTF_REGS, STAGE, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
+    }
+    static SizeOps make() {
+        SizeOps o;
+        o.N = P::N;
+        o.row = PlanInfo{P::E, P::TPF, P::S, {P::radix(0), P::radix(1), P::radix(2), P::radix(3), P::radix(4)}};
+        o.col = PlanInfo{PC::E, PC::TPF, PC::S, {PC::radix(0), PC::radix(1), PC::radix(2), PC::radix(3), PC::radix(4)}};
+        o.row_threads = NT;
+        o.row_smem = kRowSmem;
+        o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = 0;
+        o.rows = &rows; o.cols = &cols; o.prepare_rows = &prepare_rows; o.prepare_cols = &prepare_cols;
+        o.generation = 2;
+        o.row_cps = 2;
+        o.col_cps = MINB;
+        o.col_otf_regs = OTF_REGS ? 1 : 0;
+        return o;
+    }
+};
+
+}  // namespace mvdfft
