@@ -109,9 +109,13 @@ struct FftState {
 // Tensor map of the spectrum buffer S = float [pairs * H][2 W] with a box of one column tile:
 // 2 TC floats (TC complex columns) by box_h rows.
 int make_col_tensor_map(mvd_handle* h, const FftState* st, float2* S, int pairs, CUtensorMap* map) {
-    const cuuint64_t dims[2] = {(cuuint64_t)2 * h->W, (cuuint64_t)pairs * h->H};
-    const cuuint64_t strides[1] = {(cuuint64_t)h->W * sizeof(float2)};
-    const cuuint32_t box[2] = {(cuuint32_t)(2 * st->col->col_tc), (cuuint32_t)st->col->col_box_h};
+    const bool v2 = st->col->generation == 2;
+    // v1: S = float [pairs * H][2 W], box = one column tile;  v2 (tile-major S): float [pairs * W/16 * H][32]
+    // (128-byte rows), box = one team's four columns (8 floats) by up to 256 tile rows
+    const cuuint64_t dims[2] = {v2 ? (cuuint64_t)32 : (cuuint64_t)2 * h->W,
+                                v2 ? (cuuint64_t)pairs * (h->W / 16) * h->H : (cuuint64_t)pairs * h->H};
+    const cuuint64_t strides[1] = {v2 ? (cuuint64_t)128 : (cuuint64_t)h->W * sizeof(float2)};
+    const cuuint32_t box[2] = {v2 ? 8u : (cuuint32_t)(2 * st->col->col_tc), (cuuint32_t)st->col->col_box_h};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = st->encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, S, dims, strides, box, estr,
                                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -229,7 +233,7 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_str
     if (rc != MVD_OK) return rc;
     CUtensorMap tmap;
     memset(&tmap, 0, sizeof(tmap));
-    if (st->col->generation == 1) {
+    if (st->col->col_box_h > 0) {
         rc = make_col_tensor_map(h, st, (float2*)ws.b, pairs, &tmap);
         if (rc != MVD_OK) return rc;
     }

@@ -1,4 +1,6 @@
 // FFT engine, generation-2 (team-synchronous) kernels: 256, 512, 1024, 2048.
+#include <stdlib.h>
+
 #include "mvd_fft_v2.cuh"
 using namespace mvdfft;
 
@@ -7,10 +9,21 @@ const SizeOps* mvd_fft_ops_v2(int N) {
     using P512 = Plan<512, 32, 32, 16>;
     using P1024 = Plan<1024, 32, 32, 32>;
     using P2048 = Plan<2048, 32, 32, 32, 2>;
-    static const SizeOps o256 = OpsFor2<P256, 256, P256, 256, true, true, 2>::make();
-    static const SizeOps o512 = OpsFor2<P512, 256, P512, 128, false, true, 3>::make();
-    static const SizeOps o1024 = OpsFor2<P1024, 256, P1024, 128, false, true, 3>::make();
-    static const SizeOps o2048 = OpsFor2<P2048, 256, P2048, 256, false, false, 2>::make();
+    using P256C = Plan<256, 32, 32, 8>;      // column plan: four columns per warp, E = 32
+    static const SizeOps o256 = OpsFor2<P256, 256, P256, 256, true, 2>::make();
+    static const SizeOps o512 = OpsFor2<P512, 256, P512, 128, false, 3>::make();
+    static const SizeOps o1024 = OpsFor2<P1024, 256, P1024, 128, false, 3>::make();
+    static const SizeOps o2048 = OpsFor2<P2048, 256, P2048, 256, false, 2, false>::make();
+    // measurement knob: alternative column kernels for 256
+    static const SizeOps o256a = OpsFor2<P256, 256, P256, 256, true, 2, false>::make();
+    static const SizeOps o256b = OpsFor2<P256, 256, P256C, 256, false, 2>::make();
+    static const SizeOps o256c = OpsFor2<P256, 256, P256, 128, true, 4>::make();
+    static const char* var = getenv("MVD_COLS_VARIANT");
+    if (N == 256 && var) {
+        if (var[0] == 'a') return &o256a;
+        if (var[0] == 'b') return &o256b;
+        if (var[0] == 'c') return &o256c;
+    }
     switch (N) {
         case 256: return &o256;
         case 512: return &o512;

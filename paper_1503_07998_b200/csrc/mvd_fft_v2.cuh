@@ -224,19 +224,18 @@ __global__ void __launch_bounds__(NT, 2) fft2_rows_kernel(RowArgs a, const float
 // ---------------------------------------------------------------------------------------------
 // column pass: forward column FFT, . OTF (or its conjugate), inverse column FFT, in place
 // ---------------------------------------------------------------------------------------------
-// STAGE: the team's slice of the NEXT pair is copied into a staging region with cp.async while the
-// current pair is transformed (costs as much shared memory again as the exchange regions).
-template <class P, int NT, bool OTF_REGS, bool STAGE, int MINB>
+// The team's exchange region doubles as the landing zone of the NEXT item's slice: it is filled by
+// cp.async while the inverse transform runs its register-only last stage and the results are stored.
+template <class P, int NT, bool OTF_REGS, int MINB>
 __global__ void __launch_bounds__(NT, MINB)
 fft2_cols_kernel(float2* __restrict__ S, const float2* __restrict__ otf, int conj_otf, int pairs, int W,
                  const float2* __restrict__ tw_g) {
     constexpr int E = P::E, TPF = P::TPF, H = P::N, TEAM = 4 * TPF, NTEAM = NT / TEAM, TC = 4 * NTEAM;
-    static_assert(NT % TEAM == 0 && TEAM % 32 == 0 && NTEAM <= 15, "column teams are whole warps");
-    static_assert((2 * H) % TEAM == 0, "the staging copy splits evenly over the team");
+    static_assert(NT % TEAM == 0 && TEAM % 32 == 0 && (TEAM == 32 || NTEAM <= 15), "column teams are whole warps");
+    static_assert((2 * H) % TEAM == 0, "the landing copy splits evenly over the team");
     extern __shared__ __align__(16) float2 smem_cols2[];
     float2* tw = smem_cols2;                                  // [(S-1) E][TPF]
-    float2* buf = smem_cols2 + (P::S - 1) * E * TPF;          // [NTEAM][H][4]  exchange regions
-    float2* stage = buf + NTEAM * H * 4;                      // [NTEAM][H][4]  staging regions (STAGE)
+    float2* buf = smem_cols2 + (P::S - 1) * E * TPF;          // [NTEAM][H][4]  exchange regions / landing zones
     for (int k = threadIdx.x; k < (P::S - 1) * E * TPF; k += NT) tw[k] = tw_g[k];
     __syncthreads();
     pdl_launch_dependents();
@@ -245,9 +244,9 @@ fft2_cols_kernel(float2* __restrict__ S, const float2* __restrict__ otf, int con
     const ColAddr2<P> addr{team * H * 4 + c4};
     const TeamSync<TEAM> sync{team};
     const float sgn = conj_otf ? -1.f : 1.f;
-    float2* my_stage = stage + team * H * 4;
-    // Work items (column tile, pair), tile fastest, dealt round-robin to a persistent grid.  With
-    // OTF_REGS the host makes gridDim.x a multiple of the tile count, so a CTA keeps its tile.
+    float2* land = buf + team * H * 4;
+    // Work items (group of TC columns, pair), column group fastest, dealt round-robin to a persistent
+    // grid.  With OTF_REGS the host makes gridDim.x a multiple of the group count: a CTA keeps its columns.
     const int tiles = W / TC;
     const int items = tiles * pairs;
     auto first_col = [&](int item) { return (item % tiles) * TC + team * 4; };
@@ -260,7 +259,7 @@ fft2_cols_kernel(float2* __restrict__ S, const float2* __restrict__ otf, int con
 #pragma unroll
         for (int k = 0; k < 2 * H / TEAM; ++k) {
             const int q = l + TEAM * k;
-            cp_async16(my_stage + 2 * q, src + (size_t)(q >> 1) * 16 + 2 * (q & 1));
+            cp_async16(land + 2 * q, src + (size_t)(q >> 1) * 16 + 2 * (q & 1));
         }
         cp_async_commit();
     };
@@ -276,22 +275,16 @@ fft2_cols_kernel(float2* __restrict__ S, const float2* __restrict__ otf, int con
         }
     }
     pdl_wait();
-    if (STAGE && item < items) issue(item);
+    if (item < items) issue(item);
     for (; item < items; item += gridDim.x) {
         const int xg = first_col(item) + c4;
         float2* Sp = S + (size_t)(item / tiles) * H * W + plane_off(xg);
         float2 x[E];
-        if (STAGE) {
-            cp_async_wait_all();
-            sync();
+        cp_async_wait_all();
+        sync();
 #pragma unroll
-            for (int e = 0; e < E; ++e) x[e] = my_stage[(t + TPF * e) * 4 + c4];
-            sync();
-            if (item + (int)gridDim.x < items) issue(item + gridDim.x);
-        } else {
-#pragma unroll
-            for (int e = 0; e < E; ++e) x[e] = Sp[(size_t)(t + TPF * e) * 16];
-        }
+        for (int e = 0; e < E; ++e) x[e] = land[(t + TPF * e) * 4 + c4];
+        sync();
         fft_run<P, -1>(x, buf, tw, t, addr, sync);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
@@ -304,10 +297,121 @@ fft2_cols_kernel(float2* __restrict__ S, const float2* __restrict__ otf, int con
             }
             x[e] = cmul(x[e], w);
         }
-        fft_run<P, +1>(x, buf, tw, t, addr, sync);
+        fft_run_head<P, +1>(x, buf, tw, t, addr, sync);
+        if (item + (int)gridDim.x < items) issue(item + gridDim.x);
+        fft_run_tail<P, +1>(x, buf, tw, t, addr, sync);
 #pragma unroll
         for (int e = 0; e < E; ++e) Sp[(size_t)(t + TPF * e) * 16] = x[e];
     }
+}
+
+// 2D tiled tensor copy shared -> global (SASS UTMASTG), bulk-group completion
+__device__ __forceinline__ void tma_2d_s2g(const CUtensorMap* map, int x, int y, const void* src) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
+                 ::"l"(map), "r"(x), "r"(y), "r"(smem_u32(src)) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+
+// Column pass fed and drained by the TMA unit.  The spectrum is a 2D tensor of 128-byte rows
+// (tile-major: row index (pair * W/16 + tile) * H + p); a team's slice of an item is the box of
+// 32 bytes x H rows at column offset 8 * (team's column group) floats.  One lane per team issues the
+// box load of the NEXT item into the team's exchange region when the inverse transform has done its
+// last exchange, and the box store of the results from a second region -- no global load or store
+// instruction, and no L1 tag traffic, is left in the loop.
+template <class P, int NT, bool OTF_REGS, int MINB>
+__global__ void __launch_bounds__(NT, MINB)
+fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ otf, int conj_otf,
+                     int pairs, int W, const float2* __restrict__ tw_g) {
+    constexpr int E = P::E, TPF = P::TPF, H = P::N, TEAM = 4 * TPF, NTEAM = NT / TEAM, TC = 4 * NTEAM;
+    constexpr int BOXH = H < 256 ? H : 256;
+    static_assert(NT % TEAM == 0 && TEAM % 32 == 0 && (TEAM == 32 || NTEAM <= 15), "column teams are whole warps");
+    extern __shared__ __align__(128) float2 smem_cols3[];
+    constexpr int TW = (P::S - 1) * E * TPF;                  // a multiple of 16 float2: regions stay 128-byte aligned
+    static_assert(TW % 16 == 0, "twiddle table keeps the regions aligned");
+    float2* tw = smem_cols3;                                  // [(S-1) E][TPF]
+    float2* buf = smem_cols3 + TW;                            // [NTEAM][H][4]  exchange regions / landing zones
+    float2* obuf = buf + NTEAM * H * 4;                       // [NTEAM][H][4]  results on their way out
+    uint64_t* bars = reinterpret_cast<uint64_t*>(obuf + NTEAM * H * 4);   // [NTEAM]
+    if (threadIdx.x < NTEAM) mbar_init(&bars[threadIdx.x], 1);
+    if (threadIdx.x == 0) fence_mbar_init();
+    for (int k = threadIdx.x; k < TW; k += NT) tw[k] = tw_g[k];
+    __syncthreads();
+    pdl_launch_dependents();
+    const int team = threadIdx.x / TEAM, l = threadIdx.x % TEAM;
+    const int c4 = l & 3, t = l >> 2;
+    const ColAddr2<P> addr{team * H * 4 + c4};
+    const TeamSync<TEAM> sync{team};
+    const float sgn = conj_otf ? -1.f : 1.f;
+    float2* land = buf + team * H * 4;
+    float2* outz = obuf + team * H * 4;
+    uint64_t* full = &bars[team];
+    const int tiles = W / TC;            // column groups of TC columns
+    const int items = tiles * pairs;
+    auto first_col = [&](int item) { return (item % tiles) * TC + team * 4; };
+    auto plane_off = [&](int x) { return (size_t)(x >> 4) * (H * 16) + (x & 15); };
+    // tensor coordinates of the team's slice of an item: x in floats within the 128-byte row, y = tile row
+    auto box_x = [&](int item) { return 2 * (first_col(item) & 15); };
+    auto box_y = [&](int item) { return ((item / tiles) * (W / 16) + (first_col(item) >> 4)) * H; };
+    auto issue = [&](int item) {   // one lane
+        fence_proxy_async();
+        mbar_arrive_expect_tx(full, (uint32_t)(sizeof(float2) * H * 4));
+#pragma unroll
+        for (int b = 0; b < H / BOXH; ++b) tma_2d_g2s(land + b * BOXH * 4, &tmap, box_x(item), box_y(item) + b * BOXH, full);
+    };
+
+    int item = blockIdx.x;
+    float2 o[OTF_REGS ? E : 1];
+    if (OTF_REGS && item < items) {   // the OTF is written once in mvd_create: no dependency on the previous kernel
+        const int xg = first_col(item) + c4;
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            o[e] = __ldg(otf + plane_off(xg) + (size_t)(t + TPF * e) * 16);
+            o[e].y *= sgn;
+        }
+    }
+    pdl_wait();
+    if (item < items && l == 0) issue(item);
+    uint32_t phase = 0;
+    for (; item < items; item += gridDim.x) {
+        const int xg = first_col(item) + c4;
+        float2 x[E];
+        mbar_wait(full, phase);
+        phase ^= 1;
+#pragma unroll
+        for (int e = 0; e < E; ++e) x[e] = land[(t + TPF * e) * 4 + c4];
+        sync();
+        fft_run<P, -1>(x, buf, tw, t, addr, sync);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            float2 w;
+            if (OTF_REGS) {
+                w = o[e];
+            } else {
+                w = __ldg(otf + plane_off(xg) + (size_t)(t + TPF * e) * 16);
+                w.y *= sgn;
+            }
+            x[e] = cmul(x[e], w);
+        }
+        fft_run_head<P, +1>(x, buf, tw, t, addr, sync);
+        if (l == 0) {
+            if (item + (int)gridDim.x < items) issue(item + gridDim.x);
+            bulk_wait_read();            // the previous item's results have left the out region
+        }
+        fft_run_tail<P, +1>(x, buf, tw, t, addr, sync);
+        sync();                          // ... and every thread of the team knows it
+#pragma unroll
+        for (int e = 0; e < E; ++e) outz[(t + TPF * e) * 4 + c4] = x[e];
+        fence_proxy_async();
+        sync();
+        if (l == 0) {
+#pragma unroll
+            for (int b = 0; b < H / BOXH; ++b) tma_2d_s2g(&tmap, box_x(item), box_y(item) + b * BOXH, outz + b * BOXH * 4);
+            bulk_commit();
+        }
+    }
+    if (l == 0) bulk_wait_read();
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -328,21 +432,25 @@ inline cudaError_t launch_pdl(Kern kern, dim3 grid, dim3 block, size_t smem, cud
     return cudaLaunchKernelEx(&cfg, kern, args...);
 }
 
-template <class P, int NT, class PC, int NTC, bool OTF_REGS, bool STAGE, int MINB>
+template <class P, int NT, class PC, int NTC, bool OTF_REGS, int MINB, bool TMA = true>
 struct OpsFor2 {
     static_assert(P::N == PC::N, "row and column plan of one entry describe the same length");
     static constexpr size_t kRowSmem = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * P::N);
     static constexpr int kTeam = 4 * PC::TPF, kNTeam = NTC / kTeam, kTC = 4 * kNTeam;
-    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)(STAGE ? 2 : 1) * kNTeam * PC::N * 4);
+    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)(TMA ? 2 : 1) * kNTeam * PC::N * 4) +
+                                       (TMA ? sizeof(uint64_t) * kNTeam : 0);
 
     static cudaError_t rows(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st) {
         if (mode == ROWS_FIRST) return launch_pdl(fft2_rows_kernel<P, ROWS_FIRST, NT>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
         if (mode == ROWS_RATIO) return launch_pdl(fft2_rows_kernel<P, ROWS_RATIO, NT>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
         return launch_pdl(fft2_rows_kernel<P, ROWS_UPDATE, NT>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
     }
-    static cudaError_t cols(const CUtensorMap&, float2* S, const float2* otf, int conj_otf, int pairs, int W,
+    static cudaError_t cols(const CUtensorMap& tmap, float2* S, const float2* otf, int conj_otf, int pairs, int W,
                             const float2* tw, dim3 grid, cudaStream_t st) {
-        return launch_pdl(fft2_cols_kernel<PC, NTC, OTF_REGS, STAGE, MINB>, grid, dim3(NTC), kColSmem, st, S, otf, conj_otf, pairs, W, tw);
+        if constexpr (TMA)
+            return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB>, grid, dim3(NTC), kColSmem, st, tmap, otf, conj_otf, pairs, W, tw);
+        else
+        return launch_pdl(fft2_cols_kernel<PC, NTC, OTF_REGS, MINB>, grid, dim3(NTC), kColSmem, st, S, otf, conj_otf, pairs, W, tw);
     }
     static cudaError_t prepare_rows() {
         cudaError_t e;
@@ -353,7 +461,10 @@ struct OpsFor2 {
         return cudaFuncSetAttribute(fft2_rows_kernel<P, ROWS_UPDATE, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
     }
     static cudaError_t prepare_cols() {
-        return cudaFuncSetAttribute(fft2_cols_kernel<PC, NTC, OTF_REGS, STAGE, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
+        if constexpr (TMA)
+            return cudaFuncSetAttribute(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
+        else
+        return cudaFuncSetAttribute(fft2_cols_kernel<PC, NTC, OTF_REGS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
     }
     static SizeOps make() {
         SizeOps o;
@@ -362,7 +473,7 @@ struct OpsFor2 {
         o.col = PlanInfo{PC::E, PC::TPF, PC::S, {PC::radix(0), PC::radix(1), PC::radix(2), PC::radix(3), PC::radix(4)}};
         o.row_threads = NT;
         o.row_smem = kRowSmem;
-        o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = 0;
+        o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = TMA ? (PC::N < 256 ? PC::N : 256) : 0;
         o.rows = &rows; o.cols = &cols; o.prepare_rows = &prepare_rows; o.prepare_cols = &prepare_cols;
         o.generation = 2;
         o.row_cps = 2;
