@@ -42,7 +42,7 @@ UNIT = "Mvoxel/s"
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); 2 = configs[1]")
@@ -195,7 +195,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_1503_07998_b200 import binding, build
+    from paper_1503_07998_b200 import binding, build, shard
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -255,11 +255,8 @@ def main():
     launches = m.launch_count()
     ms = e0.elapsed_time(e1)
     clocks = sampler.summary(t_wall0, t_wall1)
-    tms = torch.tensor([ms], device="cuda")
-    if world > 1:
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-    ms_max = float(tms.item())
-    value = units * world * args.steps / (ms_max * 1e-3) / 1e6
+    ms_max = shard.max_over_ranks(ms, device="cuda")          # device time of the slowest rank
+    value = shard.job_throughput(units * args.steps, ms_max * 1e-3, world) / 1e6
 
     # ---- per-kernel durations (CUDA events inside the library, launching stream) ------------
     m.profile_enable(True)
@@ -305,11 +302,8 @@ def main():
             m.deconvolve_host(host_in, host_out, N)
         torch.cuda.synchronize()
         dt = time.perf_counter() - t0
-        tt = torch.tensor([dt], device="cuda")
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        dt = float(tt.item())
-        e2e = {"value": units * world * args.steps / dt / 1e6, "unit": UNIT,
+        dt = shard.max_over_ranks(dt, device="cuda")
+        e2e = {"value": shard.job_throughput(units * args.steps, dt, world) / 1e6, "unit": UNIT,
                "h2d_bytes_per_step": int(views.nbytes), "d2h_bytes_per_step": int(host_out.numel() * 4),
                "ms_per_step": dt * 1e3 / args.steps, "ratio_to_device_resident": None}
         e2e["ratio_to_device_resident"] = e2e["value"] / value
