@@ -29,7 +29,12 @@ const SizeOps* find_ops_v1(int N) {
     if (const SizeOps* o = mvd_fft_ops_mid(N)) return o;
     return mvd_fft_ops_large(N);
 }
-bool use_v2(int W, int H) { return want_v2() && mvd_fft_ops_v2(W) && mvd_fft_ops_v2(H); }
+bool use_v2(int W, int H) {
+    if (!want_v2()) return false;
+    const SizeOps* r = mvd_fft_ops_v2(W);
+    const SizeOps* c = mvd_fft_ops_v2(H);
+    return r && c && r->rows && c->cols;
+}
 const SizeOps* find_row_ops(int W, int H) { return use_v2(W, H) ? mvd_fft_ops_v2(W) : find_ops_v1(W); }
 const SizeOps* find_col_ops(int W, int H) { return use_v2(W, H) ? mvd_fft_ops_v2(H) : find_ops_v1(H); }
 
@@ -115,7 +120,7 @@ int make_col_tensor_map(mvd_handle* h, const FftState* st, float2* S, int pairs,
     const cuuint64_t dims[2] = {v2 ? (cuuint64_t)32 : (cuuint64_t)2 * h->W,
                                 v2 ? (cuuint64_t)pairs * (h->W / 16) * h->H : (cuuint64_t)pairs * h->H};
     const cuuint64_t strides[1] = {v2 ? (cuuint64_t)128 : (cuuint64_t)h->W * sizeof(float2)};
-    const cuuint32_t box[2] = {v2 ? 8u : (cuuint32_t)(2 * st->col->col_tc), (cuuint32_t)st->col->col_box_h};
+    const cuuint32_t box[2] = {v2 ? (cuuint32_t)st->col->col_box_w : (cuuint32_t)(2 * st->col->col_tc), (cuuint32_t)st->col->col_box_h};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = st->encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, S, dims, strides, box, estr,
                                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,

@@ -10,10 +10,12 @@ const SizeOps* mvd_fft_ops_v2(int N) {
     using P1024 = Plan<1024, 32, 32, 32>;
     using P2048 = Plan<2048, 32, 32, 32, 2>;
     using P256C = Plan<256, 32, 32, 8>;      // column plan: four columns per warp, E = 32
-    static const SizeOps o256 = OpsFor2<P256, 256, P256, 256, true, 2>::make();
+    static const SizeOps o256 = OpsFor2<P256, 256, P256, 128, true, 4>::make();
     static const SizeOps o512 = OpsFor2<P512, 256, P512, 128, false, 3>::make();
     static const SizeOps o1024 = OpsFor2<P1024, 256, P1024, 128, false, 3>::make();
     static const SizeOps o2048 = OpsFor2<P2048, 256, P2048, 256, false, 2, false>::make();
+    using P800C = Plan<800, 40, 40, 20>;     // columns only: eight columns per team of 160 threads
+    static const SizeOps o800 = ColsOnly2<P800C, 160, false, 2, 8>::make();
     // measurement knob: alternative column kernels for 256
     static const SizeOps o256a = OpsFor2<P256, 256, P256, 256, true, 2, false>::make();
     static const SizeOps o256b = OpsFor2<P256, 256, P256C, 256, false, 2>::make();
@@ -27,6 +29,7 @@ const SizeOps* mvd_fft_ops_v2(int N) {
     switch (N) {
         case 256: return &o256;
         case 512: return &o512;
+        case 800: return &o800;
         case 1024: return &o1024;
         case 2048: return &o2048;
         default: return nullptr;

@@ -283,6 +283,58 @@ struct Bfly<32, DIR> {
     }
 };
 
+// cos / sin of 2 pi k / 40 as compile-time constants (k any integer)
+__host__ __device__ constexpr float cos40(int k) {
+    constexpr float C[11] = {1.0f, 0.98768834059513777035f, 0.95105651629515357212f, 0.89100652418836786236f,
+                             0.80901699437494742410f, 0.70710678118654752440f, 0.58778525229247312917f,
+                             0.45399049973954679156f, 0.30901699437494742410f, 0.15643446504023086901f, 0.0f};
+    k = ((k % 40) + 40) % 40;
+    if (k > 20) k = 40 - k;
+    return k > 10 ? -C[20 - k] : C[k];
+}
+__host__ __device__ constexpr float sin40(int k) { return cos40(k - 10); }
+
+// Composite butterfly of length RA * 5 (RA = 4 or 8): n = n1 + 5 n2 (n1 < 5, n2 < RA), f = f2 + RA f1;
+// RA-point transforms over n2, twiddles w^(n1 f2) with w = exp(DIR 2 pi i / (5 RA)), 5-point transforms over n1.
+template <int RA, int DIR>
+struct BflyTimes5 {
+    static __device__ __forceinline__ void run(float2* v) {
+        constexpr int N = 5 * RA, Q = 40 / N;   // w_N^k = w_40^(Q k)
+        float2 a[5][RA];
+#pragma unroll
+        for (int n1 = 0; n1 < 5; ++n1) {
+            float2 t[RA];
+#pragma unroll
+            for (int n2 = 0; n2 < RA; ++n2) t[n2] = v[n1 + 5 * n2];
+            Bfly<RA, DIR>::run(t);
+#pragma unroll
+            for (int f2 = 0; f2 < RA; ++f2) a[n1][f2] = t[f2];
+        }
+#pragma unroll
+        for (int n1 = 1; n1 < 5; ++n1) {
+#pragma unroll
+            for (int f2 = 1; f2 < RA; ++f2) {
+                const int k = Q * n1 * f2;
+                if (k % 40 == 10) a[n1][f2] = rot90<DIR>(a[n1][f2]);
+                else if (k % 40 == 5) a[n1][f2] = rot45<DIR>(a[n1][f2]);
+                else if (k % 40 == 15) a[n1][f2] = rot135<DIR>(a[n1][f2]);
+                else a[n1][f2] = cmul(a[n1][f2], make_float2(cos40(k), (DIR < 0 ? -1.f : 1.f) * sin40(k)));
+            }
+        }
+#pragma unroll
+        for (int f2 = 0; f2 < RA; ++f2) {
+            float2 t[5] = {a[0][f2], a[1][f2], a[2][f2], a[3][f2], a[4][f2]};
+            Bfly<5, DIR>::run(t);
+#pragma unroll
+            for (int f1 = 0; f1 < 5; ++f1) v[f2 + RA * f1] = t[f1];
+        }
+    }
+};
+template <int DIR>
+struct Bfly<20, DIR> : BflyTimes5<4, DIR> {};
+template <int DIR>
+struct Bfly<40, DIR> : BflyTimes5<8, DIR> {};
+
 // ---------------------------------------------------------------------------------------------
 // plans
 // ---------------------------------------------------------------------------------------------
@@ -747,6 +799,7 @@ struct SizeOps {
                         const float2* tw, dim3 grid, cudaStream_t st);
     cudaError_t (*prepare_rows)();   // opt in to > 48 KB dynamic shared memory (length used as W)
     cudaError_t (*prepare_cols)();   // same (length used as H)
+    int col_box_w = 0;               // generation 2: floats per TMA box row (2 x columns per team)
     int col_otf_regs = 0;            // generation 2: the column kernel keeps its tile's OTF in registers
     int row_cps = 0, col_cps = 0;    // generation 2: resident CTAs per SM the persistent grids are sized for
     int generation = 1;              // 1: CTA-synchronous TMA-staged kernels (this file); 2: team kernels (mvd_fft_v2.cuh)

@@ -37,8 +37,10 @@ __device__ __forceinline__ void prefetch_l2(const void* p, uint32_t bytes) {
 template <class P>
 __device__ __forceinline__ int swz(int p) {
     constexpr int R0 = P::radix(0);
-    static_assert(R0 == 16 || R0 == 32, "the XOR swizzle is derived for first radices 16 and 32");
-    return p ^ ((p / R0) & 15);
+    static_assert(R0 == 16 || R0 == 32 || R0 == 40, "the XOR swizzle is derived for first radices 16, 32 and 40");
+    // R0 = 40 (length 800, eight columns per team, two positions per half-warp): only the parity has to
+    // differ between neighbouring threads of stage 0 (positions 40 t + m), and p ^ 1 stays inside its block of 40
+    return R0 == 40 ? p ^ ((p / R0) & 1) : p ^ ((p / R0) & 15);
 }
 // one FFT per region of N slots
 template <class P>
@@ -46,11 +48,11 @@ struct RowAddr2 {
     int base;
     __device__ __forceinline__ int operator()(int pos) const { return base + swz<P>(pos); }
 };
-// four FFTs (adjacent columns) interleaved: [slot][4]
-template <class P>
+// CPT FFTs (adjacent columns) interleaved: [slot][CPT]
+template <class P, int CPT = 4>
 struct ColAddr2 {
     int base;   // team region + column within the team
-    __device__ __forceinline__ int operator()(int pos) const { return base + 4 * swz<P>(pos); }
+    __device__ __forceinline__ int operator()(int pos) const { return base + CPT * swz<P>(pos); }
 };
 
 // 16-byte asynchronous copy global -> shared (SASS LDGSTS), no registers in between
@@ -320,45 +322,46 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // box load of the NEXT item into the team's exchange region when the inverse transform has done its
 // last exchange, and the box store of the results from a second region -- no global load or store
 // instruction, and no L1 tag traffic, is left in the loop.
-template <class P, int NT, bool OTF_REGS, int MINB>
+template <class P, int NT, bool OTF_REGS, int MINB, int CPT = 4>
 __global__ void __launch_bounds__(NT, MINB)
 fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ otf, int conj_otf,
                      int pairs, int W, const float2* __restrict__ tw_g) {
-    constexpr int E = P::E, TPF = P::TPF, H = P::N, TEAM = 4 * TPF, NTEAM = NT / TEAM, TC = 4 * NTEAM;
-    constexpr int BOXH = H < 256 ? H : 256;
+    constexpr int E = P::E, TPF = P::TPF, H = P::N, TEAM = CPT * TPF, NTEAM = NT / TEAM, TC = CPT * NTEAM;
+    constexpr int BOXH = H <= 256 ? H : (H % 256 == 0 ? 256 : 200);
+    static_assert(H % BOXH == 0 && (CPT == 4 || CPT == 8), "whole boxes; a team owns one or two 32-byte sectors per row");
     static_assert(NT % TEAM == 0 && TEAM % 32 == 0 && (TEAM == 32 || NTEAM <= 15), "column teams are whole warps");
     extern __shared__ __align__(128) float2 smem_cols3[];
     constexpr int TW = (P::S - 1) * E * TPF;                  // a multiple of 16 float2: regions stay 128-byte aligned
     static_assert(TW % 16 == 0, "twiddle table keeps the regions aligned");
     float2* tw = smem_cols3;                                  // [(S-1) E][TPF]
-    float2* buf = smem_cols3 + TW;                            // [NTEAM][H][4]  exchange regions / landing zones
-    float2* obuf = buf + NTEAM * H * 4;                       // [NTEAM][H][4]  results on their way out
-    uint64_t* bars = reinterpret_cast<uint64_t*>(obuf + NTEAM * H * 4);   // [NTEAM]
+    float2* buf = smem_cols3 + TW;                            // [NTEAM][H][CPT]  exchange regions / landing zones
+    float2* obuf = buf + NTEAM * H * CPT;                     // [NTEAM][H][CPT]  results on their way out
+    uint64_t* bars = reinterpret_cast<uint64_t*>(obuf + NTEAM * H * CPT);   // [NTEAM]
     if (threadIdx.x < NTEAM) mbar_init(&bars[threadIdx.x], 1);
     if (threadIdx.x == 0) fence_mbar_init();
     for (int k = threadIdx.x; k < TW; k += NT) tw[k] = tw_g[k];
     __syncthreads();
     pdl_launch_dependents();
     const int team = threadIdx.x / TEAM, l = threadIdx.x % TEAM;
-    const int c4 = l & 3, t = l >> 2;
-    const ColAddr2<P> addr{team * H * 4 + c4};
+    const int c4 = l % CPT, t = l / CPT;
+    const ColAddr2<P, CPT> addr{team * H * CPT + c4};
     const TeamSync<TEAM> sync{team};
     const float sgn = conj_otf ? -1.f : 1.f;
-    float2* land = buf + team * H * 4;
-    float2* outz = obuf + team * H * 4;
+    float2* land = buf + team * H * CPT;
+    float2* outz = obuf + team * H * CPT;
     uint64_t* full = &bars[team];
     const int tiles = W / TC;            // column groups of TC columns
     const int items = tiles * pairs;
-    auto first_col = [&](int item) { return (item % tiles) * TC + team * 4; };
+    auto first_col = [&](int item) { return (item % tiles) * TC + team * CPT; };
     auto plane_off = [&](int x) { return (size_t)(x >> 4) * (H * 16) + (x & 15); };
     // tensor coordinates of the team's slice of an item: x in floats within the 128-byte row, y = tile row
     auto box_x = [&](int item) { return 2 * (first_col(item) & 15); };
     auto box_y = [&](int item) { return ((item / tiles) * (W / 16) + (first_col(item) >> 4)) * H; };
     auto issue = [&](int item) {   // one lane
         fence_proxy_async();
-        mbar_arrive_expect_tx(full, (uint32_t)(sizeof(float2) * H * 4));
+        mbar_arrive_expect_tx(full, (uint32_t)(sizeof(float2) * H * CPT));
 #pragma unroll
-        for (int b = 0; b < H / BOXH; ++b) tma_2d_g2s(land + b * BOXH * 4, &tmap, box_x(item), box_y(item) + b * BOXH, full);
+        for (int b = 0; b < H / BOXH; ++b) tma_2d_g2s(land + b * BOXH * CPT, &tmap, box_x(item), box_y(item) + b * BOXH, full);
     };
 
     int item = blockIdx.x;
@@ -380,7 +383,7 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __r
         mbar_wait(full, phase);
         phase ^= 1;
 #pragma unroll
-        for (int e = 0; e < E; ++e) x[e] = land[(t + TPF * e) * 4 + c4];
+        for (int e = 0; e < E; ++e) x[e] = land[(t + TPF * e) * CPT + c4];
         sync();
         fft_run<P, -1>(x, buf, tw, t, addr, sync);
 #pragma unroll
@@ -402,12 +405,12 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __r
         fft_run_tail<P, +1>(x, buf, tw, t, addr, sync);
         sync();                          // ... and every thread of the team knows it
 #pragma unroll
-        for (int e = 0; e < E; ++e) outz[(t + TPF * e) * 4 + c4] = x[e];
+        for (int e = 0; e < E; ++e) outz[(t + TPF * e) * CPT + c4] = x[e];
         fence_proxy_async();
         sync();
         if (l == 0) {
 #pragma unroll
-            for (int b = 0; b < H / BOXH; ++b) tma_2d_s2g(&tmap, box_x(item), box_y(item) + b * BOXH, outz + b * BOXH * 4);
+            for (int b = 0; b < H / BOXH; ++b) tma_2d_s2g(&tmap, box_x(item), box_y(item) + b * BOXH, outz + b * BOXH * CPT);
             bulk_commit();
         }
     }
@@ -473,12 +476,40 @@ struct OpsFor2 {
         o.col = PlanInfo{PC::E, PC::TPF, PC::S, {PC::radix(0), PC::radix(1), PC::radix(2), PC::radix(3), PC::radix(4)}};
         o.row_threads = NT;
         o.row_smem = kRowSmem;
-        o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = TMA ? (PC::N < 256 ? PC::N : 256) : 0;
+        o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = TMA ? (PC::N < 256 ? PC::N : 256) : 0; o.col_box_w = 8;
         o.rows = &rows; o.cols = &cols; o.prepare_rows = &prepare_rows; o.prepare_cols = &prepare_cols;
         o.generation = 2;
         o.row_cps = 2;
         o.col_cps = MINB;
         o.col_otf_regs = OTF_REGS ? 1 : 0;
+        return o;
+    }
+};
+
+// A length that only has a generation-2 COLUMN kernel (800 = 40 x 20: its 20-thread FFTs are not
+// warp-aligned, so eight columns form a team of five warps).
+template <class PC, int NTC, bool OTF_REGS, int MINB, int CPT>
+struct ColsOnly2 {
+    static constexpr int kTeam = CPT * PC::TPF, kNTeam = NTC / kTeam, kTC = CPT * kNTeam;
+    static constexpr int kBoxH = PC::N <= 256 ? PC::N : (PC::N % 256 == 0 ? 256 : 200);
+    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)2 * kNTeam * PC::N * CPT) +
+                                       sizeof(uint64_t) * kNTeam;
+    static cudaError_t cols(const CUtensorMap& tmap, float2*, const float2* otf, int conj_otf, int pairs, int W,
+                            const float2* tw, dim3 grid, cudaStream_t st) {
+        return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, grid, dim3(NTC), kColSmem, st, tmap, otf, conj_otf, pairs, W, tw);
+    }
+    static cudaError_t prepare_cols() {
+        return cudaFuncSetAttribute(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
+    }
+    static SizeOps make() {
+        SizeOps o;
+        o.N = PC::N;
+        o.row = PlanInfo{0, 0, 0, {0, 0, 0, 0, 0}};
+        o.col = PlanInfo{PC::E, PC::TPF, PC::S, {PC::radix(0), PC::radix(1), PC::radix(2), PC::radix(3), PC::radix(4)}};
+        o.row_threads = 0; o.row_smem = 0;
+        o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = kBoxH; o.col_box_w = 2 * CPT;
+        o.rows = nullptr; o.cols = &cols; o.prepare_rows = nullptr; o.prepare_cols = &prepare_cols;
+        o.generation = 2; o.row_cps = 0; o.col_cps = MINB; o.col_otf_regs = OTF_REGS ? 1 : 0;
         return o;
     }
 };
