@@ -17,8 +17,8 @@ const SizeOps* mvd_fft_ops_v2(int N) {
     using P800C = Plan<800, 40, 40, 20>;     // columns only: eight columns per team of 160 threads
     static const SizeOps o800 = ColsOnly2<P800C, 160, false, 2, 8>::make();
     // measurement knob: alternative column kernels for 256
-    static const SizeOps o256a = OpsFor2<P256, 256, P256, 256, true, 2, false>::make();
-    static const SizeOps o256b = OpsFor2<P256, 256, P256C, 256, false, 2>::make();
+    static const SizeOps o256a = OpsFor2<P256, 256, P256, 128, true, 4, true, 8>::make();
+    static const SizeOps o256b = OpsFor2<P256, 256, P256, 256, true, 2, true, 16>::make();
     static const SizeOps o256c = OpsFor2<P256, 256, P256, 128, true, 4>::make();
     static const char* var = getenv("MVD_COLS_VARIANT");
     if (N == 256 && var) {

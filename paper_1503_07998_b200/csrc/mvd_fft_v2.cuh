@@ -328,7 +328,7 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __r
                      int pairs, int W, const float2* __restrict__ tw_g) {
     constexpr int E = P::E, TPF = P::TPF, H = P::N, TEAM = CPT * TPF, NTEAM = NT / TEAM, TC = CPT * NTEAM;
     constexpr int BOXH = H <= 256 ? H : (H % 256 == 0 ? 256 : 200);
-    static_assert(H % BOXH == 0 && (CPT == 4 || CPT == 8), "whole boxes; a team owns one or two 32-byte sectors per row");
+    static_assert(H % BOXH == 0 && (CPT == 4 || CPT == 8 || CPT == 16), "whole boxes; a team owns whole 32-byte sectors of a row");
     static_assert(NT % TEAM == 0 && TEAM % 32 == 0 && (TEAM == 32 || NTEAM <= 15), "column teams are whole warps");
     extern __shared__ __align__(128) float2 smem_cols3[];
     constexpr int TW = (P::S - 1) * E * TPF;                  // a multiple of 16 float2: regions stay 128-byte aligned
@@ -435,12 +435,12 @@ inline cudaError_t launch_pdl(Kern kern, dim3 grid, dim3 block, size_t smem, cud
     return cudaLaunchKernelEx(&cfg, kern, args...);
 }
 
-template <class P, int NT, class PC, int NTC, bool OTF_REGS, int MINB, bool TMA = true>
+template <class P, int NT, class PC, int NTC, bool OTF_REGS, int MINB, bool TMA = true, int CPT = 4>
 struct OpsFor2 {
     static_assert(P::N == PC::N, "row and column plan of one entry describe the same length");
     static constexpr size_t kRowSmem = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * P::N);
-    static constexpr int kTeam = 4 * PC::TPF, kNTeam = NTC / kTeam, kTC = 4 * kNTeam;
-    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)(TMA ? 2 : 1) * kNTeam * PC::N * 4) +
+    static constexpr int kTeam = CPT * PC::TPF, kNTeam = NTC / kTeam, kTC = CPT * kNTeam;
+    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)(TMA ? 2 : 1) * kNTeam * PC::N * CPT) +
                                        (TMA ? sizeof(uint64_t) * kNTeam : 0);
 
     static cudaError_t rows(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st) {
@@ -451,7 +451,7 @@ struct OpsFor2 {
     static cudaError_t cols(const CUtensorMap& tmap, float2* S, const float2* otf, int conj_otf, int pairs, int W,
                             const float2* tw, dim3 grid, cudaStream_t st) {
         if constexpr (TMA)
-            return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB>, grid, dim3(NTC), kColSmem, st, tmap, otf, conj_otf, pairs, W, tw);
+            return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, grid, dim3(NTC), kColSmem, st, tmap, otf, conj_otf, pairs, W, tw);
         else
         return launch_pdl(fft2_cols_kernel<PC, NTC, OTF_REGS, MINB>, grid, dim3(NTC), kColSmem, st, S, otf, conj_otf, pairs, W, tw);
     }
@@ -465,7 +465,7 @@ struct OpsFor2 {
     }
     static cudaError_t prepare_cols() {
         if constexpr (TMA)
-            return cudaFuncSetAttribute(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
+            return cudaFuncSetAttribute(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
         else
         return cudaFuncSetAttribute(fft2_cols_kernel<PC, NTC, OTF_REGS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
     }
@@ -476,7 +476,7 @@ struct OpsFor2 {
         o.col = PlanInfo{PC::E, PC::TPF, PC::S, {PC::radix(0), PC::radix(1), PC::radix(2), PC::radix(3), PC::radix(4)}};
         o.row_threads = NT;
         o.row_smem = kRowSmem;
-        o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = TMA ? (PC::N < 256 ? PC::N : 256) : 0; o.col_box_w = 8;
+        o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = TMA ? (PC::N < 256 ? PC::N : 256) : 0; o.col_box_w = 2 * CPT;
         o.rows = &rows; o.cols = &cols; o.prepare_rows = &prepare_rows; o.prepare_cols = &prepare_cols;
         o.generation = 2;
         o.row_cps = 2;

@@ -105,6 +105,11 @@ def test_large_configs_against_stored_oracle_planes(cid):
     (2, 2, 64, 1024, 5, 2, "random"),    # config 5's column length
     (2, 2, 1024, 512, 5, 1, "sparse"),   # config 3's plane
     (2, 2, 32, 2048, 5, 1, "random"),    # longest column transform
+    (2, 3, 512, 256, 9, 2, "random"),    # generation-2 kernels, odd plane count (half-empty last pair)
+    (1, 2, 256, 2048, 5, 1, "random"),   # generation 2: 2048-point columns (cp.async column kernel)
+    (2, 1, 2048, 256, 7, 2, "random"),   # generation 2: 2048-point rows, a single plane
+    (3, 5, 256, 256, 11, 2, "sparse"),   # generation 2: 256 x 256, three views
+    (2, 2, 1024, 1024, 7, 1, "random"),  # generation 2: config 5's plane with an asymmetric PSF
 ])
 def test_asymmetric_and_ragged(path, V, N, W, H, K, T, psf):
     _need(path, W, H, K)
@@ -180,6 +185,25 @@ def test_chunking_and_host_pipeline_are_bit_identical(path):
     assert np.array_equal(base, _run(pr.views, pr.psfs, T, path, host=True))
     assert np.array_equal(base, _run(pr.views, pr.psfs, T, path, host=True, batch_planes=2, chunk_planes=2))
     assert np.array_equal(base, _run(pr.views, pr.psfs, T, path, host=True, batch_planes=5))
+
+
+def test_generation2_is_deterministic_and_independent_of_batching():
+    """The team-synchronous kernels (private exchange regions, cp.async / TMA landing zones, persistent
+    grids) must give the same bits run after run and for every chunk / batch split: a missing team
+    barrier or an early landing shows up here as a flipped bit.  compute-sanitizer is not available
+    on the GPU pool, so this is the race check."""
+    V, N, W, H, K, T = 2, 11, 512, 256, 9, 3
+    pr = synth.make_problem(V, N, W, H, K, T, seed=123)
+    base = _run(pr.views, pr.psfs, T, binding.PATH_FFT)
+    for _ in range(4):
+        assert np.array_equal(base, _run(pr.views, pr.psfs, T, binding.PATH_FFT))
+    assert np.array_equal(base, _run(pr.views, pr.psfs, T, binding.PATH_FFT, chunk_planes=4))
+    assert np.array_equal(base, _run(pr.views, pr.psfs, T, binding.PATH_FFT, chunk_planes=2))
+    assert np.array_equal(base, _run(pr.views, pr.psfs, T, binding.PATH_FFT, host=True))
+    assert np.array_equal(base, _run(pr.views, pr.psfs, T, binding.PATH_FFT, host=True, batch_planes=2, chunk_planes=2))
+    assert np.array_equal(base, _run(pr.views, pr.psfs, T, binding.PATH_FFT, host=True, batch_planes=6))
+    ref = mvd_oracle.deconvolve(pr.views, pr.psfs, T, pr.eps)
+    assert_parity(base, ref, "generation 2, 512x256")
 
 
 @pytest.mark.parametrize("path", PATHS)
