@@ -13,7 +13,7 @@ const SizeOps* mvd_fft_ops_v2(int N) {
     static const SizeOps o256 = OpsFor2<P256, 256, P256, 128, true, 4>::make();
     static const SizeOps o512 = OpsFor2<P512, 256, P512, 128, false, 3>::make();
     static const SizeOps o1024 = OpsFor2<P1024, 256, P1024, 128, false, 3>::make();
-    static const SizeOps o2048 = OpsFor2<P2048, 256, P2048, 256, false, 2, false>::make();
+    static const SizeOps o2048 = OpsFor2<P2048, 128, P2048, 256, false, 2, false, 4, 3>::make();   // rows: 3 CTAs of 2 teams, 168 registers
     using P800C = Plan<800, 40, 40, 20>;     // columns only: eight columns per team of 160 threads
     static const SizeOps o800 = ColsOnly2<P800C, 160, false, 2, 8>::make();
     // measurement knob: alternative column kernels for 256

@@ -71,8 +71,8 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 //     [S row landed]  -> registers -> inverse FFT head | issue phi / psi row | inverse FFT tail
 //     [aux landed]    -> pointwise step               -> forward FFT head | issue next S row | tail -> store
 // ---------------------------------------------------------------------------------------------
-template <class P, int MODE, int NT>
-__global__ void __launch_bounds__(NT, 2) fft2_rows_kernel(RowArgs a, const float2* __restrict__ tw_g) {
+template <class P, int MODE, int NT, int RMINB = 2>
+__global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const float2* __restrict__ tw_g) {
     constexpr int E = P::E, TPF = P::TPF, W = P::N, RP = NT / TPF;
     static_assert(NT % TPF == 0 && (TPF <= 32 ? 32 % TPF == 0 : TPF % 32 == 0), "teams are warp-aligned");
     static_assert(TPF % 16 == 0 && W % 16 == 0, "tile-major addressing assumes whole 16-element groups per team step");
@@ -435,7 +435,7 @@ inline cudaError_t launch_pdl(Kern kern, dim3 grid, dim3 block, size_t smem, cud
     return cudaLaunchKernelEx(&cfg, kern, args...);
 }
 
-template <class P, int NT, class PC, int NTC, bool OTF_REGS, int MINB, bool TMA = true, int CPT = 4>
+template <class P, int NT, class PC, int NTC, bool OTF_REGS, int MINB, bool TMA = true, int CPT = 4, int RMINB = 2>
 struct OpsFor2 {
     static_assert(P::N == PC::N, "row and column plan of one entry describe the same length");
     static constexpr size_t kRowSmem = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * P::N);
@@ -444,9 +444,9 @@ struct OpsFor2 {
                                        (TMA ? sizeof(uint64_t) * kNTeam : 0);
 
     static cudaError_t rows(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st) {
-        if (mode == ROWS_FIRST) return launch_pdl(fft2_rows_kernel<P, ROWS_FIRST, NT>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
-        if (mode == ROWS_RATIO) return launch_pdl(fft2_rows_kernel<P, ROWS_RATIO, NT>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
-        return launch_pdl(fft2_rows_kernel<P, ROWS_UPDATE, NT>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
+        if (mode == ROWS_FIRST) return launch_pdl(fft2_rows_kernel<P, ROWS_FIRST, NT, RMINB>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
+        if (mode == ROWS_RATIO) return launch_pdl(fft2_rows_kernel<P, ROWS_RATIO, NT, RMINB>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
+        return launch_pdl(fft2_rows_kernel<P, ROWS_UPDATE, NT, RMINB>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
     }
     static cudaError_t cols(const CUtensorMap& tmap, float2* S, const float2* otf, int conj_otf, int pairs, int W,
                             const float2* tw, dim3 grid, cudaStream_t st) {
@@ -457,11 +457,11 @@ struct OpsFor2 {
     }
     static cudaError_t prepare_rows() {
         cudaError_t e;
-        e = cudaFuncSetAttribute(fft2_rows_kernel<P, ROWS_FIRST, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
+        e = cudaFuncSetAttribute(fft2_rows_kernel<P, ROWS_FIRST, NT, RMINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(fft2_rows_kernel<P, ROWS_RATIO, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
+        e = cudaFuncSetAttribute(fft2_rows_kernel<P, ROWS_RATIO, NT, RMINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
         if (e != cudaSuccess) return e;
-        return cudaFuncSetAttribute(fft2_rows_kernel<P, ROWS_UPDATE, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
+        return cudaFuncSetAttribute(fft2_rows_kernel<P, ROWS_UPDATE, NT, RMINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
     }
     static cudaError_t prepare_cols() {
         if constexpr (TMA)
@@ -479,7 +479,7 @@ struct OpsFor2 {
         o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = TMA ? (PC::N < 256 ? PC::N : 256) : 0; o.col_box_w = 2 * CPT;
         o.rows = &rows; o.cols = &cols; o.prepare_rows = &prepare_rows; o.prepare_cols = &prepare_cols;
         o.generation = 2;
-        o.row_cps = 2;
+        o.row_cps = RMINB;
         o.col_cps = MINB;
         o.col_otf_regs = OTF_REGS ? 1 : 0;
         return o;
