@@ -32,7 +32,9 @@
  * Pins (tests/test_oracle_pins.py, run with -m "not gpu"): P1 centred delta, P2 off-centre delta
  * closed form, P3 constants, P4 non-negativity, P5 dense-matrix brute force, P6 sum conservation,
  * P7 I-divergence monotone, P8 numpy-FFT cross-check of both convolutions, P9 duplicated view,
- * P10 shift equivariance, P11 zero iterations.  Parity unpinned: nothing in this file.
+ * P10 shift equivariance, P11 zero iterations; explicit back-projectors (mvd_oracle_x): PX1 X = flip(P)
+ * reduces to the Independent variant, PX2 dense-matrix brute force with an asymmetric X of another
+ * size, PX3 centred-delta X closed form.  Parity unpinned: nothing in this file.
  */
 #include <math.h>
 #include <pthread.h>
@@ -141,9 +143,13 @@ void mvd_oracle_backproject(const double* r, const float* P, int K, int W, int H
  * plane is `view_stride` uint16 elements further on.  trace (nullable) receives psi after every
  * view update: [T*V][H][W].
  * ------------------------------------------------------------------------------------------- */
+/* xs (nullable): explicit back-projectors X_v, float [V][KX][KX] ("the implemented
+ * variants all used the following formula, but replaced X"): step a3 becomes the TRUE periodic
+ * convolution q = r * X_v, q(x) = sum_u X_v(u) r(x - u), index (j,i) <-> u = (j-cx, i-cx).
+ * xs == NULL is the "Independent" variant X = P_v^* (correlation with P_v). */
 static void rl_plane(int W, int H, int V, const float* psfs, int K, int T, double eps,
                      const uint16_t* views, size_t view_stride, double* psi, double* trace,
-                     int literal) {
+                     int literal, const float* xs, int KX) {
     const size_t npx = (size_t)W * H;
     double* b = (double*)malloc(sizeof(double) * npx);
     double* r = (double*)malloc(sizeof(double) * npx);
@@ -165,7 +171,11 @@ static void rl_plane(int W, int H, int V, const float* psfs, int K, int T, doubl
                 const double den = b[p] > eps ? b[p] : eps;
                 r[p] = (double)phi[p] / den;
             }
-            if (literal) mvd_oracle_backproject_literal(r, P, K, W, H, q);       /* a3 */
+            if (xs) {                                                            /* a3 with X_v given */
+                const float* X = xs + (size_t)v * KX * KX;
+                if (literal) mvd_oracle_blur_literal(r, X, KX, W, H, q);
+                else         mvd_oracle_blur(r, X, KX, W, H, q);
+            } else if (literal) mvd_oracle_backproject_literal(r, P, K, W, H, q); /* a3, X = P_v^* */
             else         mvd_oracle_backproject(r, P, K, W, H, q);
             for (size_t p = 0; p < npx; ++p) psi[p] = psi[p] * q[p];             /* a4 */
             if (trace) memcpy(trace + ((size_t)t * V + v) * npx, psi, sizeof(double) * npx);
@@ -190,6 +200,8 @@ static int check_args(int W, int H, int V, const float* psfs, int K, int T, doub
 typedef struct {
     int W, H, V, K, T, N, literal;
     double eps;
+    const float* xs;
+    int KX;
     const float* psfs;
     const uint16_t* views;
     double* out;
@@ -201,20 +213,22 @@ static void* worker(void* arg) {
     const size_t npx = (size_t)j->W * j->H;
     for (int p = j->p_begin; p < j->p_end; ++p)
         rl_plane(j->W, j->H, j->V, j->psfs, j->K, j->T, j->eps, j->views + (size_t)p * npx,
-                 (size_t)j->N * npx, j->out + (size_t)p * npx, NULL, j->literal);
+                 (size_t)j->N * npx, j->out + (size_t)p * npx, NULL, j->literal, j->xs, j->KX);
     return NULL;
 }
 
 static int run(int W, int H, int V, const float* psfs, int K, int T, double eps,
-               const uint16_t* views, double* out, int N, int n_threads, int literal) {
+               const uint16_t* views, double* out, int N, int n_threads, int literal,
+               const float* xs, int KX) {
     int rc = check_args(W, H, V, psfs, K, T, eps, views, out, N);
     if (rc) return rc;
+    if (xs && (KX < 1 || (KX % 2) == 0)) return -1;
     if (n_threads < 1) n_threads = 1;
     if (n_threads > N) n_threads = N;           /* parallel over planes only */
     job_t* jobs = (job_t*)calloc((size_t)n_threads, sizeof(job_t));
     pthread_t* th = (pthread_t*)calloc((size_t)n_threads, sizeof(pthread_t));
     for (int k = 0; k < n_threads; ++k) {
-        job_t j = {W, H, V, K, T, N, literal, eps, psfs, views, out,
+        job_t j = {W, H, V, K, T, N, literal, eps, xs, KX, psfs, views, out,
                    (int)((long long)N * k / n_threads), (int)((long long)N * (k + 1) / n_threads)};
         jobs[k] = j;
     }
@@ -227,12 +241,19 @@ static int run(int W, int H, int V, const float* psfs, int K, int T, double eps,
 
 int mvd_oracle(int W, int H, int V, const float* psfs, int K, int T, double eps,
                const uint16_t* views, double* out, int N, int n_threads) {
-    return run(W, H, V, psfs, K, T, eps, views, out, N, n_threads, 0);
+    return run(W, H, V, psfs, K, T, eps, views, out, N, n_threads, 0, NULL, 0);
+}
+
+/* The same iteration with the back-projectors X_v given explicitly: xs float [V][KX][KX], KX odd. */
+int mvd_oracle_x(int W, int H, int V, const float* psfs, int K, const float* xs, int KX, int T,
+                 double eps, const uint16_t* views, double* out, int N, int n_threads, int literal) {
+    if (!xs) return -1;
+    return run(W, H, V, psfs, K, T, eps, views, out, N, n_threads, literal, xs, KX);
 }
 
 int mvd_oracle_literal(int W, int H, int V, const float* psfs, int K, int T, double eps,
                        const uint16_t* views, double* out, int N, int n_threads) {
-    return run(W, H, V, psfs, K, T, eps, views, out, N, n_threads, 1);
+    return run(W, H, V, psfs, K, T, eps, views, out, N, n_threads, 1, NULL, 0);
 }
 
 /* One plane (views [V][H][W]); trace [T*V][H][W] = psi after every view update; out [H][W]. */
@@ -240,6 +261,6 @@ int mvd_oracle_trace(int W, int H, int V, const float* psfs, int K, int T, doubl
                      const uint16_t* views, double* out, double* trace) {
     int rc = check_args(W, H, V, psfs, K, T, eps, views, out, 1);
     if (rc) return rc;
-    rl_plane(W, H, V, psfs, K, T, eps, views, (size_t)W * H, out, trace, 0);
+    rl_plane(W, H, V, psfs, K, T, eps, views, (size_t)W * H, out, trace, 0, NULL, 0);
     return 0;
 }

@@ -65,6 +65,8 @@ def _load() -> ctypes.CDLL:
         fn = getattr(lib, name)
         fn.argtypes = [i, i, i, fp, i, i, d, up, dp, i, i]
         fn.restype = i
+    lib.mvd_oracle_x.argtypes = [i, i, i, fp, i, fp, i, i, d, up, dp, i, i, i]
+    lib.mvd_oracle_x.restype = i
     lib.mvd_oracle_trace.argtypes = [i, i, i, fp, i, i, d, up, dp, dp]
     lib.mvd_oracle_trace.restype = i
     for name in ("mvd_oracle_blur", "mvd_oracle_backproject",
@@ -92,11 +94,14 @@ def n_cores() -> int:
 
 
 def deconvolve(views: np.ndarray, psfs: np.ndarray, T: int, eps: float = 1e-6,
-               n_threads: Optional[int] = None, literal: bool = False) -> np.ndarray:
+               n_threads: Optional[int] = None, literal: bool = False,
+               backprojectors: Optional[np.ndarray] = None) -> np.ndarray:
     """fp64 `[N][H][W]` = T sequential multi-view RL iterations on every plane.
 
     views uint16 `[V][N][H][W]`, psfs float32 `[V][K][K]`.  eps is first rounded to fp32 (the C ABI
     of the product takes `float eps`), so both sides clamp at the identical threshold (reading A6).
+    backprojectors float32 `[V][KX][KX]` (optional): step a3 is the true convolution r * X_v with these
+    kernels instead of the correlation with P_v; None is the Independent variant.
     """
     views = np.ascontiguousarray(views, dtype=np.uint16)
     psfs = _f32(psfs)
@@ -106,6 +111,15 @@ def deconvolve(views: np.ndarray, psfs: np.ndarray, T: int, eps: float = 1e-6,
     assert psfs.shape[2] == K
     out = np.empty((N, H, W), dtype=np.float64)
     nt = n_cores() if n_threads is None else n_threads
+    if backprojectors is not None:
+        xs = _f32(backprojectors)
+        assert xs.ndim == 3 and xs.shape[0] == V and xs.shape[1] == xs.shape[2]
+        rc = _load().mvd_oracle_x(W, H, V, _ptr(psfs, ctypes.c_float), K, _ptr(xs, ctypes.c_float),
+                                  xs.shape[1], int(T), float(np.float32(eps)), _ptr(views, ctypes.c_uint16),
+                                  _ptr(out, ctypes.c_double), N, int(nt), int(bool(literal)))
+        if rc != 0:
+            raise ValueError(f"mvd_oracle_x rejected its arguments (rc={rc})")
+        return out
     fn = _load().mvd_oracle_literal if literal else _load().mvd_oracle
     rc = fn(W, H, V, _ptr(psfs, ctypes.c_float), K, int(T), float(np.float32(eps)),
             _ptr(views, ctypes.c_uint16), _ptr(out, ctypes.c_double), N, int(nt))
@@ -148,3 +162,55 @@ def blur(psi, P, literal=False):
 def backproject(r, P, literal=False):
     """a3: r * P^* (periodic correlation with P)."""
     return _conv("mvd_oracle_backproject_literal" if literal else "mvd_oracle_backproject", r, P)
+
+
+# ---------------------------------------------------------------------------------------------
+# Back-projectors of Supp. Note 2 section 1 (PAPER.md:98-118), written out from the printed formulas.
+# READINGS (the text is garbled and defines none of the operators; DESIGN.md section 2, B1-B4):
+#   B1  "*" is the full (non-periodic) 2D convolution of the small kernels, P^* the flipped PSF;
+#   B2  juxtaposition and the product sign are POINTWISE products of kernels laid over a common
+#       centre (a kernel is zero outside its support), so X_v lives on P_v^*'s K x K support;
+#   B3  W_v is the set of all other views w != v; Optimization I's printed index "v in W_v" is
+#       read as "w in W_v";
+#   B4  X_v is normalised to sum 1 (constant images then stay a fixed point of the update).
+#   Optimization II's printed formula (a product over "v, w in W_v" of P_v^* alone) cannot be
+#   recovered from this text and is not built.
+# Parity of these READINGS is unpinned (no value in the paper fixes them); what is pinned is their
+# arithmetic (tests/test_oracle_pins.py) and, independently, the iteration for ANY given X_v.
+# ---------------------------------------------------------------------------------------------
+def _full_conv(a: np.ndarray, b: np.ndarray) -> np.ndarray:
+    out = np.zeros((a.shape[0] + b.shape[0] - 1, a.shape[1] + b.shape[1] - 1), dtype=np.float64)
+    for j in range(b.shape[0]):
+        for i in range(b.shape[1]):
+            out[j:j + a.shape[0], i:i + a.shape[1]] += b[j, i] * a
+    return out
+
+
+def _centre_crop(a: np.ndarray, K: int) -> np.ndarray:
+    oy, ox = (a.shape[0] - K) // 2, (a.shape[1] - K) // 2
+    return a[oy:oy + K, ox:ox + K]
+
+
+def backprojectors(psfs: np.ndarray, variant: str) -> np.ndarray:
+    """float32 `[V][K][K]` back-projectors X_v for variant in {"independent", "efficient_bayesian",
+    "optimization1"}, fp64 arithmetic, rounded to fp32 at the end."""
+    P = np.asarray(psfs, dtype=np.float64)
+    V, K, _ = P.shape
+    flip = P[:, ::-1, ::-1]
+    if variant == "independent":
+        return np.ascontiguousarray(flip, dtype=np.float32)         # PAPER.md:104, not normalised: X = P_v^*
+    out = np.empty_like(P)
+    for v in range(V):
+        X = flip[v].copy()
+        for w in range(V):
+            if w == v:
+                continue
+            if variant == "efficient_bayesian":                     # PAPER.md:108  P_v^* * P_w * P_w^*
+                f = _full_conv(_full_conv(flip[v], P[w]), flip[w])
+            elif variant == "optimization1":                        # PAPER.md:112  P_v^* * P_w
+                f = _full_conv(flip[v], P[w])
+            else:
+                raise ValueError(f"unknown variant {variant!r}")
+            X = X * _centre_crop(f, K)
+        out[v] = X / X.sum()
+    return np.ascontiguousarray(out, dtype=np.float32)

@@ -288,3 +288,100 @@ def test_threads_do_not_change_results():
     a = orc.deconvolve(prob.views, prob.psfs, prob.T, n_threads=1)
     b = orc.deconvolve(prob.views, prob.psfs, prob.T, n_threads=4)
     assert np.array_equal(a, b)
+
+
+# ---------------------------------------------------------------------------------------------
+# Explicit back-projectors X_v ("replaced X with the expressions given below").
+# Step a3 is the TRUE convolution r * X_v.
+#   PX1  X = flip(P) is the Independent variant
+#   PX2  dense-matrix brute force with an ASYMMETRIC X of a different size than P
+#   PX3  centred-delta X, centred-delta P, one view: psi_1 = psi_0 . phi / psi_0 = phi
+#   PX4  off-centre delta X at d: q(x) = r(x - d), the opposite shift of P2 (a flipped X would give +d)
+# ---------------------------------------------------------------------------------------------
+def test_PX1_flipped_psf_is_the_independent_variant():
+    views = synth.random_views(3, 2, 14, 9, seed=7)
+    psfs = rand_psfs(3, 5, 8)
+    a = orc.deconvolve(views, psfs, 4)
+    b = orc.deconvolve(views, psfs, 4, backprojectors=psfs[:, ::-1, ::-1])
+    np.testing.assert_allclose(b, a, rtol=1e-12)
+    assert np.array_equal(orc.backprojectors(psfs, "independent"), psfs[:, ::-1, ::-1])
+    wrong = orc.deconvolve(views, psfs, 4, backprojectors=psfs)          # unflipped: must differ
+    assert np.abs(wrong - a).max() > 1e-3 * a.max()
+
+
+def dense_rl_x(views_plane, psfs, xs, T, eps):
+    V, H, W = views_plane.shape
+    phi = views_plane.reshape(V, -1).astype(np.float64)
+    psi = phi.sum(0) / V
+    A = [dense_operator(psfs[v], H, W) for v in range(V)]
+    B = [dense_operator(xs[v], H, W) for v in range(V)]                   # convolution with X_v
+    for _ in range(T):
+        for v in range(V):
+            r = phi[v] / np.maximum(A[v] @ psi, eps)
+            psi = psi * (B[v] @ r)
+    return psi.reshape(H, W)
+
+
+@pytest.mark.parametrize("W,H,K,KX", [(8, 8, 3, 5), (12, 8, 5, 3), (8, 12, 5, 7), (6, 5, 3, 9)])
+def test_PX2_dense_matrix_brute_force_with_explicit_backprojectors(W, H, K, KX):
+    V, T = 2, 3
+    views = synth.random_views(V, 2, W, H, seed=70 + K)
+    psfs, xs = rand_psfs(V, K, 80 + W), rand_psfs(V, KX, 90 + H)
+    for literal in (False, True):
+        out = orc.deconvolve(views, psfs, T, backprojectors=xs, literal=literal)
+        for p in range(2):
+            ref = dense_rl_x(views[:, p], psfs, xs, T, float(np.float32(1e-6)))
+            np.testing.assert_allclose(out[p], ref, rtol=1e-11, atol=1e-11)
+
+
+def test_PX3_PX4_delta_backprojectors():
+    views = synth.random_views(1, 2, 12, 10, seed=3, lo=10, hi=4000)
+    phi = views[0].astype(np.float64)
+    d0 = synth.delta_psf(5)[None]
+    out = orc.deconvolve(views, d0, 3, backprojectors=synth.delta_psf(3)[None])
+    np.testing.assert_allclose(out, phi, rtol=1e-13)
+    # P = centred delta, X = delta at (dz, dx): psi_1(x) = phi(x) . 1 ... r = 1 everywhere, q = 1: psi stays phi;
+    # use two views so that r is not constant: psi_0 = mean, r_0 = phi_0 / psi_0, q(x) = r_0(x - d)
+    v2 = synth.random_views(2, 1, 12, 10, seed=4, lo=10, hi=4000)
+    P = np.stack([synth.delta_psf(3)] * 2)
+    dz, dx = 1, -2
+    X = np.stack([synth.delta_psf(5, dz, dx), synth.delta_psf(5)])
+    tr = orc.deconvolve(v2[:, :1], P, 1, backprojectors=X)[0]
+    f = v2[:, 0].astype(np.float64)
+    psi0 = f.mean(0)
+    psi1 = psi0 * np.roll(f[0] / psi0, shift=(dz, dx), axis=(0, 1))       # q(x) = r(x - d)
+    psi2 = psi1 * (f[1] / psi1)
+    np.testing.assert_allclose(tr, psi2, rtol=1e-12)
+
+
+def test_backprojector_builders_arithmetic():
+    """The variant builders of oracle/mvd_oracle.py against scipy's convolution and their invariants
+    (their READING of the garbled formulas is unpinned; this pins the arithmetic only)."""
+    from scipy.signal import convolve2d
+    psfs = rand_psfs(3, 5, 11)
+    P = psfs.astype(np.float64)
+    flip = P[:, ::-1, ::-1]
+    for variant, factor in (("efficient_bayesian", lambda v, w: convolve2d(convolve2d(flip[v], P[w]), flip[w])),
+                            ("optimization1", lambda v, w: convolve2d(flip[v], P[w]))):
+        X = orc.backprojectors(psfs, variant)
+        assert X.shape == psfs.shape and X.dtype == np.float32
+        np.testing.assert_allclose(X.sum(axis=(1, 2)), 1.0, rtol=1e-6)
+        for v in range(3):
+            want = flip[v].copy()
+            for w in range(3):
+                if w != v:
+                    f = factor(v, w)
+                    o = (f.shape[0] - 5) // 2
+                    want *= f[o:o + 5, o:o + 5]
+            np.testing.assert_allclose(X[v], want / want.sum(), rtol=2e-6)
+    # one view: W_v is empty, every variant is the (normalised) flipped PSF
+    one = rand_psfs(1, 7, 12)
+    np.testing.assert_allclose(orc.backprojectors(one, "efficient_bayesian")[0],
+                               one[0, ::-1, ::-1] / one[0].astype(np.float64).sum(), rtol=1e-6)
+    # sum X_v = 1 (and sum P_v = 1): constant views stay a fixed point (P3 carries over; flux
+    # conservation P6 does not -- it needs X_v to be the adjoint of P_v)
+    views = np.full((3, 1, 12, 16), 777, dtype=np.uint16)
+    out = orc.deconvolve(views, psfs, 3, backprojectors=orc.backprojectors(psfs, "optimization1"))
+    np.testing.assert_allclose(out, 777.0, rtol=1e-5)
+    with pytest.raises(ValueError):
+        orc.backprojectors(psfs, "optimization2")
