@@ -81,6 +81,35 @@ MVD_API int mvd_create_path(int plane_w, int plane_h, int n_views, const float* 
                     int iterations, float eps, int path, mvd_handle** out);
 
 /*
+ * Other back-projectors (Supp. Note 2 s.1: "the implemented variants all used the
+ * following formula, but replaced X").  Step a3 becomes the TRUE periodic convolution with X_v,
+ *   q = r (*) X_v,   q(x) = sum_u X_v(u) r(x - u),   index (j, i) <-> u = (j - cx, i - cx), cx = (bp_size - 1) / 2;
+ * X_v = flipped P_v is the Independent variant that mvd_create builds.
+ *   backprojectors  HOST, float [n_views][bp_size][bp_size]; copied; finite (any sign); bp_size odd, may
+ *                   differ from psf_size.  Used as given (not renormalised).
+ *   path            MVD_PATH_AUTO / DIRECT / FFT as in mvd_create_path.
+ * Everything else as mvd_create.  Errors: MVD_ERR_INVALID (NULL, even bp_size, non-finite value), ...
+ */
+MVD_API int mvd_create_backprojectors(int plane_w, int plane_h, int n_views, const float* psfs, int psf_size,
+                              const float* backprojectors, int bp_size, int iterations, float eps,
+                              int path, mvd_handle** out);
+
+/*
+ * mvd_build_backprojectors -- the paper's variants written out on the host (fp64, no device needed):
+ *   MVD_BP_INDEPENDENT         X_v = P_v^*
+ *   MVD_BP_EFFICIENT_BAYESIAN  X_v = P_v^* . prod_{w != v} (P_v^* * P_w * P_w^*)
+ *   MVD_BP_OPTIMIZATION1       X_v = P_v^* . prod_{w != v} (P_v^* * P_w)
+ * under the readings of DESIGN.md section 2 (B1-B4; the printed formulas define no operator): "*" is the
+ * full convolution of the small kernels, "." and the product sign are pointwise products over a common
+ * centre (so X_v lives on P_v^*'s psf_size x psf_size support), W_v is every other view, and the two
+ * compound kernels are normalised to sum 1.  Optimization II is not recoverable from the
+ * text and is not offered.
+ *   psfs  HOST float [n_views][psf_size][psf_size], finite, >= 0;   out  HOST float, same shape.
+ */
+enum { MVD_BP_INDEPENDENT = 0, MVD_BP_EFFICIENT_BAYESIAN = 1, MVD_BP_OPTIMIZATION1 = 2 };
+MVD_API int mvd_build_backprojectors(int variant, int n_views, const float* psfs, int psf_size, float* out);
+
+/*
  * mvd_deconvolve_planes -- steps a0..a5 on n_planes device-resident planes.
  *   dev_views_u16  DEVICE, uint16 [n_views][n_planes][plane_h][plane_w]; read-only.
  *   dev_out_f32    DEVICE, float  [n_planes][plane_h][plane_w]; fully overwritten; must not alias the input.

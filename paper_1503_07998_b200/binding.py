@@ -26,6 +26,8 @@ _fp = ctypes.POINTER(ctypes.c_float)
 SIGNATURES = {
     "mvd_create": (_i, [_i, _i, _i, _fp, _i, _i, _f, ctypes.POINTER(_vp)]),
     "mvd_create_path": (_i, [_i, _i, _i, _fp, _i, _i, _f, _i, ctypes.POINTER(_vp)]),
+    "mvd_create_backprojectors": (_i, [_i, _i, _i, _fp, _i, _fp, _i, _i, _f, _i, ctypes.POINTER(_vp)]),
+    "mvd_build_backprojectors": (_i, [_i, _i, _fp, _i, _fp]),
     "mvd_deconvolve_planes": (_i, [_vp, _vp, _vp, _i, _vp]),
     "mvd_deconvolve_host": (_i, [_vp, _vp, _vp, _i]),
     "mvd_destroy": (None, [_vp]),
@@ -98,7 +100,8 @@ class Mvd:
     """One plan (mvd_create ... mvd_destroy).  Same names and argument order as the C ABI."""
 
     def __init__(self, plane_w: int, plane_h: int, n_views: int, psfs: np.ndarray, psf_size: int,
-                 iterations: int, eps: float = 1e-6, path: Optional[int] = None):
+                 iterations: int, eps: float = 1e-6, path: Optional[int] = None,
+                 backprojectors: Optional[np.ndarray] = None):
         psfs = np.ascontiguousarray(psfs, dtype=np.float32)
         if psfs.size != n_views * psf_size * psf_size:
             raise ValueError("psfs must hold n_views * psf_size * psf_size floats")
@@ -106,7 +109,14 @@ class Mvd:
         self.plane_w, self.plane_h, self.n_views = plane_w, plane_h, n_views
         self.psf_size, self.iterations = psf_size, iterations
         p = psfs.ctypes.data_as(_fp)
-        if path is None:
+        if backprojectors is not None:      # mvd_create_backprojectors: explicit X_v for step a3
+            xs = np.ascontiguousarray(backprojectors, dtype=np.float32)
+            if xs.ndim != 3 or xs.shape[0] != n_views or xs.shape[1] != xs.shape[2]:
+                raise ValueError("backprojectors must be [n_views][bp_size][bp_size]")
+            rc = lib().mvd_create_backprojectors(plane_w, plane_h, n_views, p, psf_size, xs.ctypes.data_as(_fp),
+                                                 xs.shape[1], iterations, eps, PATH_AUTO if path is None else path,
+                                                 ctypes.byref(self._h))
+        elif path is None:
             rc = lib().mvd_create(plane_w, plane_h, n_views, p, psf_size, iterations, eps, ctypes.byref(self._h))
         else:
             rc = lib().mvd_create_path(plane_w, plane_h, n_views, p, psf_size, iterations, eps, path,
@@ -202,9 +212,23 @@ def _stream(s) -> _vp:
     return _vp(s.cuda_stream)
 
 
+BP_INDEPENDENT, BP_EFFICIENT_BAYESIAN, BP_OPTIMIZATION1 = 0, 1, 2
+
+
+def build_backprojectors(variant: int, psfs: np.ndarray) -> np.ndarray:
+    """mvd_build_backprojectors: float32 `[V][K][K]` back-projectors of the paper's variants (host, no device)."""
+    psfs = np.ascontiguousarray(psfs, dtype=np.float32)
+    V, K, _ = psfs.shape
+    out = np.empty_like(psfs)
+    rc = lib().mvd_build_backprojectors(int(variant), V, psfs.ctypes.data_as(_fp), K, out.ctypes.data_as(_fp))
+    if rc != MVD_OK:
+        raise MvdError(rc, "mvd_build_backprojectors")
+    return out
+
+
 def deconvolve(views: np.ndarray, psfs: np.ndarray, iterations: int, eps: float = 1e-6,
                path: Optional[int] = None, host: bool = False, chunk_planes: int = 0,
-               batch_planes: int = 0) -> np.ndarray:
+               batch_planes: int = 0, backprojectors: Optional[np.ndarray] = None) -> np.ndarray:
     """Convenience for tests: numpy uint16 `[V][N][H][W]` in, numpy float32 `[N][H][W]` out, through
     mvd_deconvolve_planes (host=False) or mvd_deconvolve_host (host=True, pinned buffers)."""
     import torch
@@ -213,7 +237,7 @@ def deconvolve(views: np.ndarray, psfs: np.ndarray, iterations: int, eps: float 
     views = np.ascontiguousarray(views, dtype=np.uint16)
     V, N, H, W = views.shape
     K = psfs.shape[-1]
-    with Mvd(W, H, V, psfs, K, iterations, eps, path) as m:
+    with Mvd(W, H, V, psfs, K, iterations, eps, path, backprojectors) as m:
         if chunk_planes:
             m.set_chunk_planes(chunk_planes)
         if batch_planes:

@@ -6,6 +6,7 @@
 
 #include <algorithm>
 #include <new>
+#include <vector>
 
 #include "mvd_internal.cuh"
 
@@ -95,10 +96,17 @@ static int choose_path(int W, int H, int K) {
     return -1;
 }
 
-int mvd_create_path(int plane_w, int plane_h, int n_views, const float* psfs, int psf_size,
-                    int iterations, float eps, int path, mvd_handle** out) {
+static int create_impl(int plane_w, int plane_h, int n_views, const float* psfs, int psf_size,
+                       const float* xs, int bp_size, int iterations, float eps, int path, mvd_handle** out) {
     if (!out) return MVD_ERR_INVALID;
     *out = nullptr;
+    if (xs) {
+        if (bp_size < 1 || (bp_size % 2) == 0 || n_views < 1) return MVD_ERR_INVALID;
+        const size_t nx = (size_t)n_views * bp_size * bp_size;
+        for (size_t k = 0; k < nx; ++k)
+            if (!isfinite(xs[k])) return MVD_ERR_INVALID;
+    }
+    const int k_eff = xs && bp_size > psf_size ? bp_size : psf_size;   // taps the direct engine works with
     if (!psfs || plane_w < 1 || plane_h < 1 || n_views < 1 || n_views > 255 || iterations < 0)
         return MVD_ERR_INVALID;
     if (psf_size < 1 || (psf_size % 2) == 0) return MVD_ERR_INVALID;
@@ -109,9 +117,9 @@ int mvd_create_path(int plane_w, int plane_h, int n_views, const float* psfs, in
         if (!isfinite(psfs[k]) || psfs[k] < 0.f) return MVD_ERR_INVALID;
     if (path != MVD_PATH_AUTO && path != MVD_PATH_DIRECT && path != MVD_PATH_FFT) return MVD_ERR_INVALID;
     if (path == MVD_PATH_AUTO) {
-        path = choose_path(plane_w, plane_h, psf_size);
+        path = choose_path(plane_w, plane_h, k_eff);
         if (path < 0) return MVD_ERR_UNSUPPORTED;
-    } else if (!mvd_path_supported(path, plane_w, plane_h, psf_size)) {
+    } else if (!mvd_path_supported(path, plane_w, plane_h, k_eff)) {
         return MVD_ERR_UNSUPPORTED;
     }
 
@@ -119,15 +127,85 @@ int mvd_create_path(int plane_w, int plane_h, int n_views, const float* psfs, in
     if (!h) return MVD_ERR_NOMEM;
     h->W = plane_w; h->H = plane_h; h->V = n_views; h->K = psf_size; h->T = iterations;
     h->eps = eps; h->path = path;
+    h->KX = xs ? bp_size : 0;
     int rc = mvd_check(h, cudaGetDevice(&h->device));
     if (rc == MVD_OK) rc = mvd_check(h, cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device));
-    if (rc == MVD_OK) rc = path == MVD_PATH_FFT ? fft_setup(h, psfs) : direct_setup(h, psfs);
+    if (rc == MVD_OK) rc = path == MVD_PATH_FFT ? fft_setup(h, psfs, xs) : direct_setup(h, psfs, xs);
     if (rc != MVD_OK) {
         // keep the cuda error visible to the caller through the return code only
         mvd_destroy(h);
         return rc;
     }
     *out = h;
+    return MVD_OK;
+}
+
+int mvd_create_path(int plane_w, int plane_h, int n_views, const float* psfs, int psf_size,
+                    int iterations, float eps, int path, mvd_handle** out) {
+    return create_impl(plane_w, plane_h, n_views, psfs, psf_size, nullptr, 0, iterations, eps, path, out);
+}
+
+int mvd_create_backprojectors(int plane_w, int plane_h, int n_views, const float* psfs, int psf_size,
+                              const float* backprojectors, int bp_size, int iterations, float eps,
+                              int path, mvd_handle** out) {
+    if (!backprojectors) {
+        if (out) *out = nullptr;
+        return MVD_ERR_INVALID;
+    }
+    return create_impl(plane_w, plane_h, n_views, psfs, psf_size, backprojectors, bp_size, iterations, eps, path, out);
+}
+
+// Back-projectors of Supp. Note 2 section 1 under readings B1-B4 of DESIGN.md:
+//   X_v = P_v^* . prod_{w != v} F_vw  (pointwise, on P_v^*'s K x K support), normalised to sum 1, with
+//   F_vw = P_v^* * P_w * P_w^* (Efficient Bayesian) or P_v^* * P_w (Optimization I), "*" the full convolution.
+int mvd_build_backprojectors(int variant, int n_views, const float* psfs, int psf_size, float* out) {
+    if (!psfs || !out || n_views < 1 || psf_size < 1 || (psf_size % 2) == 0) return MVD_ERR_INVALID;
+    if (variant != MVD_BP_INDEPENDENT && variant != MVD_BP_EFFICIENT_BAYESIAN && variant != MVD_BP_OPTIMIZATION1)
+        return MVD_ERR_INVALID;
+    const int K = psf_size, c = (K - 1) / 2, G = 2 * K - 1;
+    const size_t kk = (size_t)K * K;
+    for (size_t k = 0; k < kk * n_views; ++k)
+        if (!isfinite(psfs[k]) || psfs[k] < 0.f) return MVD_ERR_INVALID;
+    auto P = [&](int v, int j, int i) -> double {       // P_v at array index (j, i), 0 outside
+        return (j < 0 || j >= K || i < 0 || i >= K) ? 0.0 : (double)psfs[v * kk + (size_t)j * K + i];
+    };
+    auto Pf = [&](int v, int j, int i) -> double { return P(v, K - 1 - j, K - 1 - i); };   // P_v^*
+    std::vector<double> g((size_t)G * G), x(kk);
+    for (int v = 0; v < n_views; ++v) {
+        for (int j = 0; j < K; ++j)
+            for (int i = 0; i < K; ++i) x[(size_t)j * K + i] = Pf(v, j, i);
+        if (variant != MVD_BP_INDEPENDENT) {
+            for (int w = 0; w < n_views; ++w) {
+                if (w == v) continue;
+                // g = P_v^* * P_w on (2K-1)^2, index (a, b) <-> offset (a - 2c, b - 2c)
+                for (int a = 0; a < G; ++a)
+                    for (int b = 0; b < G; ++b) {
+                        double s = 0.0;
+                        for (int j = 0; j < K; ++j)
+                            for (int i = 0; i < K; ++i) s += Pf(v, j, i) * P(w, a - j, b - i);
+                        g[(size_t)a * G + b] = s;
+                    }
+                for (int j = 0; j < K; ++j)
+                    for (int i = 0; i < K; ++i) {
+                        double f;
+                        if (variant == MVD_BP_OPTIMIZATION1) {
+                            f = g[(size_t)(j + c) * G + (i + c)];          // offset (j - c, i - c)
+                        } else {                                           // (g * P_w^*) at offset (j - c, i - c)
+                            f = 0.0;
+                            for (int a = 0; a < G; ++a)
+                                for (int b = 0; b < G; ++b)
+                                    f += g[(size_t)a * G + b] * Pf(w, j + 2 * c - a, i + 2 * c - b);
+                        }
+                        x[(size_t)j * K + i] *= f;
+                    }
+            }
+            double sum = 0.0;
+            for (size_t k = 0; k < kk; ++k) sum += x[k];
+            if (!(sum > 0.0)) return MVD_ERR_INVALID;
+            for (size_t k = 0; k < kk; ++k) x[k] /= sum;
+        }
+        for (size_t k = 0; k < kk; ++k) out[v * kk + k] = (float)x[k];
+    }
     return MVD_OK;
 }
 
@@ -154,6 +232,7 @@ void mvd_destroy(mvd_handle* h) {
     }
     if (h->d_coef) cudaFree(h->d_coef);
     if (h->d_otf) cudaFree(h->d_otf);
+    if (h->d_otf_b) cudaFree(h->d_otf_b);
     fft_teardown(h);
     (void)cudaGetLastError();
     delete h;

@@ -171,7 +171,30 @@ int direct_choose_chunk(int K, int* JC, int* Kp) {
 }
 
 // Upload both coefficient arrays per view, transposed and zero-padded: G[v][which][i][j], j < Kp.
-int direct_setup(mvd_handle* h, const float* host_psfs) {
+// host_xs (nullable): explicit back-projectors X_v, [V][KX][KX].  Step a3 is then the convolution with
+// X_v, i.e. the correlation this kernel computes with the FLIPPED X_v.  Both kernels are laid, centred,
+// into arrays of Kd = max(K, KX) taps (zero outside their support); h->K becomes Kd for this engine.
+int direct_setup(mvd_handle* h, const float* host_psfs, const float* host_xs) {
+    const int K0 = h->K, KX = host_xs ? h->KX : h->K;
+    const int Kd = K0 > KX ? K0 : KX;
+    std::vector<float> pad_p((size_t)h->V * Kd * Kd, 0.f), pad_b((size_t)h->V * Kd * Kd, 0.f);
+    for (int v = 0; v < h->V; ++v) {
+        const int op = (Kd - K0) / 2, ox = (Kd - KX) / 2;
+        for (int j = 0; j < K0; ++j)
+            for (int i = 0; i < K0; ++i) {
+                const float p = host_psfs[((size_t)v * K0 + j) * K0 + i];
+                pad_p[((size_t)v * Kd + j + op) * Kd + i + op] = p;
+                if (!host_xs) pad_b[((size_t)v * Kd + j + op) * Kd + i + op] = p;   // a3 correlates with P_v
+            }
+        if (host_xs)
+            for (int j = 0; j < KX; ++j)
+                for (int i = 0; i < KX; ++i)   // correlation with flip(X_v) == convolution with X_v
+                    pad_b[((size_t)v * Kd + (Kd - 1 - (j + ox))) * Kd + (Kd - 1 - (i + ox))] =
+                        host_xs[((size_t)v * KX + j) * KX + i];
+    }
+    h->K = Kd;
+    host_psfs = pad_p.data();
+    const float* host_back = pad_b.data();
     direct_choose_chunk(h->K, &h->JC, &h->Kp);
     const int K = h->K, Kp = h->Kp;
     const size_t per = (size_t)K * Kp;
@@ -181,12 +204,13 @@ int direct_setup(mvd_handle* h, const float* host_psfs) {
     std::vector<float> g((size_t)h->V * 2 * per, 0.f);
     for (int v = 0; v < h->V; ++v) {
         const float* P = host_psfs + (size_t)v * K * K;
+        const float* B = host_back + (size_t)v * K * K;
         float* blur = g.data() + ((size_t)v * 2 + 0) * per;
         float* back = g.data() + ((size_t)v * 2 + 1) * per;
         for (int j = 0; j < K; ++j)
             for (int i = 0; i < K; ++i) {
                 blur[(size_t)i * Kp + j] = P[(size_t)(K - 1 - j) * K + (K - 1 - i)];   // a1: flipped
-                back[(size_t)i * Kp + j] = P[(size_t)j * K + i];                       // a3: as given
+                back[(size_t)i * Kp + j] = B[(size_t)j * K + i];                       // a3: as given
             }
     }
     MVD_TRY(h, cudaMalloc((void**)&h->d_coef, g.size() * sizeof(float)));

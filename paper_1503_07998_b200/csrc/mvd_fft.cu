@@ -155,7 +155,7 @@ void fft_teardown(mvd_handle* h) {
     h->fft = nullptr;
 }
 
-int fft_setup(mvd_handle* h, const float* host_psfs) {
+int fft_setup(mvd_handle* h, const float* host_psfs, const float* host_xs) {
     if (!fft_supported(h->W, h->H)) return MVD_ERR_UNSUPPORTED;
     FftState st;
     st.row = find_row_ops(h->W, h->H);
@@ -188,31 +188,38 @@ int fft_setup(mvd_handle* h, const float* host_psfs) {
     }
     h->fft = new FftState(st);
 
-    // optical transfer functions
-    const int K = h->K, W = h->W, H = h->H;
+    // optical transfer functions: O_v = FFT2(P_v) / (W H) for a1 and, when the caller supplied explicit
+    // back-projectors X_v, B_v = FFT2(X_v) / (W H) for a3 (otherwise a3 uses conj O_v)
+    const int W = h->W, H = h->H;
     const size_t npx = (size_t)W * H;
-    float* d_psf = nullptr;
-    double2* d_G = nullptr;
-    MVD_TRY(h, cudaMalloc((void**)&h->d_otf, sizeof(float2) * npx * h->V));
-    MVD_TRY(h, cudaMalloc((void**)&d_psf, sizeof(float) * (size_t)h->V * K * K));
-    rc = mvd_check(h, cudaMalloc((void**)&d_G, sizeof(double2) * (size_t)K * W));
-    if (rc == MVD_OK)
-        rc = mvd_check(h, cudaMemcpy(d_psf, host_psfs, sizeof(float) * (size_t)h->V * K * K, cudaMemcpyHostToDevice));
-    for (int v = 0; v < h->V && rc == MVD_OK; ++v) {
-        const dim3 block(128), g1((W + 127) / 128, K), g2((W + 127) / 128, H);
-        {
-            LaunchScope ls(h, KC_SETUP, 0);
-            otf_rows_kernel<<<g1, block>>>(d_psf + (size_t)v * K * K, K, W, d_G);
+    const bool tile_major = st.row->generation == 2;
+    auto build_otfs = [&](const float* host_k, int K, float2** dst) -> int {
+        float* d_k = nullptr;
+        double2* d_G = nullptr;
+        MVD_TRY(h, cudaMalloc((void**)dst, sizeof(float2) * npx * h->V));
+        MVD_TRY(h, cudaMalloc((void**)&d_k, sizeof(float) * (size_t)h->V * K * K));
+        int r = mvd_check(h, cudaMalloc((void**)&d_G, sizeof(double2) * (size_t)K * W));
+        if (r == MVD_OK)
+            r = mvd_check(h, cudaMemcpy(d_k, host_k, sizeof(float) * (size_t)h->V * K * K, cudaMemcpyHostToDevice));
+        for (int v = 0; v < h->V && r == MVD_OK; ++v) {
+            const dim3 block(128), g1((W + 127) / 128, K), g2((W + 127) / 128, H);
+            {
+                LaunchScope ls(h, KC_SETUP, 0);
+                otf_rows_kernel<<<g1, block>>>(d_k + (size_t)v * K * K, K, W, d_G);
+            }
+            {
+                LaunchScope ls(h, KC_SETUP, 0);
+                otf_cols_kernel<<<g2, block>>>(d_G, K, W, H, *dst + (size_t)v * npx, tile_major);
+            }
+            r = mvd_check(h, cudaGetLastError());
         }
-        {
-            LaunchScope ls(h, KC_SETUP, 0);
-            otf_cols_kernel<<<g2, block>>>(d_G, K, W, H, h->d_otf + (size_t)v * npx, st.row->generation == 2);
-        }
-        rc = mvd_check(h, cudaGetLastError());
-    }
-    if (rc == MVD_OK) rc = mvd_check(h, cudaDeviceSynchronize());
-    if (d_psf) cudaFree(d_psf);
-    if (d_G) cudaFree(d_G);
+        if (r == MVD_OK) r = mvd_check(h, cudaDeviceSynchronize());
+        if (d_k) cudaFree(d_k);
+        if (d_G) cudaFree(d_G);
+        return r;
+    };
+    rc = build_otfs(host_psfs, h->K, &h->d_otf);
+    if (rc == MVD_OK && host_xs) rc = build_otfs(host_xs, h->KX, &h->d_otf_b);
     h->launches = 0;
     return rc;
 }
@@ -299,7 +306,9 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_str
             if (rc != MVD_OK) return rc;
             {
                 LaunchScope ls(h, KC_FFT_COLS, stream);
-                rc = mvd_check(h, st->col->cols(tmap, a.S, otf, 1, pairs, W, st->tw_col, col_grid, stream));   // a3
+                rc = h->d_otf_b      // a3: explicit back-projector B_v, or conj O_v (X = P_v^*)
+                         ? mvd_check(h, st->col->cols(tmap, a.S, h->d_otf_b + (size_t)v * npx, 0, pairs, W, st->tw_col, col_grid, stream))
+                         : mvd_check(h, st->col->cols(tmap, a.S, otf, 1, pairs, W, st->tw_col, col_grid, stream));
             }
             if (rc != MVD_OK) return rc;
             {

@@ -48,6 +48,8 @@ struct mvd_handle {
 
     // fft path: optical transfer functions, float2 [V][H][W], pre-scaled by 1/(W*H)
     float2* d_otf = nullptr;
+    float2* d_otf_b = nullptr;   // explicit back-projectors' transfer functions (nullptr: a3 uses conj d_otf)
+    int KX = 0;                  // size of the caller's back-projectors (0: Independent variant, X = P_v^*)
     void* fft = nullptr;   // FftState (mvd_fft.cu)
 
     Workspace ws_main;
@@ -90,7 +92,7 @@ int ws_reserve(mvd_handle* h, Workspace& ws, size_t a_bytes, size_t b_bytes);
 
 // ---- direct path (mvd_direct.cu) ------------------------------------------------------------
 int direct_choose_chunk(int K, int* JC, int* Kp);
-int direct_setup(mvd_handle* h, const float* host_psfs);
+int direct_setup(mvd_handle* h, const float* host_psfs, const float* host_xs);
 size_t direct_scratch_bytes(const mvd_handle* h, int n_planes);
 // views: view v of plane p at views + (v * view_stride + p * H * W); out: [n][H][W]
 int direct_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_stride, float* out,
@@ -98,7 +100,7 @@ int direct_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_
 
 // ---- fft path (mvd_fft.cu) --------------------------------------------------------------------
 int fft_supported(int W, int H);
-int fft_setup(mvd_handle* h, const float* host_psfs);
+int fft_setup(mvd_handle* h, const float* host_psfs, const float* host_xs);
 int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_stride, float* out,
             int n_planes, cudaStream_t stream);
 int fft_default_chunk(const mvd_handle* h);
