@@ -132,6 +132,26 @@ MVD_API int mvd_deconvolve_planes(mvd_handle* h, const uint16_t* dev_views_u16, 
 MVD_API int mvd_deconvolve_host(mvd_handle* h, const uint16_t* host_views_u16, float* host_out_f32,
                         int n_planes);
 
+/*
+ * Reslicing folded into the first read (Fig. 1a: the acquired stacks
+ * are resliced into planes orthogonal to the rotation axis).  Plane p, image row y, pixel x of view v is
+ * read at  dev_views_u16[v * view_stride + p * plane_stride + y * row_stride + x]  (strides in uint16
+ * elements, each a multiple of 8 for the FFT engine; row_stride >= plane_w).  The default layout of
+ * mvd_deconvolve_planes is {n_planes * H * W, H * W, W}; a view acquired as a z-stack of camera frames,
+ * uint16 [plane_h (z)][n_planes (camera lines)][plane_w], is {H * N * W, W, N * W}.  Output as above.
+ */
+MVD_API int mvd_deconvolve_planes_strided(mvd_handle* h, const uint16_t* dev_views_u16, size_t view_stride,
+                                  size_t plane_stride, size_t row_stride, float* dev_out_f32,
+                                  int n_planes, void* stream);
+
+/*
+ * mvd_deconvolve_host with the input in camera order: host_frames_u16 is HOST (pinned) uint16
+ * [n_views][plane_h][n_planes][plane_w]; batches are gathered by one 2D copy per view and read in place.
+ * Same output, bit-identical to mvd_deconvolve_host on the resliced stack.
+ */
+MVD_API int mvd_deconvolve_host_camera(mvd_handle* h, const uint16_t* host_frames_u16, float* host_out_f32,
+                               int n_planes);
+
 /* Frees the plan, its scratch, its streams and staging buffers.  NULL is a no-op. */
 MVD_API void mvd_destroy(mvd_handle* h);
 

@@ -30,6 +30,8 @@ SIGNATURES = {
     "mvd_build_backprojectors": (_i, [_i, _i, _fp, _i, _fp]),
     "mvd_deconvolve_planes": (_i, [_vp, _vp, _vp, _i, _vp]),
     "mvd_deconvolve_host": (_i, [_vp, _vp, _vp, _i]),
+    "mvd_deconvolve_planes_strided": (_i, [_vp, _vp, ctypes.c_size_t, ctypes.c_size_t, ctypes.c_size_t, _vp, _i, _vp]),
+    "mvd_deconvolve_host_camera": (_i, [_vp, _vp, _vp, _i]),
     "mvd_destroy": (None, [_vp]),
     "mvd_strerror": (ctypes.c_char_p, [_i]),
     "mvd_last_cuda_error": (_i, [_vp]),
@@ -132,6 +134,18 @@ class Mvd:
         rc = lib().mvd_deconvolve_planes(self._h, _ptr(dev_views_u16), _ptr(dev_out_f32), n_planes,
                                          _stream(stream))
         self._raise(rc, "mvd_deconvolve_planes")
+
+    def deconvolve_planes_strided(self, dev_views_u16, view_stride: int, plane_stride: int, row_stride: int,
+                                  dev_out_f32, n_planes: int, stream=None) -> None:
+        rc = lib().mvd_deconvolve_planes_strided(self._h, _ptr(dev_views_u16), view_stride, plane_stride,
+                                                 row_stride, _ptr(dev_out_f32), n_planes, _stream(stream))
+        if rc != MVD_OK:
+            self._raise(rc, "mvd_deconvolve_planes_strided")
+
+    def deconvolve_host_camera(self, host_frames_u16, host_out_f32, n_planes: int) -> None:
+        rc = lib().mvd_deconvolve_host_camera(self._h, _ptr(host_frames_u16), _ptr(host_out_f32), n_planes)
+        if rc != MVD_OK:
+            self._raise(rc, "mvd_deconvolve_host_camera")
 
     def deconvolve_host(self, host_views_u16, host_out_f32, n_planes: int) -> None:
         """host buffers: pinned torch tensors, numpy arrays or raw host pointers.  Blocks."""

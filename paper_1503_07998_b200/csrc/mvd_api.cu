@@ -255,15 +255,15 @@ static int default_chunk(const mvd_handle* h) {
 }
 
 // All T iterations on planes [0, n) of `views`, in chunks (each chunk runs to completion).
-static int run_core(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_stride,
+static int run_core(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay,
                     float* out, int n_planes, cudaStream_t stream) {
     const size_t npx = (size_t)h->W * h->H;
     const int chunk = default_chunk(h);
     for (int p0 = 0; p0 < n_planes; p0 += chunk) {
         const int n = std::min(chunk, n_planes - p0);
         int rc = h->path == MVD_PATH_FFT
-                     ? fft_run(h, ws, views + (size_t)p0 * npx, view_stride, out + (size_t)p0 * npx, n, stream)
-                     : direct_run(h, ws, views + (size_t)p0 * npx, view_stride, out + (size_t)p0 * npx, n, stream);
+                     ? fft_run(h, ws, views + (size_t)p0 * lay.plane, lay, out + (size_t)p0 * npx, n, stream)
+                     : direct_run(h, ws, views + (size_t)p0 * lay.plane, lay, out + (size_t)p0 * npx, n, stream);
         if (rc != MVD_OK) return rc;
     }
     return MVD_OK;
@@ -275,8 +275,19 @@ int mvd_deconvolve_planes(mvd_handle* h, const uint16_t* dev_views_u16, float* d
     if (n_planes == 0) return MVD_OK;
     if (!dev_views_u16 || !dev_out_f32) return MVD_ERR_INVALID;
     const size_t npx = (size_t)h->W * h->H;
-    return run_core(h, h->ws_main, dev_views_u16, (size_t)n_planes * npx, dev_out_f32, n_planes,
-                    (cudaStream_t)stream);
+    return run_core(h, h->ws_main, dev_views_u16, ViewLayout{(size_t)n_planes * npx, npx, (size_t)h->W},
+                    dev_out_f32, n_planes, (cudaStream_t)stream);
+}
+
+int mvd_deconvolve_planes_strided(mvd_handle* h, const uint16_t* dev_views_u16, size_t view_stride,
+                                  size_t plane_stride, size_t row_stride, float* dev_out_f32,
+                                  int n_planes, void* stream) {
+    if (!h || n_planes < 0) return MVD_ERR_INVALID;
+    if (n_planes == 0) return MVD_OK;
+    if (!dev_views_u16 || !dev_out_f32) return MVD_ERR_INVALID;
+    if (row_stride < (size_t)h->W || plane_stride < 1 || (h->V > 1 && view_stride < 1)) return MVD_ERR_INVALID;
+    return run_core(h, h->ws_main, dev_views_u16, ViewLayout{view_stride, plane_stride, row_stride},
+                    dev_out_f32, n_planes, (cudaStream_t)stream);
 }
 
 static int default_batch(const mvd_handle* h, int n_planes) {
@@ -291,8 +302,11 @@ static int default_batch(const mvd_handle* h, int n_planes) {
     return h->path == MVD_PATH_FFT ? even_up((int)b) : (int)b;
 }
 
-int mvd_deconvolve_host(mvd_handle* h, const uint16_t* host_views_u16, float* host_out_f32,
-                        int n_planes) {
+// camera_order: the host stack is [V][H][n_planes][W] (z-stacks of camera frames; plane p = camera line p
+// of every frame).  A batch of B planes is then H row-blocks of B*W contiguous uint16 per view: one
+// cudaMemcpy2DAsync, landing as [V][H][B][W]; the kernels read it in place with ViewLayout{H B W, W, B W}.
+static int host_pipeline(mvd_handle* h, const uint16_t* host_views_u16, float* host_out_f32,
+                         int n_planes, bool camera_order) {
     if (!h || n_planes < 0) return MVD_ERR_INVALID;
     if (n_planes == 0) return MVD_OK;
     if (!host_views_u16 || !host_out_f32) return MVD_ERR_INVALID;
@@ -324,11 +338,23 @@ int mvd_deconvolve_host(mvd_handle* h, const uint16_t* host_views_u16, float* ho
         const int s = k % mvd_handle::kSlots;
         const int n = std::min(B, n_planes - p0);
         cudaStream_t st = h->streams[s];
-        for (int v = 0; v < h->V && rc == MVD_OK; ++v)
-            rc = mvd_check(h, cudaMemcpyAsync(h->d_in[s] + (size_t)v * B * npx,
-                                             host_views_u16 + ((size_t)v * n_planes + p0) * npx,
-                                             sizeof(uint16_t) * npx * n, cudaMemcpyHostToDevice, st));
-        if (rc == MVD_OK) rc = run_core(h, h->ws_slot[s], h->d_in[s], (size_t)B * npx, h->d_out[s], n, st);
+        ViewLayout lay;
+        if (camera_order) {
+            lay = ViewLayout{(size_t)h->H * B * h->W, (size_t)h->W, (size_t)B * h->W};
+            for (int v = 0; v < h->V && rc == MVD_OK; ++v)
+                rc = mvd_check(h, cudaMemcpy2DAsync(h->d_in[s] + (size_t)v * lay.view, sizeof(uint16_t) * B * h->W,
+                                                   host_views_u16 + ((size_t)v * h->H * n_planes + p0) * h->W,
+                                                   sizeof(uint16_t) * (size_t)n_planes * h->W,
+                                                   sizeof(uint16_t) * (size_t)n * h->W, (size_t)h->H,
+                                                   cudaMemcpyHostToDevice, st));
+        } else {
+            lay = ViewLayout{(size_t)B * npx, npx, (size_t)h->W};
+            for (int v = 0; v < h->V && rc == MVD_OK; ++v)
+                rc = mvd_check(h, cudaMemcpyAsync(h->d_in[s] + (size_t)v * B * npx,
+                                                 host_views_u16 + ((size_t)v * n_planes + p0) * npx,
+                                                 sizeof(uint16_t) * npx * n, cudaMemcpyHostToDevice, st));
+        }
+        if (rc == MVD_OK) rc = run_core(h, h->ws_slot[s], h->d_in[s], lay, h->d_out[s], n, st);
         if (rc == MVD_OK)
             rc = mvd_check(h, cudaMemcpyAsync(host_out_f32 + (size_t)p0 * npx, h->d_out[s],
                                              sizeof(float) * npx * n, cudaMemcpyDeviceToHost, st));
@@ -338,6 +364,16 @@ int mvd_deconvolve_host(mvd_handle* h, const uint16_t* host_views_u16, float* ho
         if (rc == MVD_OK) rc = rs;
     }
     return rc;
+}
+
+int mvd_deconvolve_host(mvd_handle* h, const uint16_t* host_views_u16, float* host_out_f32,
+                        int n_planes) {
+    return host_pipeline(h, host_views_u16, host_out_f32, n_planes, false);
+}
+
+int mvd_deconvolve_host_camera(mvd_handle* h, const uint16_t* host_frames_u16, float* host_out_f32,
+                               int n_planes) {
+    return host_pipeline(h, host_frames_u16, host_out_f32, n_planes, true);
 }
 
 // ---------------------------------------------------------------------------------------------

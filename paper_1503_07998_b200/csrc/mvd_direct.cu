@@ -26,13 +26,16 @@ __device__ __forceinline__ int pmod(int a, int m) {
 }
 
 // a0: psi_0 = mean of the views (exact sum in fp32: <= 2^16 * V < 2^24 for V <= 255)
-__global__ void init_mean_kernel(const uint16_t* __restrict__ views, size_t view_stride, int V,
+__global__ void init_mean_kernel(const uint16_t* __restrict__ views, ViewLayout lay, int V, int W, int H,
                                  float* __restrict__ psi, size_t n) {
     const float inv_is_exact_division = (float)V;
+    const size_t npx = (size_t)W * H;
     for (size_t p = blockIdx.x * (size_t)blockDim.x + threadIdx.x; p < n;
          p += (size_t)gridDim.x * blockDim.x) {
+        const size_t plane = p / npx, rem = p % npx;
+        const size_t q = plane * lay.plane + (rem / W) * lay.row + rem % W;
         float s = 0.f;
-        for (int v = 0; v < V; ++v) s += (float)views[(size_t)v * view_stride + p];
+        for (int v = 0; v < V; ++v) s += (float)views[(size_t)v * lay.view + q];
         psi[p] = s / inv_is_exact_division;
     }
 }
@@ -43,7 +46,7 @@ template <int KT, int JC, int MODE>
 __global__ void __launch_bounds__(BX* BY)
 direct_corr_kernel(const float* __restrict__ src, const float* __restrict__ G,
                    const uint16_t* __restrict__ phi, float* __restrict__ dst, int W, int H, int Krt,
-                   int Kp, float eps, int tiles_x, int tiles_y) {
+                   int Kp, float eps, int tiles_x, int tiles_y, size_t phi_plane, size_t phi_row) {
     extern __shared__ float smem[];
     const int K = KT > 0 ? KT : Krt;
     const int c = (K - 1) / 2;
@@ -106,7 +109,7 @@ direct_corr_kernel(const float* __restrict__ src, const float* __restrict__ G,
             const int y = y0 + threadIdx.y * RY + m;
             if (y < H) {
                 const size_t p = plane_off + (size_t)y * W + x;
-                if (MODE == 0) dst[p] = (float)phi[p] / fmaxf(acc[m], eps);   // a2
+                if (MODE == 0) dst[p] = (float)phi[(size_t)t * phi_plane + (size_t)y * phi_row + x] / fmaxf(acc[m], eps);   // a2
                 else           dst[p] = dst[p] * acc[m];                      // a4
             }
         }
@@ -115,7 +118,8 @@ direct_corr_kernel(const float* __restrict__ src, const float* __restrict__ G,
 
 template <int KT, int JC>
 int launch_pair_member(int mode, const float* src, const float* G, const uint16_t* phi, float* dst,
-                       int W, int H, int K, int Kp, float eps, int n_planes, cudaStream_t st) {
+                       int W, int H, int K, int Kp, float eps, int n_planes, cudaStream_t st,
+                       size_t phi_plane, size_t phi_row) {
     const int tiles_x = (W + BX - 1) / BX, tiles_y = (H + TILE_H - 1) / TILE_H;
     const size_t smem = sizeof(float) * ((size_t)K * Kp + (size_t)(TILE_H + Kp - 1) * (K + BX - 1));
     const long long grid = (long long)n_planes * tiles_x * tiles_y;
@@ -126,22 +130,22 @@ int launch_pair_member(int mode, const float* src, const float* G, const uint16_
         auto k = direct_corr_kernel<KT, JC, 0>;
         e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return (int)e;
-        k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y);
+        k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row);
     } else {
         auto k = direct_corr_kernel<KT, JC, 1>;
         e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return (int)e;
-        k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y);
+        k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row);
     }
     return (int)cudaGetLastError();
 }
 
 int launch_corr(int mode, const mvd_handle* h, const float* src, const float* G, const uint16_t* phi,
-                float* dst, int n_planes, cudaStream_t st) {
+                float* dst, int n_planes, cudaStream_t st, size_t phi_plane, size_t phi_row) {
 #define MVD_DIRECT_CASE(KT_, JC_)                                                                 \
     if (h->K == (KT_) && h->JC == (JC_))                                                          \
         return launch_pair_member<KT_, JC_>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp,       \
-                                            h->eps, n_planes, st);
+                                            h->eps, n_planes, st, phi_plane, phi_row);
     MVD_DIRECT_CASE(9, 9)
     MVD_DIRECT_CASE(21, 21)
     MVD_DIRECT_CASE(31, 16)
@@ -149,7 +153,7 @@ int launch_corr(int mode, const mvd_handle* h, const float* src, const float* G,
     MVD_DIRECT_CASE(51, 17)
 #undef MVD_DIRECT_CASE
     return launch_pair_member<0, 8>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp, h->eps,
-                                    n_planes, st);
+                                    n_planes, st, phi_plane, phi_row);
 }
 
 }  // namespace
@@ -222,7 +226,7 @@ size_t direct_scratch_bytes(const mvd_handle* h, int n_planes) {
     return sizeof(float) * (size_t)n_planes * h->W * h->H;
 }
 
-int direct_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_stride, float* out,
+int direct_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay, float* out,
                int n_planes, cudaStream_t stream) {
     const size_t npx = (size_t)h->W * h->H;
     const size_t n = npx * n_planes;
@@ -231,7 +235,7 @@ int direct_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_
         const int threads = 256;
         const size_t want = (n + threads - 1) / threads;
         const unsigned grid = (unsigned)(want < (size_t)h->n_sm * 16 ? want : (size_t)h->n_sm * 16);
-        init_mean_kernel<<<grid, threads, 0, stream>>>(views, view_stride, h->V, out, n);
+        init_mean_kernel<<<grid, threads, 0, stream>>>(views, lay, h->V, h->W, h->H, out, n);
     }
     MVD_TRY(h, cudaGetLastError());
     if (h->T == 0) return MVD_OK;
@@ -243,16 +247,16 @@ int direct_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_
         for (int v = 0; v < h->V; ++v) {
             const float* Gblur = h->d_coef + ((size_t)v * 2 + 0) * per;
             const float* Gback = h->d_coef + ((size_t)v * 2 + 1) * per;
-            const uint16_t* phi = views + (size_t)v * view_stride;
+            const uint16_t* phi = views + (size_t)v * lay.view;
             int e;
             {
                 LaunchScope ls(h, KC_DIRECT_BLUR_RATIO, stream);
-                e = launch_corr(0, h, out, Gblur, phi, r, n_planes, stream);
+                e = launch_corr(0, h, out, Gblur, phi, r, n_planes, stream, lay.plane, lay.row);
             }
             MVD_TRY(h, (cudaError_t)e);
             {
                 LaunchScope ls(h, KC_DIRECT_BACK_UPDATE, stream);
-                e = launch_corr(1, h, r, Gback, nullptr, out, n_planes, stream);
+                e = launch_corr(1, h, r, Gback, nullptr, out, n_planes, stream, 0, 0);
             }
             MVD_TRY(h, (cudaError_t)e);
         }

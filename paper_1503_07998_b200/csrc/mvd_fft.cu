@@ -232,7 +232,7 @@ int fft_default_chunk(const mvd_handle* h) {
     return (int)(c & ~(size_t)1);
 }
 
-int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_stride, float* out,
+int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay, float* out,
             int n_planes, cudaStream_t stream) {
     FftState* st = state_of(h);
     if (!st) return MVD_ERR_INVALID;
@@ -240,7 +240,9 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_str
     const int pairs = (n_planes + 1) / 2;
     const size_t bytes = sizeof(float2) * (size_t)pairs * H * W;
     // the bulk copies of the row kernels need 16-byte aligned rows
-    if (((uintptr_t)views & 15u) != 0 || ((view_stride * sizeof(uint16_t)) & 15u) != 0) return MVD_ERR_INVALID;
+    if (((uintptr_t)views & 15u) != 0 || ((lay.view * sizeof(uint16_t)) & 15u) != 0 ||
+        ((lay.plane * sizeof(uint16_t)) & 15u) != 0 || ((lay.row * sizeof(uint16_t)) & 15u) != 0)
+        return MVD_ERR_INVALID;
     int rc = ws_reserve(h, ws, bytes, bytes);
     if (rc != MVD_OK) return rc;
     CUtensorMap tmap;
@@ -254,7 +256,9 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_str
     a.Z = (float2*)ws.a;
     a.S = (float2*)ws.b;
     a.views = views;
-    a.view_stride = view_stride;
+    a.view_stride = lay.view;
+    a.view_plane = lay.plane;
+    a.view_row = lay.row;
     a.out = out;
     a.n_planes = n_planes;
     a.H = H;

@@ -465,6 +465,7 @@ struct RowArgs {
     float2* Z;               // [pairs][H][W] psi pairs
     const uint16_t* views;   // view 0 of plane 0 of this chunk
     size_t view_stride;      // elements between views
+    size_t view_plane, view_row;   // elements between planes / image rows of a view (ViewLayout)
     float* out;              // [n_planes][H][W]; written when `final`
     int n_planes, H, V, v;   // v: the view of this update (ROWS_RATIO)
     float eps;
@@ -493,7 +494,8 @@ __global__ void __launch_bounds__(NT) fft_rows_kernel(RowArgs a, const float2* _
         const int pa = 2 * pair, pb = 2 * pair + 1;
         const bool has_b = pb < a.n_planes;
         const size_t rowoff = (size_t)row * W;          // into S / Z
-        const size_t pxa = (size_t)pa * npx + (size_t)y * W, pxb = pxa + npx;   // into views / out
+        const size_t pxa = (size_t)pa * npx + (size_t)y * W, pxb = pxa + npx;   // into out
+        const size_t vxa = (size_t)pa * a.view_plane + (size_t)y * a.view_row, vxb = vxa + a.view_plane;   // into views
         float2 x[E];
 
         if (MODE == ROWS_FIRST) {
@@ -504,8 +506,8 @@ __global__ void __launch_bounds__(NT) fft_rows_kernel(RowArgs a, const float2* _
                 if (valid)
                     for (int v = 0; v < a.V; ++v) {
                         const uint16_t* vp = a.views + (size_t)v * a.view_stride;
-                        sa += (float)__ldg(vp + pxa + pos);
-                        if (has_b) sb += (float)__ldg(vp + pxb + pos);
+                        sa += (float)__ldg(vp + vxa + pos);
+                        if (has_b) sb += (float)__ldg(vp + vxb + pos);
                     }
                 x[e] = make_float2(sa / (float)a.V, sb / (float)a.V);       // a0
                 if (valid) {
@@ -527,8 +529,8 @@ __global__ void __launch_bounds__(NT) fft_rows_kernel(RowArgs a, const float2* _
                     const int pos = t + TPF * e;
                     uint32_t lo = 0, hi = 0;
                     if (valid) {
-                        lo = __ldg(vp + pxa + pos);
-                        if (has_b) hi = __ldg(vp + pxb + pos);
+                        lo = __ldg(vp + vxa + pos);
+                        if (has_b) hi = __ldg(vp + vxb + pos);
                     }
                     ph[e] = lo | (hi << 16);
                 }
@@ -618,7 +620,7 @@ __global__ void __launch_bounds__(NT) fft_rows_tma_kernel(RowArgs a, const float
         if (row >= a.total_rows) { mbar_arrive(&bar[s]); return; }
         const int pair = row / a.H, y = row % a.H;
         const bool has_b = 2 * pair + 1 < a.n_planes;
-        const size_t pxa = (size_t)(2 * pair) * npx + (size_t)y * W;
+        const size_t vxa = (size_t)(2 * pair) * a.view_plane + (size_t)y * a.view_row;
         unsigned char* st = smem_rows_tma + L::kStage + (size_t)s * L::kStageBytes + sizeof(float2) * W * r;
         unsigned char* ax = smem_rows_tma + L::kAux + (size_t)s * L::kAuxBytes + L::kAuxRow * r;
         const uint32_t row_bytes = sizeof(float2) * W;
@@ -626,8 +628,8 @@ __global__ void __launch_bounds__(NT) fft_rows_tma_kernel(RowArgs a, const float
             const uint32_t pb = sizeof(uint16_t) * W;
             mbar_arrive_expect_tx(&bar[s], row_bytes + (has_b ? 2 * pb : pb));
             bulk_g2s(st, a.S + (size_t)row * W, row_bytes, &bar[s]);
-            bulk_g2s(ax, vp + pxa, pb, &bar[s]);
-            if (has_b) bulk_g2s(ax + pb, vp + pxa + npx, pb, &bar[s]);
+            bulk_g2s(ax, vp + vxa, pb, &bar[s]);
+            if (has_b) bulk_g2s(ax + pb, vp + vxa + a.view_plane, pb, &bar[s]);
         } else {
             mbar_arrive_expect_tx(&bar[s], 2 * row_bytes);
             bulk_g2s(st, a.S + (size_t)row * W, row_bytes, &bar[s]);

@@ -116,8 +116,10 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
         const int pair = row / a.H, y = row % a.H;
         const bool has_b = 2 * pair + 1 < a.n_planes;
         const size_t rowoff = (size_t)row * W;                                      // into Z
-        const size_t pxa = (size_t)(2 * pair) * npx + (size_t)y * W;                // into views / out
+        const size_t pxa = (size_t)(2 * pair) * npx + (size_t)y * W;                // into out
         const size_t pxb = has_b ? pxa + npx : pxa;                                 // odd tail: plane a again, discarded
+        const size_t vxa = (size_t)(2 * pair) * a.view_plane + (size_t)y * a.view_row;   // into views
+        const size_t vxb = has_b ? vxa + a.view_plane : vxa;
         const bool st_a = valid, st_b = valid && has_b;
         float2* Srow = a.S + (size_t)pair * npx + (size_t)(t >> 4) * (a.H * 16) + (size_t)y * 16 + (t & 15);
         const size_t Sstep = (size_t)TPF * a.H;       // x advances by TPF: TPF / 16 tiles of H * 16 elements
@@ -130,8 +132,8 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
 #pragma unroll
             for (int e = 0; e < E; ++e) x[e] = make_float2(0.f, 0.f);
             for (int v = 0; v < a.V; ++v) {
-                const uint16_t* qa = a.views + (size_t)v * a.view_stride + pxa + t;
-                const uint16_t* qb = a.views + (size_t)v * a.view_stride + pxb + t;
+                const uint16_t* qa = a.views + (size_t)v * a.view_stride + vxa + t;
+                const uint16_t* qb = a.views + (size_t)v * a.view_stride + vxb + t;
 #pragma unroll
                 for (int e = 0; e < E; ++e) {
                     x[e].x += (float)__ldg(qa + TPF * e);
@@ -169,7 +171,7 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
                     const int q = t + TPF * k;                   // chunk of 8 uint16; W / 8 chunks per plane
                     const bool second = q >= W / 8;
                     const int qq = second ? q - W / 8 : q;
-                    cp_async16(lu + 8 * q, vp + (second ? pxb : pxa) + 8 * qq);
+                    cp_async16(lu + 8 * q, vp + (second ? vxb : vxa) + 8 * qq);
                 }
             } else {
 #pragma unroll

@@ -80,6 +80,14 @@ struct LaunchScope {
     ~LaunchScope();
 };
 
+// Where plane p, image row y of view v starts in a uint16 view buffer (elements): v * view + p * plane + y * row.
+// The ABI's default is view-major stacks of resliced planes {N H W, H W, W}; camera order (z-stacks of
+// camera frames, Fig. 1a: planes orthogonal to the rotation axis are x-z planes, so plane
+// p is camera line p of every frame) is {H N W, W, N W} -- reslicing is folded into the first read.
+struct ViewLayout {
+    size_t view, plane, row;
+};
+
 // Returns MVD_OK or records the CUDA error in h and returns MVD_ERR_CUDA / MVD_ERR_NOMEM.
 int mvd_check(mvd_handle* h, cudaError_t e);
 #define MVD_TRY(h, expr)                        \
@@ -95,13 +103,13 @@ int direct_choose_chunk(int K, int* JC, int* Kp);
 int direct_setup(mvd_handle* h, const float* host_psfs, const float* host_xs);
 size_t direct_scratch_bytes(const mvd_handle* h, int n_planes);
 // views: view v of plane p at views + (v * view_stride + p * H * W); out: [n][H][W]
-int direct_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_stride, float* out,
+int direct_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay, float* out,
                int n_planes, cudaStream_t stream);
 
 // ---- fft path (mvd_fft.cu) --------------------------------------------------------------------
 int fft_supported(int W, int H);
 int fft_setup(mvd_handle* h, const float* host_psfs, const float* host_xs);
-int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, size_t view_stride, float* out,
+int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay, float* out,
             int n_planes, cudaStream_t stream);
 int fft_default_chunk(const mvd_handle* h);
 void fft_teardown(mvd_handle* h);
