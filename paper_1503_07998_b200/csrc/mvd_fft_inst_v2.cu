@@ -9,17 +9,17 @@ const SizeOps* mvd_fft_ops_v2(int N) {
     using P512 = Plan<512, 32, 32, 16>;
     using P1024 = Plan<1024, 32, 32, 32>;
     using P2048 = Plan<2048, 32, 32, 32, 2>;
-    using P256C = Plan<256, 32, 32, 8>;      // column plan: four columns per warp, E = 32
     static const SizeOps o256 = OpsFor2<P256, 256, P256, 128, true, 4>::make();
     static const SizeOps o512 = OpsFor2<P512, 256, P512, 128, false, 3>::make();
     static const SizeOps o1024 = OpsFor2<P1024, 256, P1024, 128, false, 3>::make();
     static const SizeOps o2048 = OpsFor2<P2048, 128, P2048, 256, false, 2, false, 4, 3>::make();   // rows: 3 CTAs of 2 teams, 168 registers
     using P800C = Plan<800, 40, 40, 20>;     // columns only: eight columns per team of 160 threads
     static const SizeOps o800 = ColsOnly2<P800C, 160, false, 2, 8>::make();
-    // measurement knob: alternative column kernels for 256
+    // measurement knob MVD_COLS_VARIANT (profiles/r1_fft_v2_ncu_full.md): a = eight, b = sixteen columns per team,
+    // c = dedicated landing zone requested a whole item ahead; all within +-3 % of the default on config 2
     static const SizeOps o256a = OpsFor2<P256, 256, P256, 128, true, 4, true, 8>::make();
     static const SizeOps o256b = OpsFor2<P256, 256, P256, 256, true, 2, true, 16>::make();
-    static const SizeOps o256c = OpsFor2<P256, 256, P256, 128, true, 4>::make();
+    static const SizeOps o256c = OpsFor2<P256, 256, P256, 128, true, 4, true, 4, 2, true>::make();
     static const char* var = getenv("MVD_COLS_VARIANT");
     if (N == 256 && var) {
         if (var[0] == 'a') return &o256a;

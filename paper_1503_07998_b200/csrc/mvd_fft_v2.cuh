@@ -324,7 +324,7 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // box load of the NEXT item into the team's exchange region when the inverse transform has done its
 // last exchange, and the box store of the results from a second region -- no global load or store
 // instruction, and no L1 tag traffic, is left in the loop.
-template <class P, int NT, bool OTF_REGS, int MINB, int CPT = 4>
+template <class P, int NT, bool OTF_REGS, int MINB, int CPT = 4, bool EARLY = false>
 __global__ void __launch_bounds__(NT, MINB)
 fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ otf, int conj_otf,
                      int pairs, int W, const float2* __restrict__ tw_g) {
@@ -336,9 +336,12 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __r
     constexpr int TW = (P::S - 1) * E * TPF;                  // a multiple of 16 float2: regions stay 128-byte aligned
     static_assert(TW % 16 == 0, "twiddle table keeps the regions aligned");
     float2* tw = smem_cols3;                                  // [(S-1) E][TPF]
-    float2* buf = smem_cols3 + TW;                            // [NTEAM][H][CPT]  exchange regions / landing zones
+    // EARLY: a dedicated landing zone per team (the next item is requested a whole item ahead) next to
+    // the exchange region; otherwise the exchange region is the landing zone
+    float2* buf = smem_cols3 + TW;                            // [NTEAM][H][CPT]  exchange regions (/ landing zones)
     float2* obuf = buf + NTEAM * H * CPT;                     // [NTEAM][H][CPT]  results on their way out
-    uint64_t* bars = reinterpret_cast<uint64_t*>(obuf + NTEAM * H * CPT);   // [NTEAM]
+    float2* lbuf = EARLY ? obuf + NTEAM * H * CPT : buf;      // [NTEAM][H][CPT]  landing zones
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_cols3 + TW + (EARLY ? 3 : 2) * NTEAM * H * CPT);   // [NTEAM]
     if (threadIdx.x < NTEAM) mbar_init(&bars[threadIdx.x], 1);
     if (threadIdx.x == 0) fence_mbar_init();
     for (int k = threadIdx.x; k < TW; k += NT) tw[k] = tw_g[k];
@@ -349,7 +352,7 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __r
     const ColAddr2<P, CPT> addr{team * H * CPT + c4};
     const TeamSync<TEAM> sync{team};
     const float sgn = conj_otf ? -1.f : 1.f;
-    float2* land = buf + team * H * CPT;
+    float2* land = lbuf + team * H * CPT;
     float2* outz = obuf + team * H * CPT;
     uint64_t* full = &bars[team];
     const int tiles = W / TC;            // column groups of TC columns
@@ -387,6 +390,7 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __r
 #pragma unroll
         for (int e = 0; e < E; ++e) x[e] = land[(t + TPF * e) * CPT + c4];
         sync();
+        if (EARLY && l == 0 && item + (int)gridDim.x < items) issue(item + gridDim.x);
         fft_run<P, -1>(x, buf, tw, t, addr, sync);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
@@ -401,7 +405,7 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __r
         }
         fft_run_head<P, +1>(x, buf, tw, t, addr, sync);
         if (l == 0) {
-            if (item + (int)gridDim.x < items) issue(item + gridDim.x);
+            if (!EARLY && item + (int)gridDim.x < items) issue(item + gridDim.x);
             bulk_wait_read();            // the previous item's results have left the out region
         }
         fft_run_tail<P, +1>(x, buf, tw, t, addr, sync);
@@ -437,12 +441,12 @@ inline cudaError_t launch_pdl(Kern kern, dim3 grid, dim3 block, size_t smem, cud
     return cudaLaunchKernelEx(&cfg, kern, args...);
 }
 
-template <class P, int NT, class PC, int NTC, bool OTF_REGS, int MINB, bool TMA = true, int CPT = 4, int RMINB = 2>
+template <class P, int NT, class PC, int NTC, bool OTF_REGS, int MINB, bool TMA = true, int CPT = 4, int RMINB = 2, bool EARLY = false>
 struct OpsFor2 {
     static_assert(P::N == PC::N, "row and column plan of one entry describe the same length");
     static constexpr size_t kRowSmem = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * P::N);
     static constexpr int kTeam = CPT * PC::TPF, kNTeam = NTC / kTeam, kTC = CPT * kNTeam;
-    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)(TMA ? 2 : 1) * kNTeam * PC::N * CPT) +
+    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)(TMA ? (EARLY ? 3 : 2) : 1) * kNTeam * PC::N * CPT) +
                                        (TMA ? sizeof(uint64_t) * kNTeam : 0);
 
     static cudaError_t rows(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st) {
@@ -453,7 +457,7 @@ struct OpsFor2 {
     static cudaError_t cols(const CUtensorMap& tmap, float2* S, const float2* otf, int conj_otf, int pairs, int W,
                             const float2* tw, dim3 grid, cudaStream_t st) {
         if constexpr (TMA)
-            return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, grid, dim3(NTC), kColSmem, st, tmap, otf, conj_otf, pairs, W, tw);
+            return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT, EARLY>, grid, dim3(NTC), kColSmem, st, tmap, otf, conj_otf, pairs, W, tw);
         else
         return launch_pdl(fft2_cols_kernel<PC, NTC, OTF_REGS, MINB>, grid, dim3(NTC), kColSmem, st, S, otf, conj_otf, pairs, W, tw);
     }
@@ -467,7 +471,7 @@ struct OpsFor2 {
     }
     static cudaError_t prepare_cols() {
         if constexpr (TMA)
-            return cudaFuncSetAttribute(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
+            return cudaFuncSetAttribute(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT, EARLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
         else
         return cudaFuncSetAttribute(fft2_cols_kernel<PC, NTC, OTF_REGS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
     }
