@@ -11,6 +11,8 @@
 // registers: for one PSF column i it reads a (RY+JC-1)-tall window of the staged column (one
 // conflict-free LDS per value, lanes along x) and issues JC*RY FFMAs on it.  The FP32 FMA pipe is
 // the bound (4 K^2 flop against 22 B of HBM traffic per voxel-view-iteration).
+#include <stdlib.h>
+
 #include "mvd_internal.cuh"
 
 namespace {
@@ -116,6 +118,133 @@ direct_corr_kernel(const float* __restrict__ src, const float* __restrict__ G,
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// The same correlation on TWO planes at once.  The staged tile holds (plane a, plane b) as float2, a
+// thread keeps RY float2 accumulators, and the inner product is FFMA2 (fma.rn.f32x2) with the tap as a
+// broadcast scalar: one issue slot and one shared-memory load now feed two FMAs, which moves the kernel
+// from issue-bound (ncu round 1: 80 % issue slots, 60 % FMA pipe) towards the FMA pipe's own limit.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float2 ffma2_bcast(float g, float2 w, float2 c) {
+    float2 r;
+    asm("{ .reg .b64 ra, rb, rc, rd; mov.b64 ra, {%2,%2}; mov.b64 rb, {%3,%4}; mov.b64 rc, {%5,%6}; "
+        "fma.rn.f32x2 rd, ra, rb, rc; mov.b64 {%0,%1}, rd; }"
+        : "=f"(r.x), "=f"(r.y) : "f"(g), "f"(w.x), "f"(w.y), "f"(c.x), "f"(c.y));
+    return r;
+}
+
+template <int KT, int JC, int MODE>
+__global__ void __launch_bounds__(BX* BY)
+direct_corr2_kernel(const float* __restrict__ src, const float* __restrict__ G,
+                    const uint16_t* __restrict__ phi, float* __restrict__ dst, int W, int H, int Krt,
+                    int Kp, float eps, int tiles_x, int tiles_y, size_t phi_plane, size_t phi_row,
+                    int n_planes) {
+    extern __shared__ __align__(16) float smem[];
+    const int K = KT > 0 ? KT : Krt;
+    const int c = (K - 1) / 2;
+    const int SW = (KT > 0 ? KT : Krt) + BX - 1;   // staged tile width (= pitch)
+    const int SH = TILE_H + Kp - 1;                // staged rows, incl. zero rows for the padded PSF rows
+    float* sG = smem;                              // [K][Kp]  G transposed: sG[i * Kp + j]
+    float2* s = reinterpret_cast<float2*>(smem + ((K * Kp + 1) & ~1));   // [SH][SW] (a, b)
+
+    int t = blockIdx.x;
+    const int tile_x = t % tiles_x; t /= tiles_x;
+    const int tile_y = t % tiles_y; t /= tiles_y;   // t: pair index
+    const int pa = 2 * t;
+    const bool has_b = pa + 1 < n_planes;
+    const size_t offa = (size_t)pa * W * H, offb = has_b ? offa + (size_t)W * H : offa;
+    const int x0 = tile_x * BX, y0 = tile_y * TILE_H;
+    const int tid = threadIdx.y * BX + threadIdx.x;
+
+    for (int k = tid; k < K * Kp; k += BX * BY) sG[k] = G[k];
+
+    {   // stage the tile with periodic wrap: s[ty][tx] = src(y0 - c + ty, x0 - c + tx) of both planes
+        const float* spa = src + offa;
+        const float* spb = src + offb;
+        const int lane = tid & 31, warp = tid >> 5;
+        const int real_rows = TILE_H + K - 1;
+        for (int tx = lane; tx < SW; tx += 32) {
+            const int gx = pmod(x0 - c + tx, W);
+            int gy = pmod(y0 - c + warp, H);
+            for (int ty = warp; ty < SH; ty += (BX * BY) / 32) {
+                s[ty * SW + tx] = ty < real_rows ? make_float2(spa[(size_t)gy * W + gx], spb[(size_t)gy * W + gx])
+                                                 : make_float2(0.f, 0.f);
+                gy += (BX * BY) / 32;
+                while (gy >= H) gy -= H;
+            }
+        }
+    }
+    __syncthreads();
+
+    float2 acc[RY];
+#pragma unroll
+    for (int m = 0; m < RY; ++m) acc[m] = make_float2(0.f, 0.f);
+
+    const float2* sbase = s + (threadIdx.y * RY) * SW + threadIdx.x;
+    for (int i = 0; i < K; ++i) {
+        const float* sg = sG + i * Kp;
+        const float2* scol = sbase + i;
+        for (int jc = 0; jc < Kp; jc += JC) {
+            float2 w[RY + JC - 1];
+#pragma unroll
+            for (int n = 0; n < RY + JC - 1; ++n) w[n] = scol[(jc + n) * SW];
+            float g[JC];
+#pragma unroll
+            for (int jj = 0; jj < JC; ++jj) g[jj] = sg[jc + jj];
+#pragma unroll
+            for (int jj = 0; jj < JC; ++jj)
+#pragma unroll
+                for (int m = 0; m < RY; ++m) acc[m] = ffma2_bcast(g[jj], w[m + jj], acc[m]);
+        }
+    }
+
+    const int x = x0 + threadIdx.x;
+    if (x < W) {
+#pragma unroll
+        for (int m = 0; m < RY; ++m) {
+            const int y = y0 + threadIdx.y * RY + m;
+            if (y < H) {
+                const size_t q = (size_t)y * W + x;
+                if (MODE == 0) {                                              // a2
+                    const size_t f = (size_t)pa * phi_plane + (size_t)y * phi_row + x;
+                    dst[offa + q] = (float)phi[f] / fmaxf(acc[m].x, eps);
+                    if (has_b) dst[offb + q] = (float)phi[f + phi_plane] / fmaxf(acc[m].y, eps);
+                } else {                                                      // a4
+                    dst[offa + q] = dst[offa + q] * acc[m].x;
+                    if (has_b) dst[offb + q] = dst[offb + q] * acc[m].y;
+                }
+            }
+        }
+    }
+}
+
+inline size_t pair_smem_bytes(int K, int Kp) {
+    return sizeof(float) * (size_t)((K * Kp + 1) & ~1) + sizeof(float2) * (size_t)(TILE_H + Kp - 1) * (K + BX - 1);
+}
+
+template <int KT, int JC>
+int launch_pair2(int mode, const float* src, const float* G, const uint16_t* phi, float* dst,
+                 int W, int H, int K, int Kp, float eps, int n_planes, cudaStream_t st,
+                 size_t phi_plane, size_t phi_row) {
+    const int tiles_x = (W + BX - 1) / BX, tiles_y = (H + TILE_H - 1) / TILE_H;
+    const size_t smem = pair_smem_bytes(K, Kp);
+    const long long grid = (long long)((n_planes + 1) / 2) * tiles_x * tiles_y;
+    if (grid > 0x7fffffffLL) return (int)cudaErrorInvalidConfiguration;
+    dim3 block(BX, BY);
+    cudaError_t e;
+    if (mode == 0) {
+        auto k = direct_corr2_kernel<KT, JC, 0>;
+        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return (int)e;
+        k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row, n_planes);
+    } else {
+        auto k = direct_corr2_kernel<KT, JC, 1>;
+        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return (int)e;
+        k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row, n_planes);
+    }
+    return (int)cudaGetLastError();
+}
+
 template <int KT, int JC>
 int launch_pair_member(int mode, const float* src, const float* G, const uint16_t* phi, float* dst,
                        int W, int H, int K, int Kp, float eps, int n_planes, cudaStream_t st,
@@ -142,16 +271,31 @@ int launch_pair_member(int mode, const float* src, const float* G, const uint16_
 
 int launch_corr(int mode, const mvd_handle* h, const float* src, const float* G, const uint16_t* phi,
                 float* dst, int n_planes, cudaStream_t st, size_t phi_plane, size_t phi_row) {
+    // two planes per thread whenever the float2 tile fits in shared memory; K as a template
+    // parameter for the config sizes
+    if (pair_smem_bytes(h->K, h->Kp) <= 227u * 1024u && getenv("MVD_DIRECT_SINGLE") == nullptr) {
 #define MVD_DIRECT_CASE(KT_, JC_)                                                                 \
     if (h->K == (KT_) && h->JC == (JC_))                                                          \
-        return launch_pair_member<KT_, JC_>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp,       \
-                                            h->eps, n_planes, st, phi_plane, phi_row);
-    MVD_DIRECT_CASE(9, 9)
-    MVD_DIRECT_CASE(21, 21)
-    MVD_DIRECT_CASE(31, 16)
-    MVD_DIRECT_CASE(41, 21)
-    MVD_DIRECT_CASE(51, 17)
+        return launch_pair2<KT_, JC_>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp,             \
+                                      h->eps, n_planes, st, phi_plane, phi_row);
+        MVD_DIRECT_CASE(9, 9)
+        MVD_DIRECT_CASE(21, 7)
+        MVD_DIRECT_CASE(21, 11)
+        MVD_DIRECT_CASE(21, 21)
+        MVD_DIRECT_CASE(31, 8)
+        MVD_DIRECT_CASE(31, 11)
+        MVD_DIRECT_CASE(41, 7)
+        MVD_DIRECT_CASE(41, 14)
+        MVD_DIRECT_CASE(51, 9)
+        MVD_DIRECT_CASE(51, 13)
+        MVD_DIRECT_CASE(51, 17)
 #undef MVD_DIRECT_CASE
+        if (h->JC == 8)
+            return launch_pair2<0, 8>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp, h->eps, n_planes, st,
+                                      phi_plane, phi_row);
+    }
+    if (h->JC == 9) return launch_pair_member<0, 9>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp, h->eps, n_planes, st, phi_plane, phi_row);
+    if (h->JC == 7) return launch_pair_member<0, 7>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp, h->eps, n_planes, st, phi_plane, phi_row);
     return launch_pair_member<0, 8>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp, h->eps,
                                     n_planes, st, phi_plane, phi_row);
 }
@@ -162,12 +306,18 @@ int launch_corr(int mode, const mvd_handle* h, const float* src, const float* G,
 int direct_choose_chunk(int K, int* JC, int* Kp) {
     int jc;
     switch (K) {
-        case 9: jc = 9; break;
-        case 21: jc = 21; break;
-        case 31: jc = 16; break;
-        case 41: jc = 21; break;
+        case 9: jc = 9; break;      // row chunks sized for the two-plane kernel's register budget
+        case 21: jc = 7; break;
+        case 31: jc = 8; break;
+        case 41: jc = 7; break;
         case 51: jc = 17; break;
         default: jc = 8; break;
+    }
+    if (const char* e = getenv("MVD_DIRECT_JC")) {   // measurement knob
+        const int v = atoi(e);
+        if ((K == 21 && (v == 7 || v == 11 || v == 21)) || (K == 31 && (v == 8 || v == 11)) ||
+            (K == 41 && (v == 7 || v == 14)) || (K == 51 && (v == 9 || v == 13 || v == 17)))
+            jc = v;
     }
     *JC = jc;
     *Kp = ((K + jc - 1) / jc) * jc;
