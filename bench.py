@@ -143,6 +143,29 @@ def oracle_sample(cfg, psfs, views, n_planes, steps=1, warmup=0):
     return units / dt / 1e6, dt, min(cores, n_planes), cores
 
 
+def cpu_baseline(cfg, psfs, views, n_forced=0, target_s=15.0):
+    """The oracle as it stands on a bounded sample of this workload: one plane per core and one RL
+    iteration as a pilot, then as many planes (all T iterations) -- or, when a single plane's T
+    iterations alone exceed the budget, as many iterations of one plane per core -- as fit ~target_s."""
+    import dataclasses
+    from oracle import mvd_oracle
+    cores = mvd_oracle.n_cores()
+    N, T = cfg.N, cfg.T
+    n0 = max(1, min(N, cores))
+    if n_forced:
+        val, dt, used, cores = oracle_sample(cfg, psfs, views, min(n_forced, N))
+        n, Ts = min(n_forced, N), T
+    else:
+        _, t1, _, _ = oracle_sample(dataclasses.replace(cfg, T=1), psfs, views, n0)       # pilot
+        if t1 * T <= target_s:
+            n, Ts = int(min(N, n0 * max(1, int(target_s / (t1 * T))))), T
+        else:
+            n, Ts = n0, max(1, int(target_s / t1))
+        val, dt, used, cores = oracle_sample(dataclasses.replace(cfg, T=Ts), psfs, views, n)
+    return {"value": val, "unit": UNIT, "cores": used, "kind": "oracle", "seconds": round(dt, 2),
+            "sample": f"first {n} of {N} planes, {Ts} of {T} iterations, one plane per thread"}
+
+
 def run_reference(args, cfg):
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
@@ -323,15 +346,10 @@ def main():
         e2e["bit_identical_to_device_resident"] = same
     sampler.stop()
 
-    # ---- the oracle beside it (rank 0, N = 1 only) -------------------------------------------
+    # ---- the oracle beside it (rank 0, N = 1 only): a bounded sample of about 10-30 s of CPU work ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
-        from oracle import mvd_oracle
-        cores = mvd_oracle.n_cores()
-        n_cpu = args.cpu_planes or max(1, min(N, 2 * cores, 32))
-        val, dt, used, cores = oracle_sample(cfg, psfs, views, n_cpu)
-        cpu = {"value": val, "unit": UNIT, "cores": used, "kind": "oracle", "seconds": round(dt, 2),
-               "sample": f"first {n_cpu} of {N} planes, all {T} iterations, one plane per thread"}
+        cpu = cpu_baseline(cfg, psfs, views, args.cpu_planes)
     m.destroy()
 
     if rank == 0:
