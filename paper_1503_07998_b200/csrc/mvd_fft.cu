@@ -109,6 +109,8 @@ struct FftState {
     float2* tw_row = nullptr;
     float2* tw_col = nullptr;
     EncodeTiledFn encode = nullptr; // cuTensorMapEncodeTiled, resolved through the runtime (no -lcuda)
+    // generation-2 column kernels without OTF registers fetch their OTF slice by TMA: one map per view
+    std::vector<CUtensorMap> otf_maps, otf_b_maps;
 };
 
 // Tensor map of the spectrum buffer S = float [pairs * H][2 W] with a box of one column tile:
@@ -123,6 +125,22 @@ int make_col_tensor_map(mvd_handle* h, const FftState* st, float2* S, int pairs,
     const cuuint32_t box[2] = {v2 ? (cuuint32_t)st->col->col_box_w : (cuuint32_t)(2 * st->col->col_tc), (cuuint32_t)st->col->col_box_h};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = st->encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, S, dims, strides, box, estr,
+                                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                  CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        h->last_cuda = (int)cudaErrorInvalidValue;
+        return MVD_ERR_CUDA;
+    }
+    return MVD_OK;
+}
+
+// Tensor map of one view's tile-major OTF, float [(W/16) * H][32], same box as the spectrum's map.
+int make_otf_tensor_map(mvd_handle* h, const FftState* st, const float2* otf, CUtensorMap* map) {
+    const cuuint64_t dims[2] = {32, (cuuint64_t)(h->W / 16) * h->H};
+    const cuuint64_t strides[1] = {128};
+    const cuuint32_t box[2] = {(cuuint32_t)st->col->col_box_w, (cuuint32_t)st->col->col_box_h};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = st->encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)otf, dims, strides, box, estr,
                                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
                                   CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
     if (r != CUDA_SUCCESS) {
@@ -220,6 +238,17 @@ int fft_setup(mvd_handle* h, const float* host_psfs, const float* host_xs) {
     };
     rc = build_otfs(host_psfs, h->K, &h->d_otf);
     if (rc == MVD_OK && host_xs) rc = build_otfs(host_xs, h->KX, &h->d_otf_b);
+    if (rc == MVD_OK && st.col->generation == 2 && st.col->col_box_h > 0 && !st.col->col_otf_regs) {
+        FftState* fs = state_of(h);
+        fs->otf_maps.resize(h->V);
+        for (int v = 0; v < h->V && rc == MVD_OK; ++v)
+            rc = make_otf_tensor_map(h, fs, h->d_otf + (size_t)v * npx, &fs->otf_maps[v]);
+        if (h->d_otf_b) {
+            fs->otf_b_maps.resize(h->V);
+            for (int v = 0; v < h->V && rc == MVD_OK; ++v)
+                rc = make_otf_tensor_map(h, fs, h->d_otf_b + (size_t)v * npx, &fs->otf_b_maps[v]);
+        }
+    }
     h->launches = 0;
     return rc;
 }
@@ -298,7 +327,8 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay,
             const float2* otf = h->d_otf + (size_t)v * npx;
             {
                 LaunchScope ls(h, KC_FFT_COLS, stream);
-                rc = mvd_check(h, st->col->cols(tmap, a.S, otf, 0, pairs, W, st->tw_col, col_grid, stream));   // a1
+                rc = mvd_check(h, st->col->cols(tmap, st->otf_maps.empty() ? tmap : st->otf_maps[v], a.S, otf, 0, pairs, W,
+                                                st->tw_col, col_grid, stream));   // a1
             }
             if (rc != MVD_OK) return rc;
             {
@@ -311,8 +341,10 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay,
             {
                 LaunchScope ls(h, KC_FFT_COLS, stream);
                 rc = h->d_otf_b      // a3: explicit back-projector B_v, or conj O_v (X = P_v^*)
-                         ? mvd_check(h, st->col->cols(tmap, a.S, h->d_otf_b + (size_t)v * npx, 0, pairs, W, st->tw_col, col_grid, stream))
-                         : mvd_check(h, st->col->cols(tmap, a.S, otf, 1, pairs, W, st->tw_col, col_grid, stream));
+                         ? mvd_check(h, st->col->cols(tmap, st->otf_b_maps.empty() ? tmap : st->otf_b_maps[v], a.S,
+                                                      h->d_otf_b + (size_t)v * npx, 0, pairs, W, st->tw_col, col_grid, stream))
+                         : mvd_check(h, st->col->cols(tmap, st->otf_maps.empty() ? tmap : st->otf_maps[v], a.S, otf, 1, pairs, W,
+                                                      st->tw_col, col_grid, stream));
             }
             if (rc != MVD_OK) return rc;
             {

@@ -797,7 +797,7 @@ struct SizeOps {
     int col_tc;                      // TC of the column kernel
     cudaError_t (*rows)(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st);
     int col_box_h;                   // rows per TMA box of the column kernel's tile
-    cudaError_t (*cols)(const CUtensorMap& tmap, float2* S, const float2* otf, int conj_otf, int pairs, int W,
+    cudaError_t (*cols)(const CUtensorMap& tmap, const CUtensorMap& otf_map, float2* S, const float2* otf, int conj_otf, int pairs, int W,
                         const float2* tw, dim3 grid, cudaStream_t st);
     cudaError_t (*prepare_rows)();   // opt in to > 48 KB dynamic shared memory (length used as W)
     cudaError_t (*prepare_cols)();   // same (length used as H)
@@ -821,8 +821,9 @@ struct OpsFor {
         else fft_rows_tma_kernel<P, ROWS_UPDATE, NT><<<grid, NT, kUpdateSmem, st>>>(a, tw);
         return cudaGetLastError();
     }
-    static cudaError_t cols(const CUtensorMap& tmap, float2* S, const float2* otf, int conj_otf, int pairs, int W,
+    static cudaError_t cols(const CUtensorMap& tmap, const CUtensorMap& otf_map, float2* S, const float2* otf, int conj_otf, int pairs, int W,
                             const float2* tw, dim3 grid, cudaStream_t st) {
+        (void)otf_map;
         fft_cols_tma_kernel<PC, TC, OTF_REGS><<<grid, TC * PC::TPF, kColSmem, st>>>(tmap, S, otf, conj_otf, pairs, W, tw);
         return cudaGetLastError();
     }

@@ -326,8 +326,8 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // instruction, and no L1 tag traffic, is left in the loop.
 template <class P, int NT, bool OTF_REGS, int MINB, int CPT = 4, bool EARLY = false>
 __global__ void __launch_bounds__(NT, MINB)
-fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ otf, int conj_otf,
-                     int pairs, int W, const float2* __restrict__ tw_g) {
+fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap omap,
+                     const float2* __restrict__ otf, int conj_otf, int pairs, int W, const float2* __restrict__ tw_g) {
     constexpr int E = P::E, TPF = P::TPF, H = P::N, TEAM = CPT * TPF, NTEAM = NT / TEAM, TC = CPT * NTEAM;
     constexpr int BOXH = H <= 256 ? H : (H % 256 == 0 ? 256 : 200);
     static_assert(H % BOXH == 0 && (CPT == 4 || CPT == 8 || CPT == 16), "whole boxes; a team owns whole 32-byte sectors of a row");
@@ -341,8 +341,8 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __r
     float2* buf = smem_cols3 + TW;                            // [NTEAM][H][CPT]  exchange regions (/ landing zones)
     float2* obuf = buf + NTEAM * H * CPT;                     // [NTEAM][H][CPT]  results on their way out
     float2* lbuf = EARLY ? obuf + NTEAM * H * CPT : buf;      // [NTEAM][H][CPT]  landing zones
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_cols3 + TW + (EARLY ? 3 : 2) * NTEAM * H * CPT);   // [NTEAM]
-    if (threadIdx.x < NTEAM) mbar_init(&bars[threadIdx.x], 1);
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_cols3 + TW + (EARLY ? 3 : 2) * NTEAM * H * CPT);   // [2][NTEAM]
+    if (threadIdx.x < 2 * NTEAM) mbar_init(&bars[threadIdx.x], 1);
     if (threadIdx.x == 0) fence_mbar_init();
     for (int k = threadIdx.x; k < TW; k += NT) tw[k] = tw_g[k];
     __syncthreads();
@@ -355,6 +355,7 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __r
     float2* land = lbuf + team * H * CPT;
     float2* outz = obuf + team * H * CPT;
     uint64_t* full = &bars[team];
+    uint64_t* full_otf = &bars[NTEAM + team];   // !OTF_REGS: the team's OTF slice lands in the out region
     const int tiles = W / TC;            // column groups of TC columns
     const int items = tiles * pairs;
     auto first_col = [&](int item) { return (item % tiles) * TC + team * CPT; };
@@ -391,22 +392,35 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __r
         for (int e = 0; e < E; ++e) x[e] = land[(t + TPF * e) * CPT + c4];
         sync();
         if (EARLY && l == 0 && item + (int)gridDim.x < items) issue(item + gridDim.x);
-        fft_run<P, -1>(x, buf, tw, t, addr, sync);
+        if (!OTF_REGS && l == 0) {
+            // The OTF slice of these columns (same tile-major tensor shape as S, one "pair" per view)
+            // comes through the TMA unit into the out region, which the previous item's results have
+            // left by now; it has the whole forward transform's time to arrive.
+            bulk_wait_read();
+            fence_proxy_async();
+            mbar_arrive_expect_tx(full_otf, (uint32_t)(sizeof(float2) * H * CPT));
+            const int oy = (first_col(item) >> 4) * H;
 #pragma unroll
-        for (int e = 0; e < E; ++e) {
-            float2 w;
-            if (OTF_REGS) {
-                w = o[e];
-            } else {
-                w = __ldg(otf + plane_off(xg) + (size_t)(t + TPF * e) * 16);
+            for (int b = 0; b < H / BOXH; ++b) tma_2d_g2s(outz + b * BOXH * CPT, &omap, box_x(item), oy + b * BOXH, full_otf);
+        }
+        fft_run<P, -1>(x, buf, tw, t, addr, sync);
+        if (OTF_REGS) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) x[e] = cmul(x[e], o[e]);
+        } else {
+            mbar_wait(full_otf, phase ^ 1);      // same parity sequence as `full`: one completion per item
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                float2 w = outz[(t + TPF * e) * CPT + c4];
                 w.y *= sgn;
+                x[e] = cmul(x[e], w);
             }
-            x[e] = cmul(x[e], w);
+            sync();                              // the out region is free for this item's results
         }
         fft_run_head<P, +1>(x, buf, tw, t, addr, sync);
         if (l == 0) {
             if (!EARLY && item + (int)gridDim.x < items) issue(item + gridDim.x);
-            bulk_wait_read();            // the previous item's results have left the out region
+            if (OTF_REGS) bulk_wait_read();   // the previous item's results have left the out region
         }
         fft_run_tail<P, +1>(x, buf, tw, t, addr, sync);
         sync();                          // ... and every thread of the team knows it
@@ -447,17 +461,17 @@ struct OpsFor2 {
     static constexpr size_t kRowSmem = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * P::N);
     static constexpr int kTeam = CPT * PC::TPF, kNTeam = NTC / kTeam, kTC = CPT * kNTeam;
     static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)(TMA ? (EARLY ? 3 : 2) : 1) * kNTeam * PC::N * CPT) +
-                                       (TMA ? sizeof(uint64_t) * kNTeam : 0);
+                                       (TMA ? 2 * sizeof(uint64_t) * kNTeam : 0);
 
     static cudaError_t rows(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st) {
         if (mode == ROWS_FIRST) return launch_pdl(fft2_rows_kernel<P, ROWS_FIRST, NT, RMINB>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
         if (mode == ROWS_RATIO) return launch_pdl(fft2_rows_kernel<P, ROWS_RATIO, NT, RMINB>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
         return launch_pdl(fft2_rows_kernel<P, ROWS_UPDATE, NT, RMINB>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
     }
-    static cudaError_t cols(const CUtensorMap& tmap, float2* S, const float2* otf, int conj_otf, int pairs, int W,
+    static cudaError_t cols(const CUtensorMap& tmap, const CUtensorMap& otf_map, float2* S, const float2* otf, int conj_otf, int pairs, int W,
                             const float2* tw, dim3 grid, cudaStream_t st) {
         if constexpr (TMA)
-            return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT, EARLY>, grid, dim3(NTC), kColSmem, st, tmap, otf, conj_otf, pairs, W, tw);
+            return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT, EARLY>, grid, dim3(NTC), kColSmem, st, tmap, otf_map, otf, conj_otf, pairs, W, tw);
         else
         return launch_pdl(fft2_cols_kernel<PC, NTC, OTF_REGS, MINB>, grid, dim3(NTC), kColSmem, st, S, otf, conj_otf, pairs, W, tw);
     }
@@ -499,10 +513,10 @@ struct ColsOnly2 {
     static constexpr int kTeam = CPT * PC::TPF, kNTeam = NTC / kTeam, kTC = CPT * kNTeam;
     static constexpr int kBoxH = PC::N <= 256 ? PC::N : (PC::N % 256 == 0 ? 256 : 200);
     static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)2 * kNTeam * PC::N * CPT) +
-                                       sizeof(uint64_t) * kNTeam;
-    static cudaError_t cols(const CUtensorMap& tmap, float2*, const float2* otf, int conj_otf, int pairs, int W,
+                                       2 * sizeof(uint64_t) * kNTeam;
+    static cudaError_t cols(const CUtensorMap& tmap, const CUtensorMap& otf_map, float2*, const float2* otf, int conj_otf, int pairs, int W,
                             const float2* tw, dim3 grid, cudaStream_t st) {
-        return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, grid, dim3(NTC), kColSmem, st, tmap, otf, conj_otf, pairs, W, tw);
+        return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, grid, dim3(NTC), kColSmem, st, tmap, otf_map, otf, conj_otf, pairs, W, tw);
     }
     static cudaError_t prepare_cols() {
         return cudaFuncSetAttribute(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
