@@ -50,6 +50,7 @@ def parse():
     ap.add_argument("--path", default="auto", choices=["auto", "direct", "fft"])
     ap.add_argument("--chunk", type=int, default=0, help="mvd_set_chunk_planes (0 = library default)")
     ap.add_argument("--batch", type=int, default=0, help="mvd_set_batch_planes (0 = library default)")
+    ap.add_argument("--streams", type=int, default=0, help="mvd_set_resident_streams (0 = library default)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--cpu-planes", type=int, default=0, help="planes in the oracle sample (0 = 2 per core, <= 32)")
@@ -265,6 +266,8 @@ def main():
         m.set_chunk_planes(args.chunk)
     if args.batch:
         m.set_batch_planes(args.batch)
+    if args.streams:
+        m.set_resident_streams(args.streams)
     path_name = binding.PATH_NAMES[m.path]
 
     # ---- device-resident: warm-up, then exactly K timed steps -------------------------------

@@ -171,7 +171,11 @@ MVD_API int mvd_path_supported(int path, int plane_w, int plane_h, int psf_size)
  * Tuning knobs (measurement; defaults are chosen in mvd_create).
  *   mvd_set_chunk_planes  planes processed per internal pass of mvd_deconvolve_planes (0 = default)
  *   mvd_set_batch_planes  planes per pipeline batch of mvd_deconvolve_host (0 = default)
+ *   mvd_set_resident_streams  1..3: mvd_deconvolve_planes deals batches of planes (the pipeline's batch size)
+ *                         to this many internal streams forked from / joined to the caller's stream, so that
+ *                         kernel tails of one batch overlap the next batch; results are bit-identical
  */
+MVD_API int mvd_set_resident_streams(mvd_handle* h, int n);
 MVD_API int mvd_set_chunk_planes(mvd_handle* h, int planes);
 MVD_API int mvd_set_batch_planes(mvd_handle* h, int planes);
 

@@ -39,6 +39,7 @@ SIGNATURES = {
     "mvd_path_supported": (_i, [_i, _i, _i, _i]),
     "mvd_set_chunk_planes": (_i, [_vp, _i]),
     "mvd_set_batch_planes": (_i, [_vp, _i]),
+    "mvd_set_resident_streams": (_i, [_vp, _i]),
     "mvd_launch_count": (_ll, [_vp]),
     "mvd_launch_count_reset": (None, [_vp]),
     "mvd_profile_enable": (_i, [_vp, _i]),
@@ -164,6 +165,9 @@ class Mvd:
     def set_chunk_planes(self, planes: int) -> None:
         self._raise(lib().mvd_set_chunk_planes(self._h, planes), "mvd_set_chunk_planes")
 
+    def set_resident_streams(self, n: int) -> None:
+        self._raise(lib().mvd_set_resident_streams(self._h, n), "mvd_set_resident_streams")
+
     def set_batch_planes(self, planes: int) -> None:
         self._raise(lib().mvd_set_batch_planes(self._h, planes), "mvd_set_batch_planes")
 
@@ -242,7 +246,8 @@ def build_backprojectors(variant: int, psfs: np.ndarray) -> np.ndarray:
 
 def deconvolve(views: np.ndarray, psfs: np.ndarray, iterations: int, eps: float = 1e-6,
                path: Optional[int] = None, host: bool = False, chunk_planes: int = 0,
-               batch_planes: int = 0, backprojectors: Optional[np.ndarray] = None) -> np.ndarray:
+               batch_planes: int = 0, backprojectors: Optional[np.ndarray] = None,
+               resident_streams: int = 0) -> np.ndarray:
     """Convenience for tests: numpy uint16 `[V][N][H][W]` in, numpy float32 `[N][H][W]` out, through
     mvd_deconvolve_planes (host=False) or mvd_deconvolve_host (host=True, pinned buffers)."""
     import torch
@@ -256,6 +261,8 @@ def deconvolve(views: np.ndarray, psfs: np.ndarray, iterations: int, eps: float 
             m.set_chunk_planes(chunk_planes)
         if batch_planes:
             m.set_batch_planes(batch_planes)
+        if resident_streams:
+            m.set_resident_streams(resident_streams)
         tv = torch.from_numpy(views.view(np.int16))
         if host:
             hv = tv.pin_memory()

@@ -229,7 +229,9 @@ void mvd_destroy(mvd_handle* h) {
         if (h->d_in[s]) cudaFree(h->d_in[s]);
         if (h->d_out[s]) cudaFree(h->d_out[s]);
         if (h->streams[s]) cudaStreamDestroy(h->streams[s]);
+        if (h->ev_join[s]) cudaEventDestroy(h->ev_join[s]);
     }
+    if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     if (h->d_coef) cudaFree(h->d_coef);
     if (h->d_otf) cudaFree(h->d_otf);
     if (h->d_otf_b) cudaFree(h->d_otf_b);
@@ -269,14 +271,45 @@ static int run_core(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLay
     return MVD_OK;
 }
 
+static int default_batch(const mvd_handle* h, int n_planes);
+
+// Device-resident work on `lay`: one stream, or batches dealt round-robin to internal streams that fork
+// from and join the caller's stream (planes are independent; results do not depend on the split).
+static int run_resident(mvd_handle* h, const uint16_t* views, ViewLayout lay, float* out, int n_planes,
+                        cudaStream_t stream) {
+    const size_t npx = (size_t)h->W * h->H;
+    const int B = default_batch(h, n_planes);
+    const int ns = std::min(h->resident_streams, mvd_handle::kSlots);
+    if (ns <= 1 || h->profiling || n_planes <= B) return run_core(h, h->ws_main, views, lay, out, n_planes, stream);
+    if (!h->ev_fork) MVD_TRY(h, cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+    for (int s = 0; s < ns; ++s) {
+        if (!h->streams[s]) MVD_TRY(h, cudaStreamCreateWithFlags(&h->streams[s], cudaStreamNonBlocking));
+        if (!h->ev_join[s]) MVD_TRY(h, cudaEventCreateWithFlags(&h->ev_join[s], cudaEventDisableTiming));
+    }
+    MVD_TRY(h, cudaEventRecord(h->ev_fork, stream));
+    for (int s = 0; s < ns; ++s) MVD_TRY(h, cudaStreamWaitEvent(h->streams[s], h->ev_fork, 0));
+    int rc = MVD_OK, k = 0;
+    for (int p0 = 0; p0 < n_planes && rc == MVD_OK; p0 += B, ++k) {
+        const int s = k % ns;
+        rc = run_core(h, h->ws_slot[s], views + (size_t)p0 * lay.plane, lay, out + (size_t)p0 * npx,
+                      std::min(B, n_planes - p0), h->streams[s]);
+    }
+    for (int s = 0; s < ns; ++s) {   // join even after an error so that the caller's stream stays ordered
+        int rj = mvd_check(h, cudaEventRecord(h->ev_join[s], h->streams[s]));
+        if (rj == MVD_OK) rj = mvd_check(h, cudaStreamWaitEvent(stream, h->ev_join[s], 0));
+        if (rc == MVD_OK) rc = rj;
+    }
+    return rc;
+}
+
 int mvd_deconvolve_planes(mvd_handle* h, const uint16_t* dev_views_u16, float* dev_out_f32,
                           int n_planes, void* stream) {
     if (!h || n_planes < 0) return MVD_ERR_INVALID;
     if (n_planes == 0) return MVD_OK;
     if (!dev_views_u16 || !dev_out_f32) return MVD_ERR_INVALID;
     const size_t npx = (size_t)h->W * h->H;
-    return run_core(h, h->ws_main, dev_views_u16, ViewLayout{(size_t)n_planes * npx, npx, (size_t)h->W},
-                    dev_out_f32, n_planes, (cudaStream_t)stream);
+    return run_resident(h, dev_views_u16, ViewLayout{(size_t)n_planes * npx, npx, (size_t)h->W},
+                        dev_out_f32, n_planes, (cudaStream_t)stream);
 }
 
 int mvd_deconvolve_planes_strided(mvd_handle* h, const uint16_t* dev_views_u16, size_t view_stride,
@@ -286,8 +319,8 @@ int mvd_deconvolve_planes_strided(mvd_handle* h, const uint16_t* dev_views_u16, 
     if (n_planes == 0) return MVD_OK;
     if (!dev_views_u16 || !dev_out_f32) return MVD_ERR_INVALID;
     if (row_stride < (size_t)h->W || plane_stride < 1 || (h->V > 1 && view_stride < 1)) return MVD_ERR_INVALID;
-    return run_core(h, h->ws_main, dev_views_u16, ViewLayout{view_stride, plane_stride, row_stride},
-                    dev_out_f32, n_planes, (cudaStream_t)stream);
+    return run_resident(h, dev_views_u16, ViewLayout{view_stride, plane_stride, row_stride},
+                        dev_out_f32, n_planes, (cudaStream_t)stream);
 }
 
 static int default_batch(const mvd_handle* h, int n_planes) {
@@ -397,6 +430,12 @@ int mvd_get_path(const mvd_handle* h) { return h ? h->path : MVD_ERR_INVALID; }
 int mvd_set_chunk_planes(mvd_handle* h, int planes) {
     if (!h || planes < 0) return MVD_ERR_INVALID;
     h->chunk_planes = planes;
+    return MVD_OK;
+}
+
+int mvd_set_resident_streams(mvd_handle* h, int n) {
+    if (!h || n < 1 || n > mvd_handle::kSlots) return MVD_ERR_INVALID;
+    h->resident_streams = n;
     return MVD_OK;
 }
 

@@ -61,6 +61,11 @@ struct mvd_handle {
     float* d_out[kSlots] = {nullptr, nullptr, nullptr};
     size_t slot_planes = 0;
 
+    // device-resident calls: planes are dealt in batches to this many internal streams, forked from and
+    // joined to the caller's stream, so that one batch's kernel tails overlap the next batch's kernels
+    int resident_streams = 2;   // measured: 2 beats 1 by 7-20 % and 3 by 3-10 % on configs 2-5
+    cudaEvent_t ev_fork = nullptr, ev_join[kSlots] = {nullptr, nullptr, nullptr};
+
     int chunk_planes = 0;   // 0 = default
     int batch_planes = 0;   // 0 = default
 

@@ -199,6 +199,8 @@ def test_generation2_is_deterministic_and_independent_of_batching():
         assert np.array_equal(base, _run(pr.views, pr.psfs, T, binding.PATH_FFT))
     assert np.array_equal(base, _run(pr.views, pr.psfs, T, binding.PATH_FFT, chunk_planes=4))
     assert np.array_equal(base, _run(pr.views, pr.psfs, T, binding.PATH_FFT, chunk_planes=2))
+    for streams in (1, 2, 3):          # forked internal streams of the device-resident call
+        assert np.array_equal(base, _run(pr.views, pr.psfs, T, binding.PATH_FFT, batch_planes=2, resident_streams=streams))
     assert np.array_equal(base, _run(pr.views, pr.psfs, T, binding.PATH_FFT, host=True))
     assert np.array_equal(base, _run(pr.views, pr.psfs, T, binding.PATH_FFT, host=True, batch_planes=2, chunk_planes=2))
     assert np.array_equal(base, _run(pr.views, pr.psfs, T, binding.PATH_FFT, host=True, batch_planes=6))
