@@ -326,11 +326,11 @@ int mvd_deconvolve_planes_strided(mvd_handle* h, const uint16_t* dev_views_u16, 
 static int default_batch(const mvd_handle* h, int n_planes) {
     if (h->batch_planes > 0)
         return h->path == MVD_PATH_FFT ? even_up(h->batch_planes) : std::min(h->batch_planes, n_planes);
-    // ~64 MiB of uint16 input per batch, at least 12 batches when the stack allows it so that the
+    // ~64 MiB of uint16 input per batch, at least 16 batches when the stack allows it so that the
     // pipeline's fill and drain (one H2D and one D2H that overlap nothing) stay a few percent
     const size_t per_plane = (size_t)h->W * h->H * sizeof(uint16_t) * h->V;
     size_t b = std::max<size_t>(1, ((size_t)64 << 20) / per_plane);
-    b = std::min<size_t>(b, std::max(1, n_planes / 12));
+    b = std::min<size_t>(b, std::max(1, n_planes / 16));
     b = std::max<size_t>(1, std::min<size_t>(b, (size_t)n_planes));
     return h->path == MVD_PATH_FFT ? even_up((int)b) : (int)b;
 }
@@ -346,8 +346,10 @@ static int host_pipeline(mvd_handle* h, const uint16_t* host_views_u16, float* h
     const size_t npx = (size_t)h->W * h->H;
     const int B = default_batch(h, n_planes);
 
-    for (int s = 0; s < mvd_handle::kSlots; ++s)
+    for (int s = 0; s < mvd_handle::kSlots; ++s) {
         if (!h->streams[s]) MVD_TRY(h, cudaStreamCreateWithFlags(&h->streams[s], cudaStreamNonBlocking));
+        if (!h->ev_join[s]) MVD_TRY(h, cudaEventCreateWithFlags(&h->ev_join[s], cudaEventDisableTiming));
+    }
     if ((size_t)B > h->slot_planes) {
         MVD_TRY(h, cudaDeviceSynchronize());
         for (int s = 0; s < mvd_handle::kSlots; ++s) {
@@ -387,7 +389,11 @@ static int host_pipeline(mvd_handle* h, const uint16_t* host_views_u16, float* h
                                                  host_views_u16 + ((size_t)v * n_planes + p0) * npx,
                                                  sizeof(uint16_t) * npx * n, cudaMemcpyHostToDevice, st));
         }
+        // at most two batches compute at a time (measured: two concurrent batches fill each other's kernel
+        // tails, a third only adds contention), while the copies of all three streams overlap freely
+        if (rc == MVD_OK && k >= 2) rc = mvd_check(h, cudaStreamWaitEvent(st, h->ev_join[(k - 2) % mvd_handle::kSlots], 0));
         if (rc == MVD_OK) rc = run_core(h, h->ws_slot[s], h->d_in[s], lay, h->d_out[s], n, st);
+        if (rc == MVD_OK) rc = mvd_check(h, cudaEventRecord(h->ev_join[s], st));
         if (rc == MVD_OK)
             rc = mvd_check(h, cudaMemcpyAsync(host_out_f32 + (size_t)p0 * npx, h->d_out[s],
                                              sizeof(float) * npx * n, cudaMemcpyDeviceToHost, st));
