@@ -280,7 +280,7 @@ static int run_resident(mvd_handle* h, const uint16_t* views, ViewLayout lay, fl
     const size_t npx = (size_t)h->W * h->H;
     const int B = default_batch(h, n_planes);
     const int ns = std::min(h->resident_streams, mvd_handle::kSlots);
-    if (ns <= 1 || h->profiling || n_planes <= B) return run_core(h, h->ws_main, views, lay, out, n_planes, stream);
+    if (ns <= 1 || h->profiling || n_planes < 2 * B) return run_core(h, h->ws_main, views, lay, out, n_planes, stream);
     if (!h->ev_fork) MVD_TRY(h, cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
     for (int s = 0; s < ns; ++s) {
         if (!h->streams[s]) MVD_TRY(h, cudaStreamCreateWithFlags(&h->streams[s], cudaStreamNonBlocking));
@@ -331,6 +331,10 @@ static int default_batch(const mvd_handle* h, int n_planes) {
     const size_t per_plane = (size_t)h->W * h->H * sizeof(uint16_t) * h->V;
     size_t b = std::max<size_t>(1, ((size_t)64 << 20) / per_plane);
     b = std::min<size_t>(b, std::max(1, n_planes / 16));
+    // ... but never batches so small that a launch has nothing to chew on: at least ~2 Mvoxel
+    // (config 1's 8 planes of 64 x 64 stay one batch)
+    const size_t floor_planes = (((size_t)2 << 20) + (size_t)h->W * h->H - 1) / ((size_t)h->W * h->H);
+    b = std::max(b, floor_planes);
     b = std::max<size_t>(1, std::min<size_t>(b, (size_t)n_planes));
     return h->path == MVD_PATH_FFT ? even_up((int)b) : (int)b;
 }
