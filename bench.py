@@ -209,11 +209,11 @@ def algorithmic_work(cls, cfg, n_planes, K):
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
-# (profiles/r1_fft_v2_ncu_full.md), keyed by (config id, planes per launch, kernel class)
+# (profiles/r1_final_launches.md), keyed by (config id, planes per launch, kernel class)
 NCU_TRAFFIC = {
-    (2, 512, "fft_cols_otf"): 483.8e6,
-    (2, 512, "fft_rows_ratio"): 633.6e6,
-    (2, 512, "fft_rows_update"): 1032.7e6,
+    (2, 512, "fft_cols_otf"): 485.4e6,
+    (2, 512, "fft_rows_ratio"): 635.2e6,
+    (2, 512, "fft_rows_update"): 1032.5e6,
 }
 
 
@@ -324,7 +324,7 @@ def main():
                 if "hbm_gbs" in peaks else "fallback 6650 GB/s (of fallback)"}
     roof["traffic"] = NCU_TRAFFIC.get((cfg.cid, int(round(chunk_planes)), top)) if path_name == "fft" else None
     roof["algorithmic_bytes_per_launch" if wunit == "B" else "algorithmic_flop_per_launch"] = work
-    roof["traffic_source"] = "profiles/r1_fft_v2_ncu_full.md (ncu --set full, bytes per launch)" if roof["traffic"] else None
+    roof["traffic_source"] = "profiles/r1_final_launches.md (ncu --set full, bytes per launch)" if roof["traffic"] else None
     roof.update({"kernel": top, "launches_profiled": top_n, "avg_launch_us": avg_s * 1e6,
                  "share_of_step": top_ms / total_prof_ms, "planes_per_launch": chunk_planes,
                  "per_class_ms_per_step": {k: round(v[0] / prof_steps, 4) for k, v in prof.items() if v[1]}})
