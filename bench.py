@@ -238,6 +238,9 @@ def main():
     torch.cuda.set_device(local)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+        if local == 0:
+            build.build()              # one rank per node compiles; the others wait for the .so
+        dist.barrier()
     build.build()
 
     try:
