@@ -77,7 +77,7 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
     static_assert(NT % TPF == 0 && (TPF <= 32 ? 32 % TPF == 0 : TPF % 32 == 0), "teams are warp-aligned");
     static_assert(TPF % 16 == 0 && W % 16 == 0, "tile-major addressing assumes whole 16-element groups per team step");
     static_assert(TPF <= 32 || RP <= 15, "one named barrier per team");
-    static_assert(E % 4 == 0, "the landing copies split evenly over the team");
+    static_assert(E % 8 == 0 && TPF % 8 == 0, "the landing copies split evenly over the team");
     extern __shared__ __align__(16) float2 smem_rows2[];
     float2* tw = smem_rows2;                                  // [(S-1) E][TPF]
     float2* buf = smem_rows2 + (P::S - 1) * E * TPF;          // [RP][N]
@@ -94,15 +94,15 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
     float2* land = buf + team * W;                            // the team's region, used linearly as landing zone
     const int last_row = a.total_rows - 1;
 
-    // S is tile-major: 16-byte chunk q of image row `row` (elements 2q, 2q+1)
+    // S is tile-major: 16-byte chunk q = t + TPF k of image row `row` (elements 2q, 2q+1) sits in tile q / 8 at
+    // chunk q % 8 of the row's 128 bytes.  TPF is a multiple of 8, so the source address is LINEAR in k
+    // (one base + k * step): no per-chunk 64-bit offsets for the compiler to hoist and spill.
+    const size_t chunk_step = (size_t)(TPF / 8) * a.H * 16;
     auto issue_S = [&](int row) {
         const int pair = row / a.H, y = row % a.H;
-        const float2* src = a.S + (size_t)pair * npx + (size_t)y * 16;
+        const float2* src = a.S + (size_t)pair * npx + (size_t)y * 16 + (size_t)(t >> 3) * (a.H * 16) + 2 * (t & 7);
 #pragma unroll
-        for (int k = 0; k < E / 2; ++k) {
-            const int q = t + TPF * k;
-            cp_async16(land + 2 * q, src + (size_t)(q >> 3) * (a.H * 16) + 2 * (q & 7));
-        }
+        for (int k = 0; k < E / 2; ++k) cp_async16(land + 2 * (t + TPF * k), src + k * chunk_step);
         cp_async_commit();
     };
 
@@ -164,14 +164,15 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
             sync();
             fft_run_head<P, +1>(x, buf, tw, t, addr, sync);
             if (MODE == ROWS_RATIO) {
-                // phi rows of the two planes: W uint16 each, [0, W) plane a, [W, 2 W) plane b
+                // phi rows of the two planes: W uint16 each, [0, W) plane a, [W, 2 W) plane b;
+                // W / 8 chunks of 8 uint16 per plane, E / 8 of them per thread and plane
                 uint16_t* lu = reinterpret_cast<uint16_t*>(land);
+                const uint16_t* qa = vp + vxa + 8 * t;
+                const uint16_t* qb = vp + vxb + 8 * t;
 #pragma unroll
-                for (int k = 0; k < E / 4; ++k) {
-                    const int q = t + TPF * k;                   // chunk of 8 uint16; W / 8 chunks per plane
-                    const bool second = q >= W / 8;
-                    const int qq = second ? q - W / 8 : q;
-                    cp_async16(lu + 8 * q, vp + (second ? vxb : vxa) + 8 * qq);
+                for (int k = 0; k < E / 8; ++k) {
+                    cp_async16(lu + 8 * (t + TPF * k), qa + 8 * TPF * k);
+                    cp_async16(lu + W + 8 * (t + TPF * k), qb + 8 * TPF * k);
                 }
             } else {
 #pragma unroll
