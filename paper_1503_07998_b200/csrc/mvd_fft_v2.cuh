@@ -416,7 +416,8 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
                 w.y *= sgn;
                 x[e] = cmul(x[e], w);
             }
-            sync();                              // the out region is free for this item's results
+            // no barrier here: the inverse transform's exchanges (team barriers) lie between these
+            // reads of the out region and the next writes to it
         }
         fft_run_head<P, +1>(x, buf, tw, t, addr, sync);
         if (l == 0) {
@@ -424,7 +425,8 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
             if (OTF_REGS) bulk_wait_read();   // the previous item's results have left the out region
         }
         fft_run_tail<P, +1>(x, buf, tw, t, addr, sync);
-        sync();                          // ... and every thread of the team knows it
+        if (OTF_REGS) sync();            // ... and every thread of the team knows it (without OTF registers lane 0
+                                         // waited at the start of the item, many team barriers ago)
 #pragma unroll
         for (int e = 0; e < E; ++e) outz[(t + TPF * e) * CPT + c4] = x[e];
         fence_proxy_async();
