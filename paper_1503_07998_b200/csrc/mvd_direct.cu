@@ -273,7 +273,7 @@ int launch_corr(int mode, const mvd_handle* h, const float* src, const float* G,
                 float* dst, int n_planes, cudaStream_t st, size_t phi_plane, size_t phi_row) {
     // two planes per thread whenever the float2 tile fits in shared memory; K as a template
     // parameter for the config sizes
-    if (pair_smem_bytes(h->K, h->Kp) <= 227u * 1024u && getenv("MVD_DIRECT_SINGLE") == nullptr) {
+    if (h->direct_pair) {
 #define MVD_DIRECT_CASE(KT_, JC_)                                                                 \
     if (h->K == (KT_) && h->JC == (JC_))                                                          \
         return launch_pair2<KT_, JC_>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp,             \
@@ -350,6 +350,8 @@ int direct_setup(mvd_handle* h, const float* host_psfs, const float* host_xs) {
     host_psfs = pad_p.data();
     const float* host_back = pad_b.data();
     direct_choose_chunk(h->K, &h->JC, &h->Kp);
+    // two planes per thread whenever the float2 tile fits (MVD_DIRECT_SINGLE: measurement knob)
+    h->direct_pair = pair_smem_bytes(h->K, h->Kp) <= 227u * 1024u && getenv("MVD_DIRECT_SINGLE") == nullptr;
     const int K = h->K, Kp = h->Kp;
     const size_t per = (size_t)K * Kp;
     // shared memory needed by one CTA must fit the 227 KB limit

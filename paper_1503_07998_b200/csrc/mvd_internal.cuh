@@ -45,6 +45,7 @@ struct mvd_handle {
     float* d_coef = nullptr;
     int Kp = 0;   // padded number of PSF rows (multiple of the kernel's row chunk)
     int JC = 0;   // row chunk of the direct kernel chosen for K
+    bool direct_pair = false;   // the two-plane FFMA2 kernel serves this plan (its float2 tile fits in shared memory)
 
     // fft path: optical transfer functions, float2 [V][H][W], pre-scaled by 1/(W*H)
     float2* d_otf = nullptr;
