@@ -255,3 +255,35 @@ def test_profile_hooks_report_every_launch():
 def test_fp32_peak_microbenchmark_is_plausible():
     tf, mhz = binding.measure_fp32_peak()
     assert 20.0 < tf < 120.0 and 500.0 < mhz < 3000.0
+
+
+def test_config2_full_stack_in_the_bench_launch_configuration():
+    """The whole 512-plane stack exactly as bench.py times it (default batches dealt to two streams):
+    P12 on every plane (sum(psi) = sum(phi_last)), planes sampled from different batches bit-identical to
+    the same plane pair run on its own, and two sampled planes against the oracle."""
+    import importlib.util
+    import torch
+    spec = importlib.util.spec_from_file_location("bench", os.path.join(os.path.dirname(GOLDEN), "..", "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    cfg = synth.config(2)
+    psfs, views = bench.make_stack(cfg)
+    with binding.Mvd(cfg.W, cfg.H, cfg.V, psfs, cfg.K, cfg.T, cfg.eps) as m:
+        dv = torch.from_numpy(views.view(np.int16)).cuda()
+        do = torch.empty((cfg.N, cfg.H, cfg.W), dtype=torch.float32, device="cuda")
+        m.deconvolve_planes(dv, do, cfg.N)
+        torch.cuda.synchronize()
+        out = do.cpu().numpy()
+        assert np.isfinite(out).all() and (out >= 0).all()
+        np.testing.assert_allclose(out.astype(np.float64).sum(axis=(1, 2)),
+                                   views[-1].astype(np.float64).sum(axis=(1, 2)), rtol=2e-5)
+        for p0 in (0, 30, 32, 254, 300, 510):                       # pairs from different batches / streams
+            sub = np.ascontiguousarray(views[:, p0:p0 + 2])
+            ds = torch.from_numpy(sub.view(np.int16)).cuda()
+            d2 = torch.empty((2, cfg.H, cfg.W), dtype=torch.float32, device="cuda")
+            m.deconvolve_planes(ds, d2, 2)
+            torch.cuda.synchronize()
+            assert np.array_equal(d2.cpu().numpy(), out[p0:p0 + 2]), p0
+    sample = [1, 257]
+    ref = mvd_oracle.deconvolve(np.ascontiguousarray(views[:, sample]), psfs, cfg.T, cfg.eps)
+    assert_parity(out[sample], ref, "config2 full stack, sampled planes")
