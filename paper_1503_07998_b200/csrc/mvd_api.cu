@@ -371,11 +371,24 @@ static int host_pipeline(mvd_handle* h, const uint16_t* host_views_u16, float* h
     // Algorithm 1 with batches of planes instead of single planes and pinned
     // host memory instead of disk: batch k goes to stream k mod 3; within a stream H2D, the RL
     // steps and D2H are ordered, across streams they overlap.  Nothing blocks until the end.
+    // Batch sizes: B, with a ramp B/4, B/2 at both ends of a long stack so that the first H2D copy and the
+    // last D2H copy -- the only ones that overlap no compute -- are short (sizes stay even: plane pairs)
+    std::vector<int> sizes;
+    {
+        std::vector<int> ramp;
+        if (h->batch_planes == 0 && n_planes >= 8 * B && B >= 8) ramp = {(B / 4 + 1) & ~1, (B / 2 + 1) & ~1};
+        int left = n_planes;
+        for (int r : ramp) { sizes.push_back(r); left -= r; }
+        int tail = 0;
+        for (int r : ramp) tail += r;
+        while (left - tail > 0) { const int n = std::min(B, left - tail); sizes.push_back(n); left -= n; }
+        for (auto it = ramp.rbegin(); it != ramp.rend(); ++it) sizes.push_back(*it);
+    }
     int rc = MVD_OK;
-    int k = 0;
-    for (int p0 = 0; p0 < n_planes && rc == MVD_OK; p0 += B, ++k) {
+    int k = 0, p0 = 0;
+    for (size_t bi = 0; bi < sizes.size() && rc == MVD_OK; p0 += sizes[bi], ++bi, ++k) {
         const int s = k % mvd_handle::kSlots;
-        const int n = std::min(B, n_planes - p0);
+        const int n = sizes[bi];
         cudaStream_t st = h->streams[s];
         ViewLayout lay;
         if (camera_order) {
