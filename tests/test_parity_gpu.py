@@ -110,6 +110,8 @@ def test_large_configs_against_stored_oracle_planes(cid):
     (2, 1, 2048, 256, 7, 2, "random"),   # generation 2: 2048-point rows, a single plane
     (3, 5, 256, 256, 11, 2, "sparse"),   # generation 2: 256 x 256, three views
     (2, 2, 1024, 1024, 7, 1, "random"),  # generation 2: config 5's plane with an asymmetric PSF
+    (1, 2, 2048, 2048, 5, 1, "random"),  # the largest plane the FFT engine takes
+    (2, 3, 64, 32, 1, 3, "random"),      # psf_size 1: a scalar "PSF"
 ])
 def test_asymmetric_and_ragged(path, V, N, W, H, K, T, psf):
     _need(path, W, H, K)
