@@ -84,14 +84,29 @@ def make_stack(cfg, n_canonical=64):
 # clocks
 # ---------------------------------------------------------------------------------------------
 class ClockSampler:
+    """SM clock, power and throttle reasons sampled every ~10 ms through NVML (nvidia-ml-py) while the
+    timed region runs; falls back to `nvidia-smi -lms 100` when NVML cannot be loaded."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
 
     def __init__(self, index):
-        self.rows, self.proc, self.index = [], None, index
+        self.rows, self.proc, self.index, self.stop_flag, self.thread = [], None, index, False, None
 
     def start(self):
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            idx = int(vis.split(",")[self.index]) if vis and vis.split(",")[self.index].isdigit() else self.index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(idx)
+            self.nv = pynvml
+            self.thread = threading.Thread(target=self._poll, daemon=True)
+            self.thread.start()
+            return
+        except Exception:
+            self.nv = None
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
@@ -101,11 +116,37 @@ class ClockSampler:
         except OSError:
             self.proc = None
 
+    def _poll(self):
+        nv = self.nv
+        bits = [getattr(nv, n, 0) for n in ("nvmlClocksEventReasonHwSlowdown", "nvmlClocksEventReasonHwThermalSlowdown",
+                                            "nvmlClocksEventReasonSwThermalSlowdown", "nvmlClocksEventReasonSwPowerCap")]
+        legacy = [getattr(nv, n, 0) for n in ("nvmlClocksThrottleReasonHwSlowdown", "nvmlClocksThrottleReasonHwThermalSlowdown",
+                                              "nvmlClocksThrottleReasonSwThermalSlowdown", "nvmlClocksThrottleReasonSwPowerCap")]
+        bits = [b or l for b, l in zip(bits, legacy)]
+        try:
+            mx = nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM)
+        except Exception:
+            mx = 0
+        while not self.stop_flag:
+            try:
+                sm = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                pw = nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0
+                try:
+                    why = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h)
+                except Exception:
+                    why = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                self.rows.append((time.time(), [str(sm), str(mx), f"{pw:.2f}"] +
+                                  ["Active" if (why & b) else "Not Active" for b in bits]))
+            except Exception:
+                pass
+            time.sleep(0.01)
+
     def _read(self):
         for line in self.proc.stdout:
             self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
 
     def stop(self):
+        self.stop_flag = True
         if self.proc:
             self.proc.terminate()
             try:
@@ -113,17 +154,21 @@ class ClockSampler:
             except Exception:
                 self.proc.kill()
 
-    def summary(self, t0, t1):
-        rows = [r for t, r in self.rows if t0 - 0.05 <= t <= t1 + 0.15 and len(r) >= 7] or \
-               [r for _, r in self.rows if len(r) >= 7]
+    def summary(self, t0, t1, t_load0=None):
+        """Samples inside the timed region; a region too short for three samples also takes the
+        warm-up steps right before it (the same kernels under the same load)."""
+        rows = [r for t, r in self.rows if t0 - 0.005 <= t <= t1 + 0.005 and len(r) >= 7]
+        if len(rows) < 3 and t_load0 is not None:
+            rows = [r for t, r in self.rows if t_load0 <= t <= t1 + 0.15 and len(r) >= 7]
+        rows = rows or [r for _, r in self.rows if len(r) >= 7]
         if not rows:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         sm = [float(r[0]) for r in rows if r[0].replace(".", "").isdigit()]
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = [n for k, n in enumerate(names) if any(r[3 + k].lower().startswith("active") for r in rows)]
+        reasons = [n for k, n in enumerate(self.NAMES) if any(r[3 + k].lower().startswith("active") for r in rows)]
         pw = [float(r[2]) for r in rows if r[2].replace(".", "").isdigit()]
         return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": float(rows[0][1]),
-                "power_w_max": max(pw) if pw else None, "samples": len(rows), "reasons": reasons}
+                "power_w_max": max(pw) if pw else None, "samples": len(rows), "reasons": reasons,
+                "source": "nvml" if getattr(self, "nv", None) else "nvidia-smi"}
 
 
 # ---------------------------------------------------------------------------------------------
@@ -274,12 +319,13 @@ def main():
     path_name = binding.PATH_NAMES[m.path]
 
     # ---- device-resident: warm-up, then exactly K timed steps -------------------------------
-    for _ in range(max(args.warmup, 3)):
-        m.deconvolve_planes(dev_in, dev_out, N, stream)
-    barrier()
     sampler = ClockSampler(local)
     sampler.start()
     time.sleep(0.25)
+    t_load0 = time.time()
+    for _ in range(max(args.warmup, 3)):
+        m.deconvolve_planes(dev_in, dev_out, N, stream)
+    barrier()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     m.launch_count_reset()
     barrier()
@@ -292,7 +338,7 @@ def main():
     t_wall1 = time.time()
     launches = m.launch_count()
     ms = e0.elapsed_time(e1)
-    clocks = sampler.summary(t_wall0, t_wall1)
+    clocks = sampler.summary(t_wall0, t_wall1, t_load0)
     ms_max = shard.max_over_ranks(ms, device="cuda")          # device time of the slowest rank
     value = shard.job_throughput(units * args.steps, ms_max * 1e-3, world) / 1e6
 
