@@ -1,12 +1,14 @@
 #!/usr/bin/env python
 """bench.py -- deconvolved Mvoxel/s of the plane-wise multi-view RL hot path on B200.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 2] [--path auto|direct|fft]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--path auto|direct|fft]
     python bench.py --impl reference ...      # the fp64 CPU oracle, as it stands, on the host cores
 
 One "step" = one pass of the whole hot path (a0..a5: ingest, T iterations x V views of blur, ratio,
-back-projection, update) over one synthetic stack shaped like BASELINE.json's config (default:
-configs[1] = "config 2", 2 views x 512 planes of 512x256 uint16, 21x21 PSFs, 10 iterations).
+back-projection, update) over one synthetic stack shaped like a BASELINE.json config.  BASELINE.json's
+`metric` names no config, so the headline line is the LARGEST single-GPU workload, config 4 (2 views x
+2048 planes of 2048x800 uint16, 41x41 PSFs, 10 iterations: 13.4 GB in, 13.4 GB out), and the same JSON
+line carries `per_config`: value, e2e, roofline (every kernel class) and clocks of configs 1-5.
 
   value      device-resident throughput: inputs already in HBM, CUDA events on the launching stream
              around K calls of mvd_deconvolve_planes, max over ranks.
@@ -45,7 +47,9 @@ def parse():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-5); 2 = configs[1]")
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config number (1-5) of the headline line")
+    ap.add_argument("--per-config", default="1,2,3,4,5", help="configs reported in `per_config` (N = 1 only; '' = none)")
+    ap.add_argument("--per-config-steps", type=int, default=5, help="timed steps of the per_config entries")
     ap.add_argument("--planes", type=int, default=0, help="override the number of planes (0 = the config's)")
     ap.add_argument("--path", default="auto", choices=["auto", "direct", "fft"])
     ap.add_argument("--chunk", type=int, default=0, help="mvd_set_chunk_planes (0 = library default)")
@@ -212,24 +216,48 @@ def cpu_baseline(cfg, psfs, views, n_forced=0, target_s=15.0):
             "sample": f"first {n} of {N} planes, {Ts} of {T} iterations, one plane per thread"}
 
 
+def config_record(cfg, world=1):
+    """The workload-defining part of the JSON line's `config`, shared by both arms (the reference arm runs a
+    bounded sample of the SAME workload; the sample is described under `cpu_baseline.sample`)."""
+    in_b = cfg.V * cfg.N * cfg.H * cfg.W * 2
+    out_b = cfg.N * cfg.H * cfg.W * 4
+    return {"workload": cfg.name, "planes_per_gpu": cfg.N, "plane": f"{cfg.W}x{cfg.H}", "views": cfg.V,
+            "psf": cfg.K, "iterations": cfg.T,
+            "l2": ("inputs+outputs per step (%.0f MB) exceed the 126 MB L2; no flush" % ((in_b + out_b) / 1e6))
+                  if in_b + out_b > 126e6 else
+                  ("inputs+outputs per step (%.2f MB) fit the 126 MB L2; a 256 MB buffer is written between "
+                   "timed steps (flush)" % ((in_b + out_b) / 1e6)),
+            "parallelism": f"planes sharded over {world} GPU(s), no collective"}
+
+
 def run_reference(args, cfg):
+    """--impl reference: the oracle as it stands on the host cores, on the headline arm's config.  Each step is a
+    bounded sample of that workload (the first n planes, Ts of its T iterations, one plane per thread) sized
+    by a one-iteration pilot so that the whole --steps K --warmup W run ends within a few minutes; the
+    metric counts exactly the voxel-view-iterations the sample did."""
+    import dataclasses
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     from oracle import mvd_oracle
     from paper_1503_07998_b200 import synth
     cores = mvd_oracle.n_cores()
+    steps, warm = max(1, args.steps), max(0, args.warmup)
     n = args.cpu_planes or max(1, min(cfg.N, cores))
     psfs = synth.config_psfs(cfg.cid)
     views = synth.views(cfg, range(n), psfs)
-    steps, warm = max(1, args.steps), min(args.warmup, 1)
-    val, dt, used, cores = oracle_sample(cfg, psfs, views, n, steps=steps, warmup=warm)
-    sample = f"first {n} planes of the {cfg.N}-plane stack per step, one plane per thread"
+    _, t1, _, _ = oracle_sample(dataclasses.replace(cfg, T=1), psfs, views, n)            # pilot
+    per_step = 150.0 / (steps + warm)
+    Ts = int(max(1, min(cfg.T, per_step // max(t1, 1e-9))))   # one iteration of one plane per thread is the smallest sample
+    sub = dataclasses.replace(cfg, T=Ts)
+    val, dt, used, cores = oracle_sample(sub, psfs, views, n, steps=steps, warmup=warm)
+    sample = (f"per step: first {n} of {cfg.N} planes, {Ts} of {cfg.T} iterations, one plane per thread "
+              f"({n * cfg.W * cfg.H * cfg.V * Ts} voxel-view-iterations)")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus,
         "steps": steps, "warmup": warm, "ms_per_step": dt * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": cfg.name, "planes_per_step": n},
+        "config": config_record(cfg, max(1, args.gpus)),
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0}))
@@ -239,7 +267,7 @@ def run_reference(args, cfg):
 # ours
 # ---------------------------------------------------------------------------------------------
 def algorithmic_work(cls, cfg, n_planes, K):
-    """(amount per launch, unit) of one launch of kernel class `cls` over n_planes planes (DESIGN.md)."""
+    """(amount per launch, unit) of one launch of kernel class `cls` over n_planes planes (DESIGN.md 6)."""
     vox = n_planes * cfg.W * cfg.H
     table = {
         "init_mean": (vox * (2 * cfg.V + 4), "B"),
@@ -249,17 +277,176 @@ def algorithmic_work(cls, cfg, n_planes, K):
         "fft_cols_otf": (vox * 8, "B"),                            # spectrum in + out (OTF is L2-resident)
         "fft_rows_ratio": (vox * 10, "B"),                         # spectrum in, phi u16 in, spectrum out
         "fft_rows_update": (vox * 16, "B"),                        # spectrum in, psi in+out, spectrum out
+        "small_resident": (vox * (2 * cfg.V + 4), "B"),            # whole RL run on chip: views in, psi out
     }
     return table.get(cls, (0, "B"))
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
-# (profiles/r1_final_launches.md), keyed by (config id, planes per launch, kernel class)
-NCU_TRAFFIC = {
-    (2, 512, "fft_cols_otf"): 485.4e6,
-    (2, 512, "fft_rows_ratio"): 635.2e6,
-    (2, 512, "fft_rows_update"): 1032.5e6,
-}
+def passes_per_step(cls, cfg):
+    """Launches of class `cls` that one plane goes through in one step."""
+    return {"init_mean": 1, "fft_rows_first": 1, "small_resident": 1,
+            "fft_cols_otf": 2 * cfg.T * cfg.V}.get(cls, cfg.T * cfg.V)
+
+
+def load_traffic_table():
+    """profiles/ncu_traffic.csv: dram__bytes_read.sum + dram__bytes_write.sum per launch of each kernel class
+    from the committed `ncu --set full` captures (one row per config and class, with its source file)."""
+    import csv
+    table = {}
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.csv")) as f:
+            for row in csv.DictReader(r for r in f if not r.startswith("#")):
+                table[(int(row["config"]), row["kernel_class"])] = (
+                    float(row["dram_bytes_per_launch"]), float(row["planes_per_launch"]), row["source"])
+    except OSError:
+        pass
+    return table
+
+
+def make_roofline(prof, prof_steps, cfg, N, K, path_name, peaks, traffic_table, fp32_peak):
+    """`roofline` of the dominant kernel class plus the same figures for every class (`per_class`)."""
+    fp32_tf, fp32_mhz = fp32_peak
+    hbm = float(peaks.get("hbm_gbs", 6650.0))
+    hbm_src = "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (of fallback)"
+    total_ms = sum(v[0] for v in prof.values()) or 1.0
+    per_class = {}
+    for cls, (ms, n) in prof.items():
+        if not n or cls == "setup":
+            continue
+        launches_per_step = max(n // prof_steps, 1)
+        planes = N * passes_per_step(cls, cfg) / launches_per_step          # mean planes per launch
+        work, wunit = algorithmic_work(cls, cfg, planes, K)
+        avg_s = ms * 1e-3 / n
+        rec = {"ms_per_step": round(ms / prof_steps, 4), "launches_per_step": launches_per_step,
+               "avg_launch_us": avg_s * 1e6, "planes_per_launch": planes, "share_of_step": ms / total_ms}
+        if wunit == "flop":
+            rec.update(bound="alu", achieved=work / avg_s / 1e12, peak=fp32_tf, unit="TFLOP/s",
+                       algorithmic_flop_per_launch=work)
+        else:
+            rec.update(bound="hbm", achieved=work / avg_s / 1e9, peak=hbm, unit="GB/s",
+                       algorithmic_bytes_per_launch=work)
+        rec["frac"] = rec["achieved"] / rec["peak"] if rec["peak"] else None
+        t = traffic_table.get((cfg.cid, cls)) if path_name == "fft" else None
+        rec["traffic"] = t[0] * planes / t[1] if t else None
+        if t:
+            rec["traffic_source"] = f"{t[2]} (ncu --set full; bytes per launch of {t[1]:g} planes, scaled to {planes:g})"
+            rec["frac_of_traffic"] = rec["traffic"] / avg_s / 1e9 / hbm
+        per_class[cls] = rec
+    top = max(per_class, key=lambda k: per_class[k]["share_of_step"])
+    roof = dict(per_class[top])
+    roof["kernel"] = top
+    roof["peak_source"] = hbm_src if roof["bound"] == "hbm" else (
+        f"measured FFMA micro-kernel in this run at {fp32_mhz:.0f} MHz (nominal 148 SM x 128 lanes x 2 x 1.965 GHz = 74.4)")
+    roof["launches_profiled"] = prof[top][1]
+    roof["per_class"] = {k: {kk: vv for kk, vv in v.items() if kk != "traffic_source"} for k, v in per_class.items()}
+    return roof
+
+
+def run_config(cfg, args, steps, warmup, world, local, peaks, traffic_table, fp32_peak, do_e2e=True):
+    """One config on this rank's GPU: device-resident value, e2e through the host pipeline, per-class
+    roofline, clocks.  Returns a dict (times are this rank's; the caller reduces over ranks)."""
+    import torch
+    from paper_1503_07998_b200 import binding, shard
+    psfs, views = make_stack(cfg)
+    V, N, H, W, K, T = cfg.V, cfg.N, cfg.H, cfg.W, cfg.K, cfg.T
+    units = cfg.units
+    path = {"auto": None, "direct": binding.PATH_DIRECT, "fft": binding.PATH_FFT}[args.path]
+    host_in = torch.from_numpy(views.view(np.int16)).pin_memory()
+    host_out = torch.empty((N, H, W), dtype=torch.float32).pin_memory()
+    dev_in = host_in.cuda()
+    dev_out = torch.empty((N, H, W), dtype=torch.float32, device="cuda")
+    stream = torch.cuda.Stream()
+    small = views.nbytes + N * H * W * 4 <= 126e6           # fits L2: flush between timed steps
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda") if small else None
+
+    def barrier():
+        import torch.distributed as dist
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    m = binding.Mvd(W, H, V, psfs, K, T, cfg.eps, path)
+    if args.chunk:
+        m.set_chunk_planes(args.chunk)
+    if args.batch:
+        m.set_batch_planes(args.batch)
+    if args.streams:
+        m.set_resident_streams(args.streams)
+    m.reserve(N)
+    path_name = binding.PATH_NAMES[m.path]
+
+    # ---- device-resident: warm-up, then exactly `steps` timed steps ---------------------------
+    sampler = ClockSampler(local)
+    sampler.start()
+    time.sleep(0.25)
+    t_load0 = time.time()
+    for _ in range(max(warmup, 3)):
+        m.deconvolve_planes(dev_in, dev_out, N, stream)
+    barrier()
+    m.launch_count_reset()
+    t_wall0 = time.time()
+    if small:
+        # steps are timed one by one (CUDA events on the launching stream) with an L2 flush in between
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for e0, e1 in evs:
+            with torch.cuda.stream(stream):
+                flush.fill_(1)
+            e0.record(stream)
+            m.deconvolve_planes(dev_in, dev_out, N, stream)
+            e1.record(stream)
+        barrier()
+        ms = sum(e0.elapsed_time(e1) for e0, e1 in evs)
+    else:
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(stream)
+        for _ in range(steps):
+            m.deconvolve_planes(dev_in, dev_out, N, stream)
+        e1.record(stream)
+        barrier()
+        ms = e0.elapsed_time(e1)
+    t_wall1 = time.time()
+    launches = m.launch_count()
+    clocks = sampler.summary(t_wall0, t_wall1, t_load0)
+    ms_max = shard.max_over_ranks(ms, device="cuda")          # device time of the slowest rank
+    value = shard.job_throughput(units * steps, ms_max * 1e-3, world) / 1e6
+
+    # ---- per-kernel durations (CUDA events inside the library, launching stream) ------------
+    m.profile_enable(True)
+    prof_steps = 2
+    for _ in range(prof_steps):
+        m.deconvolve_planes(dev_in, dev_out, N, stream)
+    prof = m.profile_read()
+    m.profile_enable(False)
+    torch.cuda.synchronize()
+    roof = make_roofline(prof, prof_steps, cfg, N, K, path_name, peaks, traffic_table, fp32_peak)
+
+    # ---- end to end: pinned host -> host through mvd_deconvolve_host -------------------------
+    e2e = None
+    if do_e2e:
+        m.deconvolve_planes(dev_in, dev_out, N, stream)      # the profiled steps ran single-stream: same bits, but redo
+        for _ in range(max(1, min(warmup, 2))):
+            m.deconvolve_host(host_in, host_out, N)
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(steps):
+            m.deconvolve_host(host_in, host_out, N)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        dt = shard.max_over_ranks(dt, device="cuda")
+        e2e = {"value": shard.job_throughput(units * steps, dt, world) / 1e6, "unit": UNIT,
+               "h2d_bytes_per_step": int(views.nbytes), "d2h_bytes_per_step": int(host_out.numel() * 4),
+               "ms_per_step": dt * 1e3 / steps}
+        e2e["ratio_to_device_resident"] = e2e["value"] / value
+        same = True
+        for p0 in range(0, N, 256):                          # compare in slices: no second 13 GB host copy
+            same = same and bool(torch.equal(host_out[p0:p0 + 256], dev_out[p0:p0 + 256].cpu()))
+        e2e["bit_identical_to_device_resident"] = same
+    sampler.stop()
+    m.destroy()
+    rec = {"value": value, "ms_per_step": ms_max / steps, "steps": steps, "e2e": e2e, "roofline": roof,
+           "clocks": clocks, "gpu_launches": launches, "path": path_name,
+           "whole_step_algorithmic_GBps": (42.0 if path_name == "fft" else 22.0) * units / (ms_max / steps * 1e-3) / 1e9}
+    return rec, psfs, views
 
 
 def main():
@@ -273,7 +460,7 @@ def main():
 
     import torch
     import torch.distributed as dist
-    from paper_1503_07998_b200 import binding, build, shard
+    from paper_1503_07998_b200 import binding, build
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
     rank = int(os.environ.get("RANK", "0"))
@@ -293,128 +480,43 @@ def main():
             peaks = json.load(f)
     except OSError:
         peaks = {}
-    psfs, views = make_stack(cfg)
-    V, N, H, W, K, T = cfg.V, cfg.N, cfg.H, cfg.W, cfg.K, cfg.T
-    units = cfg.units                                     # voxel-view-iterations per step per rank
-    path = {"auto": None, "direct": binding.PATH_DIRECT, "fft": binding.PATH_FFT}[args.path]
+    traffic_table = load_traffic_table()
+    fp32_peak = binding.measure_fp32_peak()
 
-    host_in = torch.from_numpy(views.view(np.int16)).pin_memory()
-    host_out = torch.empty((N, H, W), dtype=torch.float32).pin_memory()
-    dev_in = host_in.cuda()
-    dev_out = torch.empty((N, H, W), dtype=torch.float32, device="cuda")
-    stream = torch.cuda.Stream()
-
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    m = binding.Mvd(W, H, V, psfs, K, T, cfg.eps, path)
-    if args.chunk:
-        m.set_chunk_planes(args.chunk)
-    if args.batch:
-        m.set_batch_planes(args.batch)
-    if args.streams:
-        m.set_resident_streams(args.streams)
-    path_name = binding.PATH_NAMES[m.path]
-
-    # ---- device-resident: warm-up, then exactly K timed steps -------------------------------
-    sampler = ClockSampler(local)
-    sampler.start()
-    time.sleep(0.25)
-    t_load0 = time.time()
-    for _ in range(max(args.warmup, 3)):
-        m.deconvolve_planes(dev_in, dev_out, N, stream)
-    barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    m.launch_count_reset()
-    barrier()
-    t_wall0 = time.time()
-    e0.record(stream)
-    for _ in range(args.steps):
-        m.deconvolve_planes(dev_in, dev_out, N, stream)
-    e1.record(stream)
-    barrier()
-    t_wall1 = time.time()
-    launches = m.launch_count()
-    ms = e0.elapsed_time(e1)
-    clocks = sampler.summary(t_wall0, t_wall1, t_load0)
-    ms_max = shard.max_over_ranks(ms, device="cuda")          # device time of the slowest rank
-    value = shard.job_throughput(units * args.steps, ms_max * 1e-3, world) / 1e6
-
-    # ---- per-kernel durations (CUDA events inside the library, launching stream) ------------
-    m.profile_enable(True)
-    prof_steps = 2
-    for _ in range(prof_steps):
-        m.deconvolve_planes(dev_in, dev_out, N, stream)
-    prof = m.profile_read()
-    m.profile_enable(False)
-    torch.cuda.synchronize()
-    total_prof_ms = sum(v[0] for v in prof.values()) or 1.0
-    top = max(prof, key=lambda k: prof[k][0])
-    top_ms, top_n = prof[top]
-    passes = {"init_mean": 1, "fft_rows_first": 1, "fft_cols_otf": 2 * T * V}.get(top, T * V)   # per plane per step
-    launches_per_step = max(top_n // prof_steps, 1)
-    chunk_planes = N * passes / launches_per_step                      # mean planes per launch
-    work, wunit = algorithmic_work(top, cfg, chunk_planes, K)
-    avg_s = top_ms * 1e-3 / max(top_n, 1)
-    fp32_tf, fp32_mhz = binding.measure_fp32_peak()
-    if wunit == "flop":
-        achieved = work / avg_s / 1e12
-        roof = {"bound": "alu", "achieved": achieved, "peak": fp32_tf, "unit": "TFLOP/s",
-                "frac": achieved / fp32_tf, "traffic": None,
-                "peak_source": f"measured FFMA micro-kernel in this run at {fp32_mhz:.0f} MHz "
-                               f"(nominal 148 SM x 128 lanes x 2 x 1.965 GHz = 74.4)"}
-    else:
-        achieved = work / avg_s / 1e9
-        peak = float(peaks.get("hbm_gbs", 6650.0))
-        roof = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": None, "peak_source": "MEASURED_PEAKS.json hbm_gbs (of measured)"
-                if "hbm_gbs" in peaks else "fallback 6650 GB/s (of fallback)"}
-    roof["traffic"] = NCU_TRAFFIC.get((cfg.cid, int(round(chunk_planes)), top)) if path_name == "fft" else None
-    roof["algorithmic_bytes_per_launch" if wunit == "B" else "algorithmic_flop_per_launch"] = work
-    roof["traffic_source"] = "profiles/r1_final_launches.md (ncu --set full, bytes per launch)" if roof["traffic"] else None
-    roof.update({"kernel": top, "launches_profiled": top_n, "avg_launch_us": avg_s * 1e6,
-                 "share_of_step": top_ms / total_prof_ms, "planes_per_launch": chunk_planes,
-                 "per_class_ms_per_step": {k: round(v[0] / prof_steps, 4) for k, v in prof.items() if v[1]}})
-
-    # ---- end to end: pinned host -> host through mvd_deconvolve_host -------------------------
-    e2e = None
-    if not args.no_e2e:
-        for _ in range(max(1, min(args.warmup, 2))):
-            m.deconvolve_host(host_in, host_out, N)
-        barrier()
-        t0 = time.perf_counter()
-        for _ in range(args.steps):
-            m.deconvolve_host(host_in, host_out, N)
-        torch.cuda.synchronize()
-        dt = time.perf_counter() - t0
-        dt = shard.max_over_ranks(dt, device="cuda")
-        e2e = {"value": shard.job_throughput(units * args.steps, dt, world) / 1e6, "unit": UNIT,
-               "h2d_bytes_per_step": int(views.nbytes), "d2h_bytes_per_step": int(host_out.numel() * 4),
-               "ms_per_step": dt * 1e3 / args.steps, "ratio_to_device_resident": None}
-        e2e["ratio_to_device_resident"] = e2e["value"] / value
-        same = bool(torch.equal(host_out, dev_out.cpu()))
-        e2e["bit_identical_to_device_resident"] = same
-    sampler.stop()
+    main_rec, psfs, views = run_config(cfg, args, args.steps, args.warmup, world, local, peaks, traffic_table,
+                                       fp32_peak, do_e2e=not args.no_e2e)
 
     # ---- the oracle beside it (rank 0, N = 1 only): a bounded sample of about 10-30 s of CPU work ----
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu:
         cpu = cpu_baseline(cfg, psfs, views, args.cpu_planes)
-    m.destroy()
+    del psfs, views
+
+    # ---- every config, shorter (N = 1 only): value, e2e, per-class roofline, clocks ---------------
+    per_config = None
+    if world == 1 and args.per_config and not args.planes:
+        per_config = []
+        for cid in [int(c) for c in args.per_config.split(",") if c]:
+            if cid == cfg.cid:
+                rec = dict(main_rec)
+            else:
+                c2 = synth.config(cid)
+                rec, _, _ = run_config(c2, args, max(1, args.per_config_steps), 3, world, local, peaks,
+                                       traffic_table, fp32_peak, do_e2e=not args.no_e2e)
+            rec = {"config": cid, **config_record(synth.config(cid), world), **rec}
+            per_config.append(rec)
 
     if rank == 0:
+        conf = config_record(cfg, world)
+        conf["path"] = main_rec["path"]
         print(json.dumps({
-            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+            "metric": METRIC, "value": main_rec["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": main_rec["ms_per_step"], "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": cfg.name, "planes_per_gpu": N, "path": path_name,
-                       "l2": "inputs+outputs per step (%.0f MB) exceed the 126 MB L2; no flush" %
-                             ((views.nbytes + N * H * W * 4) / 1e6),
-                       "parallelism": f"planes sharded over {world} GPU(s), no collective"},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "cpu_baseline": cpu,
-            "fp32_peak_measured_tflops": fp32_tf,
+            "config": conf, "clocks": main_rec["clocks"], "e2e": main_rec["e2e"],
+            "gpu_launches": main_rec["gpu_launches"], "roofline": main_rec["roofline"], "cpu_baseline": cpu,
+            "whole_step_algorithmic_GBps": main_rec["whole_step_algorithmic_GBps"],
+            "fp32_peak_measured_tflops": fp32_peak[0], "per_config": per_config,
             "context": "paper Table 1 (other hardware, FFT implementation, whole workflow): 1128 Mvoxel/s "
                        "at 2048^3 on a GTX Titan Black; plane-wise speedups up to 25x / 75x over 3D "
                        "deconvolution with / without GPU (PAPER.md:31, :164-175)"}))

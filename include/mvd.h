@@ -114,8 +114,9 @@ MVD_API int mvd_build_backprojectors(int variant, int n_views, const float* psfs
  *   dev_views_u16  DEVICE, uint16 [n_views][n_planes][plane_h][plane_w]; read-only.
  *   dev_out_f32    DEVICE, float  [n_planes][plane_h][plane_w]; fully overwritten; must not alias the input.
  *   stream         a cudaStream_t (NULL = legacy default stream).  The call ENQUEUES and returns; it does
- *                  not synchronise.  Calls on one handle must all be ordered on one stream (scratch is
- *                  per handle, grown at first use and kept until mvd_destroy).
+ *                  not synchronise -- except that scratch is per handle and grown on demand: a call that needs
+ *                  more than is reserved allocates first (see mvd_reserve).  Calls on one handle must all be
+ *                  ordered on one stream.
  * n_planes == 0 is a no-op.  Errors: MVD_ERR_INVALID, MVD_ERR_CUDA, MVD_ERR_NOMEM.
  */
 MVD_API int mvd_deconvolve_planes(mvd_handle* h, const uint16_t* dev_views_u16, float* dev_out_f32,
@@ -151,6 +152,19 @@ MVD_API int mvd_deconvolve_planes_strided(mvd_handle* h, const uint16_t* dev_vie
  */
 MVD_API int mvd_deconvolve_host_camera(mvd_handle* h, const uint16_t* host_frames_u16, float* host_out_f32,
                                int n_planes);
+
+/*
+ * mvd_reserve -- size everything a later call on up to max_planes planes needs (scratch of the engine, the
+ * internal streams and events, the pipeline's device slots) now.  After it, mvd_deconvolve_planes* with
+ * n_planes <= max_planes only enqueues: no allocation, no synchronisation, so the call can be captured into a
+ * CUDA graph (stream capture on `stream`).  Without it the first call (and any call that needs more scratch
+ * than an earlier one) allocates, which synchronises the device.  Errors: MVD_ERR_INVALID, MVD_ERR_NOMEM.
+ */
+MVD_API int mvd_reserve(mvd_handle* h, int max_planes);
+
+/* Planes per batch that mvd_deconvolve_host / the forked device-resident path use for a stack of n_planes
+ * (the default policy, or mvd_set_batch_planes); batches start at multiples of it. */
+MVD_API int mvd_get_batch_planes(const mvd_handle* h, int n_planes);
 
 /* Frees the plan, its scratch, its streams and staging buffers.  NULL is a no-op. */
 MVD_API void mvd_destroy(mvd_handle* h);

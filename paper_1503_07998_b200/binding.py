@@ -37,6 +37,8 @@ SIGNATURES = {
     "mvd_last_cuda_error": (_i, [_vp]),
     "mvd_get_path": (_i, [_vp]),
     "mvd_path_supported": (_i, [_i, _i, _i, _i]),
+    "mvd_reserve": (_i, [_vp, _i]),
+    "mvd_get_batch_planes": (_i, [_vp, _i]),
     "mvd_set_chunk_planes": (_i, [_vp, _i]),
     "mvd_set_batch_planes": (_i, [_vp, _i]),
     "mvd_set_resident_streams": (_i, [_vp, _i]),
@@ -161,6 +163,15 @@ class Mvd:
     @property
     def path(self) -> int:
         return lib().mvd_get_path(self._h)
+
+    def reserve(self, max_planes: int) -> None:
+        self._raise(lib().mvd_reserve(self._h, max_planes), "mvd_reserve")
+
+    def get_batch_planes(self, n_planes: int) -> int:
+        rc = lib().mvd_get_batch_planes(self._h, n_planes)
+        if rc < 0:
+            self._raise(rc, "mvd_get_batch_planes")
+        return rc
 
     def set_chunk_planes(self, planes: int) -> None:
         self._raise(lib().mvd_set_chunk_planes(self._h, planes), "mvd_set_chunk_planes")

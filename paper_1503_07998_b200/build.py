@@ -20,7 +20,7 @@ _STAMP = os.path.join(_HERE, "csrc", ".build_stamp")
 SOURCES = ["mvd_api.cu", "mvd_direct.cu", "mvd_fft.cu", "mvd_fft_inst_small.cu", "mvd_fft_inst_mid.cu",
            "mvd_fft_inst_large.cu", "mvd_fft_inst_v2.cu", "mvd_peak.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-              "--use_fast_math=false", "-Xcompiler", "-fPIC,-O2,-fvisibility=hidden",
+              "-Xcompiler", "-fPIC,-O2,-fvisibility=hidden",
               "-Xptxas", "-v", "-shared", "-cudart", "static"]
 
 
@@ -49,7 +49,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         with open(_STAMP) as f:
             if f.read().strip() == dig:
                 return LIB
-    flags = [f for f in NVCC_FLAGS if f != "--use_fast_math=false"]
+    flags = list(NVCC_FLAGS)
     objs = []
     procs = []
     for src in SOURCES:

@@ -274,6 +274,64 @@ static int run_core(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLay
 
 static int default_batch(const mvd_handle* h, int n_planes);
 
+// Streams and events of the host pipeline / the forked device-resident batches, created once.
+static int ensure_streams(mvd_handle* h) {
+    if (!h->ev_fork) MVD_TRY(h, cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+    for (int s = 0; s < mvd_handle::kSlots; ++s) {
+        if (!h->streams[s]) MVD_TRY(h, cudaStreamCreateWithFlags(&h->streams[s], cudaStreamNonBlocking));
+        if (!h->ev_join[s]) MVD_TRY(h, cudaEventCreateWithFlags(&h->ev_join[s], cudaEventDisableTiming));
+    }
+    return MVD_OK;
+}
+
+// Scratch of one workspace that runs n planes at a time (FFT: Z and S, 8 B per voxel each; direct: r).
+static void scratch_bytes(const mvd_handle* h, int n, size_t* a, size_t* b) {
+    const size_t npx = (size_t)h->W * h->H;
+    if (h->path == MVD_PATH_FFT) {
+        *a = *b = sizeof(float2) * (size_t)((n + 1) / 2) * npx;
+    } else {
+        *a = h->T > 0 ? sizeof(float) * (size_t)n * npx : 0;
+        *b = 0;
+    }
+}
+
+// Pipeline slots (uint16 in, fp32 out) for batches of B planes.
+static int reserve_slots(mvd_handle* h, int B) {
+    if ((size_t)B <= h->slot_planes) return MVD_OK;
+    const size_t npx = (size_t)h->W * h->H;
+    MVD_TRY(h, cudaDeviceSynchronize());
+    for (int s = 0; s < mvd_handle::kSlots; ++s) {
+        if (h->d_in[s]) { cudaFree(h->d_in[s]); h->d_in[s] = nullptr; }
+        if (h->d_out[s]) { cudaFree(h->d_out[s]); h->d_out[s] = nullptr; }
+    }
+    h->slot_planes = 0;
+    for (int s = 0; s < mvd_handle::kSlots; ++s) {
+        MVD_TRY(h, cudaMalloc((void**)&h->d_in[s], sizeof(uint16_t) * npx * B * h->V));
+        MVD_TRY(h, cudaMalloc((void**)&h->d_out[s], sizeof(float) * npx * B));
+    }
+    h->slot_planes = (size_t)B;
+    return MVD_OK;
+}
+
+int mvd_reserve(mvd_handle* h, int max_planes) {
+    if (!h || max_planes < 1) return MVD_ERR_INVALID;
+    int rc = ensure_streams(h);
+    if (rc != MVD_OK) return rc;
+    const int B = default_batch(h, max_planes), chunk = default_chunk(h);
+    size_t a, b;
+    scratch_bytes(h, std::min(chunk, max_planes), &a, &b);
+    if ((rc = ws_reserve(h, h->ws_main, a, b)) != MVD_OK) return rc;
+    scratch_bytes(h, std::min(chunk, B), &a, &b);
+    for (int s = 0; s < mvd_handle::kSlots; ++s)
+        if ((rc = ws_reserve(h, h->ws_slot[s], a, b)) != MVD_OK) return rc;
+    return reserve_slots(h, B);
+}
+
+int mvd_get_batch_planes(const mvd_handle* h, int n_planes) {
+    if (!h || n_planes < 1) return MVD_ERR_INVALID;
+    return default_batch(h, n_planes);
+}
+
 // Device-resident work on `lay`: one stream, or batches dealt round-robin to internal streams that fork
 // from and join the caller's stream (planes are independent; results do not depend on the split).
 static int run_resident(mvd_handle* h, const uint16_t* views, ViewLayout lay, float* out, int n_planes,
@@ -282,14 +340,16 @@ static int run_resident(mvd_handle* h, const uint16_t* views, ViewLayout lay, fl
     const int B = default_batch(h, n_planes);
     const int ns = std::min(h->resident_streams, mvd_handle::kSlots);
     if (ns <= 1 || h->profiling || n_planes < 2 * B) return run_core(h, h->ws_main, views, lay, out, n_planes, stream);
-    if (!h->ev_fork) MVD_TRY(h, cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
-    for (int s = 0; s < ns; ++s) {
-        if (!h->streams[s]) MVD_TRY(h, cudaStreamCreateWithFlags(&h->streams[s], cudaStreamNonBlocking));
-        if (!h->ev_join[s]) MVD_TRY(h, cudaEventCreateWithFlags(&h->ev_join[s], cudaEventDisableTiming));
+    int rc = ensure_streams(h);
+    {
+        size_t a, b;
+        scratch_bytes(h, std::min(default_chunk(h), B), &a, &b);
+        for (int s = 0; s < ns && rc == MVD_OK; ++s) rc = ws_reserve(h, h->ws_slot[s], a, b);
     }
+    if (rc != MVD_OK) return rc;
     MVD_TRY(h, cudaEventRecord(h->ev_fork, stream));
     for (int s = 0; s < ns; ++s) MVD_TRY(h, cudaStreamWaitEvent(h->streams[s], h->ev_fork, 0));
-    int rc = MVD_OK, k = 0;
+    int k = 0;
     for (int p0 = 0; p0 < n_planes && rc == MVD_OK; p0 += B, ++k) {
         const int s = k % ns;
         rc = run_core(h, h->ws_slot[s], views + (size_t)p0 * lay.plane, lay, out + (size_t)p0 * npx,
@@ -351,22 +411,13 @@ static int host_pipeline(mvd_handle* h, const uint16_t* host_views_u16, float* h
     const size_t npx = (size_t)h->W * h->H;
     const int B = default_batch(h, n_planes);
 
-    for (int s = 0; s < mvd_handle::kSlots; ++s) {
-        if (!h->streams[s]) MVD_TRY(h, cudaStreamCreateWithFlags(&h->streams[s], cudaStreamNonBlocking));
-        if (!h->ev_join[s]) MVD_TRY(h, cudaEventCreateWithFlags(&h->ev_join[s], cudaEventDisableTiming));
-    }
-    if ((size_t)B > h->slot_planes) {
-        MVD_TRY(h, cudaDeviceSynchronize());
-        for (int s = 0; s < mvd_handle::kSlots; ++s) {
-            if (h->d_in[s]) { cudaFree(h->d_in[s]); h->d_in[s] = nullptr; }
-            if (h->d_out[s]) { cudaFree(h->d_out[s]); h->d_out[s] = nullptr; }
-        }
-        h->slot_planes = 0;
-        for (int s = 0; s < mvd_handle::kSlots; ++s) {
-            MVD_TRY(h, cudaMalloc((void**)&h->d_in[s], sizeof(uint16_t) * npx * B * h->V));
-            MVD_TRY(h, cudaMalloc((void**)&h->d_out[s], sizeof(float) * npx * B));
-        }
-        h->slot_planes = (size_t)B;
+    {   // everything the batches need is sized before the first copy is enqueued: nothing below allocates
+        int rc0 = ensure_streams(h);
+        if (rc0 == MVD_OK) rc0 = reserve_slots(h, B);
+        size_t a, b;
+        scratch_bytes(h, std::min(default_chunk(h), B), &a, &b);
+        for (int s = 0; s < mvd_handle::kSlots && rc0 == MVD_OK; ++s) rc0 = ws_reserve(h, h->ws_slot[s], a, b);
+        if (rc0 != MVD_OK) return rc0;
     }
 
     // Algorithm 1 with batches of planes instead of single planes and pinned
@@ -374,16 +425,25 @@ static int host_pipeline(mvd_handle* h, const uint16_t* host_views_u16, float* h
     // steps and D2H are ordered, across streams they overlap.  Nothing blocks until the end.
     // Batch sizes: B, with a ramp B/4, B/2 at both ends of a long stack so that the first H2D copy and the
     // last D2H copy -- the only ones that overlap no compute -- are short (sizes stay even: plane pairs)
+    // Every batch except the very last holds an EVEN number of planes: the FFT engine pairs planes (2m, 2m+1)
+    // counted from the start of its batch, so a batch that started on an odd plane would pair differently
+    // from mvd_deconvolve_planes and the output bits would differ.  An odd stack is split as if it had one
+    // plane less and the last plane joins the last batch (or forms a batch of its own when that one is full).
     std::vector<int> sizes;
     {
         std::vector<int> ramp;
-        if (h->batch_planes == 0 && n_planes >= 8 * B && B >= 8) ramp = {(B / 4 + 1) & ~1, (B / 2 + 1) & ~1};
-        int left = n_planes;
+        const int n_even = n_planes & ~1;
+        if (h->batch_planes == 0 && n_even >= 8 * B && B >= 8) ramp = {(B / 4 + 1) & ~1, (B / 2 + 1) & ~1};
+        int left = n_even;
         for (int r : ramp) { sizes.push_back(r); left -= r; }
         int tail = 0;
         for (int r : ramp) tail += r;
         while (left - tail > 0) { const int n = std::min(B, left - tail); sizes.push_back(n); left -= n; }
         for (auto it = ramp.rbegin(); it != ramp.rend(); ++it) sizes.push_back(*it);
+        if (n_planes & 1) {
+            if (!sizes.empty() && sizes.back() < B) sizes.back() += 1;
+            else sizes.push_back(1);
+        }
     }
     int rc = MVD_OK;
     int k = 0, p0 = 0;

@@ -11,8 +11,6 @@
 // registers: for one PSF column i it reads a (RY+JC-1)-tall window of the staged column (one
 // conflict-free LDS per value, lanes along x) and issues JC*RY FFMAs on it.  The FP32 FMA pipe is
 // the bound (4 K^2 flop against 22 B of HBM traffic per voxel-view-iteration).
-#include <stdlib.h>
-
 #include "mvd_internal.cuh"
 
 namespace {
@@ -231,15 +229,23 @@ int launch_pair2(int mode, const float* src, const float* G, const uint16_t* phi
     if (grid > 0x7fffffffLL) return (int)cudaErrorInvalidConfiguration;
     dim3 block(BX, BY);
     cudaError_t e;
+    // the opt-in to > 48 KB of dynamic shared memory is raised once per kernel and size (not per launch)
+    static size_t opted[2] = {0, 0};
     if (mode == 0) {
         auto k = direct_corr2_kernel<KT, JC, 0>;
-        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return (int)e;
+        if (smem > opted[0]) {
+            e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return (int)e;
+            opted[0] = smem;
+        }
         k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row, n_planes);
     } else {
         auto k = direct_corr2_kernel<KT, JC, 1>;
-        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return (int)e;
+        if (smem > opted[1]) {
+            e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return (int)e;
+            opted[1] = smem;
+        }
         k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row, n_planes);
     }
     return (int)cudaGetLastError();
@@ -255,15 +261,22 @@ int launch_pair_member(int mode, const float* src, const float* G, const uint16_
     if (grid > 0x7fffffffLL) return (int)cudaErrorInvalidConfiguration;
     dim3 block(BX, BY);
     cudaError_t e;
+    static size_t opted[2] = {0, 0};
     if (mode == 0) {
         auto k = direct_corr_kernel<KT, JC, 0>;
-        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return (int)e;
+        if (smem > opted[0]) {
+            e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return (int)e;
+            opted[0] = smem;
+        }
         k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row);
     } else {
         auto k = direct_corr_kernel<KT, JC, 1>;
-        e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return (int)e;
+        if (smem > opted[1]) {
+            e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+            if (e != cudaSuccess) return (int)e;
+            opted[1] = smem;
+        }
         k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row);
     }
     return (int)cudaGetLastError();
@@ -280,22 +293,14 @@ int launch_corr(int mode, const mvd_handle* h, const float* src, const float* G,
                                       h->eps, n_planes, st, phi_plane, phi_row);
         MVD_DIRECT_CASE(9, 9)
         MVD_DIRECT_CASE(21, 7)
-        MVD_DIRECT_CASE(21, 11)
-        MVD_DIRECT_CASE(21, 21)
         MVD_DIRECT_CASE(31, 8)
-        MVD_DIRECT_CASE(31, 11)
         MVD_DIRECT_CASE(41, 7)
-        MVD_DIRECT_CASE(41, 14)
-        MVD_DIRECT_CASE(51, 9)
-        MVD_DIRECT_CASE(51, 13)
         MVD_DIRECT_CASE(51, 17)
 #undef MVD_DIRECT_CASE
         if (h->JC == 8)
             return launch_pair2<0, 8>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp, h->eps, n_planes, st,
                                       phi_plane, phi_row);
     }
-    if (h->JC == 9) return launch_pair_member<0, 9>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp, h->eps, n_planes, st, phi_plane, phi_row);
-    if (h->JC == 7) return launch_pair_member<0, 7>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp, h->eps, n_planes, st, phi_plane, phi_row);
     return launch_pair_member<0, 8>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp, h->eps,
                                     n_planes, st, phi_plane, phi_row);
 }
@@ -312,12 +317,6 @@ int direct_choose_chunk(int K, int* JC, int* Kp) {
         case 41: jc = 7; break;
         case 51: jc = 17; break;
         default: jc = 8; break;
-    }
-    if (const char* e = getenv("MVD_DIRECT_JC")) {   // measurement knob
-        const int v = atoi(e);
-        if ((K == 21 && (v == 7 || v == 11 || v == 21)) || (K == 31 && (v == 8 || v == 11)) ||
-            (K == 41 && (v == 7 || v == 14)) || (K == 51 && (v == 9 || v == 13 || v == 17)))
-            jc = v;
     }
     *JC = jc;
     *Kp = ((K + jc - 1) / jc) * jc;
@@ -350,8 +349,12 @@ int direct_setup(mvd_handle* h, const float* host_psfs, const float* host_xs) {
     host_psfs = pad_p.data();
     const float* host_back = pad_b.data();
     direct_choose_chunk(h->K, &h->JC, &h->Kp);
-    // two planes per thread whenever the float2 tile fits (MVD_DIRECT_SINGLE: measurement knob)
-    h->direct_pair = pair_smem_bytes(h->K, h->Kp) <= 227u * 1024u && getenv("MVD_DIRECT_SINGLE") == nullptr;
+    // two planes per thread whenever the float2 tile fits; the single-plane kernel works in row chunks of 8
+    h->direct_pair = pair_smem_bytes(h->K, h->Kp) <= 227u * 1024u;
+    if (!h->direct_pair) {
+        h->JC = 8;
+        h->Kp = (h->K + 7) / 8 * 8;
+    }
     const int K = h->K, Kp = h->Kp;
     const size_t per = (size_t)K * Kp;
     // shared memory needed by one CTA must fit the 227 KB limit

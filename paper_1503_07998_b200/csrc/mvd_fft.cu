@@ -16,12 +16,6 @@ using mvdfft::SizeOps;
 
 namespace {
 
-// MVD_FFT_GEN=1 keeps the first-generation kernels for every length (measurement only)
-bool want_v2() {
-    const char* g = getenv("MVD_FFT_GEN");
-    return !(g && g[0] == '1');
-}
-
 // The two generations lay the spectrum out differently (v2: tile-major), so a plane uses v2 kernels
 // only when BOTH of its lengths have them.
 const SizeOps* find_ops_v1(int N) {
@@ -30,7 +24,6 @@ const SizeOps* find_ops_v1(int N) {
     return mvd_fft_ops_large(N);
 }
 bool use_v2(int W, int H) {
-    if (!want_v2()) return false;
     const SizeOps* r = mvd_fft_ops_v2(W);
     const SizeOps* c = mvd_fft_ops_v2(H);
     return r && c && r->rows && c->cols;

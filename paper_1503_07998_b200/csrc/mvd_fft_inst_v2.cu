@@ -1,6 +1,4 @@
 // FFT engine, generation-2 (team-synchronous) kernels: 256, 512, 1024, 2048.
-#include <stdlib.h>
-
 #include "mvd_fft_v2.cuh"
 using namespace mvdfft;
 
@@ -15,17 +13,6 @@ const SizeOps* mvd_fft_ops_v2(int N) {
     static const SizeOps o2048 = OpsFor2<P2048, 128, P2048, 256, false, 2, false, 4, 3>::make();   // rows: 3 CTAs of 2 teams, 168 registers
     using P800C = Plan<800, 40, 40, 20>;     // columns only: eight columns per team of 160 threads
     static const SizeOps o800 = ColsOnly2<P800C, 160, false, 2, 8>::make();
-    // measurement knob MVD_COLS_VARIANT (profiles/r1_fft_v2_ncu_full.md): a = eight, b = sixteen columns per team,
-    // c = dedicated landing zone requested a whole item ahead; all within +-3 % of the default on config 2
-    static const SizeOps o256a = OpsFor2<P256, 256, P256, 128, true, 4, true, 8>::make();
-    static const SizeOps o256b = OpsFor2<P256, 256, P256, 256, true, 2, true, 16>::make();
-    static const SizeOps o256c = OpsFor2<P256, 256, P256, 128, true, 4, true, 4, 2, true>::make();
-    static const char* var = getenv("MVD_COLS_VARIANT");
-    if (N == 256 && var) {
-        if (var[0] == 'a') return &o256a;
-        if (var[0] == 'b') return &o256b;
-        if (var[0] == 'c') return &o256c;
-    }
     switch (N) {
         case 256: return &o256;
         case 512: return &o512;

@@ -88,6 +88,135 @@ def test_large_configs_against_stored_oracle_planes(cid):
 
 
 # ---------------------------------------------------------------------------------------------
+# Configs 3-5, element by element against WHOLE stored oracle planes (tests/golden/config*_planes.npz)
+# ---------------------------------------------------------------------------------------------
+def _whole_planes(cid):
+    fn = os.path.join(GOLDEN, f"config{cid}_planes.npz")
+    if not os.path.exists(fn):
+        pytest.skip(f"{fn} not generated yet")
+    g = np.load(fn)
+    planes = [int(p) for p in g["planes"]]
+    ref = np.stack([g[f"plane_{p}"] for p in planes]).astype(np.float64)
+    return planes, ref, g["view_sums"], int(g["pipeline_batch"])
+
+
+@pytest.mark.parametrize("path", [binding.PATH_FFT, binding.PATH_DIRECT])
+@pytest.mark.parametrize("cid", [3, 4, 5])
+def test_large_configs_whole_planes_both_engines(cid, path):
+    """Planes {0, B-1, B, N/2, N-1} of configs 3-5 at full size as a five-plane stack (odd: the last pair is
+    half empty), every pixel against the stored fp64 oracle plane, on the FFT engine AND the direct engine
+    (K = 31 / 41 / 51 templated kernels)."""
+    cfg = synth.config(cid)
+    _need(path, cfg.W, cfg.H, cfg.K)
+    planes, ref, view_sums, _ = _whole_planes(cid)
+    psfs = synth.config_psfs(cid)
+    views = synth.views(cfg, planes, psfs)
+    for k in range(len(planes)):      # the stored planes belong to exactly these inputs
+        assert [int(views[v, k].astype(np.int64).sum()) for v in range(cfg.V)] == [int(x) for x in view_sums[k]]
+    out = _run(views, psfs, cfg.T, path)
+    l2, pooled, mx = assert_parity(out, ref, f"config{cid} whole planes {binding.PATH_NAMES[path]}")
+    print(f"config{cid} {binding.PATH_NAMES[path]}: rel L2 {l2:.2e} (pooled {pooled:.2e}) max rel {mx:.2e}")
+
+
+def _load_bench():
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("bench", os.path.join(os.path.dirname(GOLDEN), "..", "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    return bench
+
+
+@pytest.mark.parametrize("cid", [3, 4, 5])
+def test_large_configs_full_stack_in_the_bench_launch_configuration(cid):
+    """The whole N-plane stack of configs 3-5 exactly as bench.py times it (same stack builder, default batches
+    dealt to the library's internal streams), with the canonical planes that have stored oracle planes written
+    at their own positions -- first, last, middle and both sides of a batch boundary of the launch
+    configuration -- and compared element by element; plus, on EVERY plane, pin P12: psi >= 0, finite,
+    sum(psi) = sum(phi_last)."""
+    import torch
+    bench = _load_bench()
+    cfg = synth.config(cid)
+    planes, ref, _, b_stored = _whole_planes(cid)
+    psfs, views = bench.make_stack(cfg)
+    canon = synth.views(cfg, planes, psfs)
+    with binding.Mvd(cfg.W, cfg.H, cfg.V, psfs, cfg.K, cfg.T, cfg.eps) as m:
+        B = m.get_batch_planes(cfg.N)
+        where = {p: k for k, p in enumerate(planes)}          # stack position -> index into ref
+        if B != b_stored:                                      # the boundary moved: put the stored pair on it
+            where[B - 1], where[B] = planes.index(b_stored - 1), planes.index(b_stored)
+        for pos, k in where.items():
+            views[:, pos] = canon[:, k]
+        assert {0, B - 1, B, cfg.N // 2, cfg.N - 1} <= set(where)
+        m.reserve(cfg.N)
+        dv = torch.empty((cfg.V, cfg.N, cfg.H, cfg.W), dtype=torch.int16, device="cuda")
+        step = 64
+        for p0 in range(0, cfg.N, step):                       # upload in slices: no second 13 GB host copy
+            dv[:, p0:p0 + step] = torch.from_numpy(views[:, p0:p0 + step].view(np.int16)).cuda()
+        do = torch.empty((cfg.N, cfg.H, cfg.W), dtype=torch.float32, device="cuda")
+        m.deconvolve_planes(dv, do, cfg.N)
+        torch.cuda.synchronize()
+        assert bool(torch.isfinite(do).all()) and bool((do >= 0).all())
+        got = do.sum(dim=(1, 2), dtype=torch.float64).cpu().numpy()
+        want = np.array([views[-1, p].astype(np.int64).sum() for p in range(cfg.N)], dtype=np.float64)
+        np.testing.assert_allclose(got, want, rtol=2e-5)
+        pos = sorted(where)
+        out = do[torch.tensor(pos, device="cuda")].cpu().numpy()
+    assert_parity(out, ref[[where[p] for p in pos]], f"config{cid} full stack, planes {pos}")
+
+
+def test_host_pipeline_with_ramp_and_odd_plane_count_is_bit_identical():
+    """with the batch ramp (B/4, B/2 at both ends) and an odd n_planes every non-final batch must
+    still start on an even plane, or the FFT engine pairs (2m+1, 2m+2) and the bits differ."""
+    import torch
+    V, W, H, K, T = 2, 256, 256, 5, 2
+    N = 8 * 32 + 9                     # >= 8 B with B = 32 planes of 256 x 256 (the 2 Mvoxel floor): ramp on, odd
+    pr = synth.make_problem(V, 16, W, H, K, T, seed=991)
+    views = np.concatenate([np.roll(pr.views, 7 * k, axis=3) for k in range(N // 16 + 1)], axis=1)[:, :N]
+    views = np.ascontiguousarray(views)
+    with binding.Mvd(W, H, V, pr.psfs, K, T, pr.eps, binding.PATH_FFT) as m:
+        B = m.get_batch_planes(N)
+        assert B >= 8 and N >= 8 * B and N % 2 == 1
+        hv = torch.from_numpy(views.view(np.int16)).pin_memory()
+        ho = torch.empty((N, H, W), dtype=torch.float32).pin_memory()
+        m.deconvolve_host(hv, ho, N)
+        dv = hv.cuda()
+        do = torch.empty((N, H, W), dtype=torch.float32, device="cuda")
+        m.deconvolve_planes(dv, do, N)
+        torch.cuda.synchronize()
+        assert torch.equal(ho, do.cpu())
+    ref = mvd_oracle.deconvolve(np.ascontiguousarray(views[:, -3:]), pr.psfs, T, pr.eps)
+    assert_parity(ho.numpy()[-3:], ref, "odd tail of the ramped pipeline")
+
+
+@pytest.mark.parametrize("path", PATHS)
+def test_reserved_handle_is_capturable_into_a_cuda_graph(path):
+    """After mvd_reserve the device-resident call only enqueues (no allocation, no synchronisation): it can be
+    captured into a CUDA graph and replayed, with the same bits as the eager call."""
+    import torch
+    V, N, W, H, K, T = 2, 6, 64, 64, 9, 3
+    _need(path, W, H, K)
+    pr = synth.make_problem(V, N, W, H, K, T, seed=4242)
+    with binding.Mvd(W, H, V, pr.psfs, K, T, pr.eps, path) as m:
+        m.reserve(N)
+        dv = torch.from_numpy(pr.views.view(np.int16)).cuda()
+        eager = torch.empty((N, H, W), dtype=torch.float32, device="cuda")
+        st = torch.cuda.Stream()
+        m.deconvolve_planes(dv, eager, N, st)
+        st.synchronize()
+        out = torch.zeros_like(eager)
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.graph(g, stream=st):
+            m.deconvolve_planes(dv, out, N, st)
+        assert not out.any()                    # capture enqueued nothing
+        for _ in range(2):
+            out.zero_()
+            g.replay()
+            torch.cuda.synchronize()
+            assert torch.equal(out, eager)
+        del g
+
+
+# ---------------------------------------------------------------------------------------------
 # Cases the configs lack: asymmetric PSFs (conv vs corr, flip, centre), ragged shapes, aliasing
 # ---------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("path", PATHS)
@@ -100,6 +229,7 @@ def test_large_configs_against_stored_oracle_planes(cid):
     (4, 2, 60, 36, 9, 3, "gauss"),
     (2, 2, 37, 23, 5, 3, "random"),      # primes: direct only
     (2, 2, 192, 320, 51, 1, "random"),   # largest templated K, 3-chunk rows
+    (2, 3, 160, 96, 41, 2, "random"),    # config 4's PSF size on the direct engine (direct_corr2_kernel<41, 7>)
     (2, 2, 256, 800, 9, 2, "random"),    # config 4's column length (800 = 2^5 5^2)
     (1, 3, 2048, 64, 7, 2, "random"),    # config 4's row length
     (2, 2, 64, 1024, 5, 2, "random"),    # config 5's column length
