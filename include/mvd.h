@@ -166,6 +166,18 @@ MVD_API int mvd_reserve(mvd_handle* h, int max_planes);
  * (the default policy, or mvd_set_batch_planes); batches start at multiples of it. */
 MVD_API int mvd_get_batch_planes(const mvd_handle* h, int n_planes);
 
+/*
+ * Guard of the FFT engine.  Step a2 divides by the blur b = psi (*) P_v; where b is smaller than the
+ * round-off of an fp32 transform (about 1e-6 of the plane's maximum) and phi_v > 0 there, the quotient is noise of
+ * the order phi / eps, and the next transform spreads it over the whole plane pair.  (This needs data that say
+ * "signal" where the estimate says "nothing": a view zero-filled where the others are not, photons on an exactly
+ * zero background.)  The FFT engine therefore flags every plane pair in which some pixel has phi_v > 0 and
+ * b < 2^-13 max(psi_0), and recomputes the flagged pairs from scratch with the direct engine's arithmetic, in the
+ * same call and on the same stream; the result is the direct engine's, bit for bit.  mvd_guard_flagged returns how
+ * many plane pairs this handle has handed over so far (blocks until the handle's work is done).
+ */
+MVD_API long long mvd_guard_flagged(mvd_handle* h);
+
 /* Frees the plan, its scratch, its streams and staging buffers.  NULL is a no-op. */
 MVD_API void mvd_destroy(mvd_handle* h);
 
@@ -202,7 +214,7 @@ MVD_API int mvd_set_batch_planes(mvd_handle* h, int planes);
  *                         since the last read; both arrays are HOST, length MVD_N_KERNEL_CLASSES.
  *   mvd_kernel_class_name static name of class k (NULL if out of range).
  */
-enum { MVD_N_KERNEL_CLASSES = 8 };
+enum { MVD_N_KERNEL_CLASSES = 10 };
 MVD_API long long mvd_launch_count(const mvd_handle* h);
 MVD_API void mvd_launch_count_reset(mvd_handle* h);
 MVD_API int mvd_profile_enable(mvd_handle* h, int on);

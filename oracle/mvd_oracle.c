@@ -34,7 +34,10 @@
  * P7 I-divergence monotone, P8 numpy-FFT cross-check of both convolutions, P9 duplicated view,
  * P10 shift equivariance, P11 zero iterations; explicit back-projectors (mvd_oracle_x): PX1 X = flip(P)
  * reduces to the Independent variant, PX2 dense-matrix brute force with an asymmetric X of another
- * size, PX3 centred-delta X closed form.  Parity unpinned: nothing in this file.
+ * size, PX3 centred-delta X closed form; per-view weights (mvd_oracle_w): PW1 w = 1 is the unweighted run bit for
+ * bit, PW2 a view with w = 0 is never applied, PW3 constants stay fixed, PW4 dense-matrix brute force with random
+ * weights.  Parity unpinned: READING W1 (what the paper's "weights" buffer, does) -- its arithmetic is
+ * pinned, its meaning is not fixed by anything the paper prints.
  */
 #include <math.h>
 #include <pthread.h>
@@ -147,9 +150,15 @@ void mvd_oracle_backproject(const double* r, const float* P, int K, int W, int H
  * variants all used the following formula, but replaced X"): step a3 becomes the TRUE periodic
  * convolution q = r * X_v, q(x) = sum_u X_v(u) r(x - u), index (j,i) <-> u = (j-cx, i-cx).
  * xs == NULL is the "Independent" variant X = P_v^* (correlation with P_v). */
+/* weights (nullable): per-view, per-pixel weights w_v in [0, 1], float, same layout as the views
+ * (PAPER.md:88 lists "weights, float, 4 v bytes/pixel" and never says what they do; READING W1, DESIGN.md
+ * section 2, parity unpinned): the weight blends view v's multiplicative correction with the identity,
+ *     a4w   psi <- psi . (w_v q + (1 - w_v)),
+ * so w_v = 1 is the unweighted update (bit for bit: 1 q + 0) and w_v = 0 leaves the pixel untouched by view v
+ * (a registered view that does not cover it).  a0 (the mean of the views) and a1-a3 are unchanged. */
 static void rl_plane(int W, int H, int V, const float* psfs, int K, int T, double eps,
                      const uint16_t* views, size_t view_stride, double* psi, double* trace,
-                     int literal, const float* xs, int KX) {
+                     int literal, const float* xs, int KX, const float* weights, size_t w_view_stride) {
     const size_t npx = (size_t)W * H;
     double* b = (double*)malloc(sizeof(double) * npx);
     double* r = (double*)malloc(sizeof(double) * npx);
@@ -177,7 +186,13 @@ static void rl_plane(int W, int H, int V, const float* psfs, int K, int T, doubl
                 else         mvd_oracle_blur(r, X, KX, W, H, q);
             } else if (literal) mvd_oracle_backproject_literal(r, P, K, W, H, q); /* a3, X = P_v^* */
             else         mvd_oracle_backproject(r, P, K, W, H, q);
-            for (size_t p = 0; p < npx; ++p) psi[p] = psi[p] * q[p];             /* a4 */
+            if (weights) {                                                       /* a4w (reading W1) */
+                const float* w = weights + (size_t)v * w_view_stride;
+                for (size_t p = 0; p < npx; ++p)
+                    psi[p] = psi[p] * ((double)w[p] * q[p] + (1.0 - (double)w[p]));
+            } else {
+                for (size_t p = 0; p < npx; ++p) psi[p] = psi[p] * q[p];         /* a4 */
+            }
             if (trace) memcpy(trace + ((size_t)t * V + v) * npx, psi, sizeof(double) * npx);
         }
     }
@@ -202,6 +217,7 @@ typedef struct {
     double eps;
     const float* xs;
     int KX;
+    const float* weights;
     const float* psfs;
     const uint16_t* views;
     double* out;
@@ -213,13 +229,14 @@ static void* worker(void* arg) {
     const size_t npx = (size_t)j->W * j->H;
     for (int p = j->p_begin; p < j->p_end; ++p)
         rl_plane(j->W, j->H, j->V, j->psfs, j->K, j->T, j->eps, j->views + (size_t)p * npx,
-                 (size_t)j->N * npx, j->out + (size_t)p * npx, NULL, j->literal, j->xs, j->KX);
+                 (size_t)j->N * npx, j->out + (size_t)p * npx, NULL, j->literal, j->xs, j->KX,
+                 j->weights ? j->weights + (size_t)p * npx : NULL, (size_t)j->N * npx);
     return NULL;
 }
 
 static int run(int W, int H, int V, const float* psfs, int K, int T, double eps,
                const uint16_t* views, double* out, int N, int n_threads, int literal,
-               const float* xs, int KX) {
+               const float* xs, int KX, const float* weights) {
     int rc = check_args(W, H, V, psfs, K, T, eps, views, out, N);
     if (rc) return rc;
     if (xs && (KX < 1 || (KX % 2) == 0)) return -1;
@@ -228,7 +245,7 @@ static int run(int W, int H, int V, const float* psfs, int K, int T, double eps,
     job_t* jobs = (job_t*)calloc((size_t)n_threads, sizeof(job_t));
     pthread_t* th = (pthread_t*)calloc((size_t)n_threads, sizeof(pthread_t));
     for (int k = 0; k < n_threads; ++k) {
-        job_t j = {W, H, V, K, T, N, literal, eps, xs, KX, psfs, views, out,
+        job_t j = {W, H, V, K, T, N, literal, eps, xs, KX, weights, psfs, views, out,
                    (int)((long long)N * k / n_threads), (int)((long long)N * (k + 1) / n_threads)};
         jobs[k] = j;
     }
@@ -241,19 +258,30 @@ static int run(int W, int H, int V, const float* psfs, int K, int T, double eps,
 
 int mvd_oracle(int W, int H, int V, const float* psfs, int K, int T, double eps,
                const uint16_t* views, double* out, int N, int n_threads) {
-    return run(W, H, V, psfs, K, T, eps, views, out, N, n_threads, 0, NULL, 0);
+    return run(W, H, V, psfs, K, T, eps, views, out, N, n_threads, 0, NULL, 0, NULL);
 }
 
 /* The same iteration with the back-projectors X_v given explicitly: xs float [V][KX][KX], KX odd. */
 int mvd_oracle_x(int W, int H, int V, const float* psfs, int K, const float* xs, int KX, int T,
                  double eps, const uint16_t* views, double* out, int N, int n_threads, int literal) {
     if (!xs) return -1;
-    return run(W, H, V, psfs, K, T, eps, views, out, N, n_threads, literal, xs, KX);
+    return run(W, H, V, psfs, K, T, eps, views, out, N, n_threads, literal, xs, KX, NULL);
+}
+
+/* The same iteration with per-view weights (reading W1 above): weights float [V][N][H][W], finite, in [0, 1];
+ * xs (nullable) as in mvd_oracle_x. */
+int mvd_oracle_w(int W, int H, int V, const float* psfs, int K, const float* xs, int KX, int T, double eps,
+                 const uint16_t* views, const float* weights, double* out, int N, int n_threads, int literal) {
+    if (!weights) return -1;
+    const size_t nw = (size_t)V * N * H * W;
+    for (size_t k = 0; k < nw; ++k)
+        if (!(weights[k] >= 0.f && weights[k] <= 1.f)) return -1;
+    return run(W, H, V, psfs, K, T, eps, views, out, N, n_threads, literal, xs, KX, weights);
 }
 
 int mvd_oracle_literal(int W, int H, int V, const float* psfs, int K, int T, double eps,
                        const uint16_t* views, double* out, int N, int n_threads) {
-    return run(W, H, V, psfs, K, T, eps, views, out, N, n_threads, 1, NULL, 0);
+    return run(W, H, V, psfs, K, T, eps, views, out, N, n_threads, 1, NULL, 0, NULL);
 }
 
 /* One plane (views [V][H][W]); trace [T*V][H][W] = psi after every view update; out [H][W]. */
@@ -261,6 +289,6 @@ int mvd_oracle_trace(int W, int H, int V, const float* psfs, int K, int T, doubl
                      const uint16_t* views, double* out, double* trace) {
     int rc = check_args(W, H, V, psfs, K, T, eps, views, out, 1);
     if (rc) return rc;
-    rl_plane(W, H, V, psfs, K, T, eps, views, (size_t)W * H, out, trace, 0, NULL, 0);
+    rl_plane(W, H, V, psfs, K, T, eps, views, (size_t)W * H, out, trace, 0, NULL, 0, NULL, 0);
     return 0;
 }

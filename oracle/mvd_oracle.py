@@ -67,6 +67,8 @@ def _load() -> ctypes.CDLL:
         fn.restype = i
     lib.mvd_oracle_x.argtypes = [i, i, i, fp, i, fp, i, i, d, up, dp, i, i, i]
     lib.mvd_oracle_x.restype = i
+    lib.mvd_oracle_w.argtypes = [i, i, i, fp, i, fp, i, i, d, up, fp, dp, i, i, i]
+    lib.mvd_oracle_w.restype = i
     lib.mvd_oracle_trace.argtypes = [i, i, i, fp, i, i, d, up, dp, dp]
     lib.mvd_oracle_trace.restype = i
     for name in ("mvd_oracle_blur", "mvd_oracle_backproject",
@@ -95,13 +97,16 @@ def n_cores() -> int:
 
 def deconvolve(views: np.ndarray, psfs: np.ndarray, T: int, eps: float = 1e-6,
                n_threads: Optional[int] = None, literal: bool = False,
-               backprojectors: Optional[np.ndarray] = None) -> np.ndarray:
+               backprojectors: Optional[np.ndarray] = None,
+               weights: Optional[np.ndarray] = None) -> np.ndarray:
     """fp64 `[N][H][W]` = T sequential multi-view RL iterations on every plane.
 
     views uint16 `[V][N][H][W]`, psfs float32 `[V][K][K]`.  eps is first rounded to fp32 (the C ABI
     of the product takes `float eps`), so both sides clamp at the identical threshold (reading A6).
     backprojectors float32 `[V][KX][KX]` (optional): step a3 is the true convolution r * X_v with these
     kernels instead of the correlation with P_v; None is the Independent variant.
+    weights float32 `[V][N][H][W]` in [0, 1] (optional): step a4 becomes psi <- psi . (w_v q + 1 - w_v)
+    ("weights"; READING W1, parity unpinned).
     """
     views = np.ascontiguousarray(views, dtype=np.uint16)
     psfs = _f32(psfs)
@@ -111,6 +116,18 @@ def deconvolve(views: np.ndarray, psfs: np.ndarray, T: int, eps: float = 1e-6,
     assert psfs.shape[2] == K
     out = np.empty((N, H, W), dtype=np.float64)
     nt = n_cores() if n_threads is None else n_threads
+    if weights is not None:
+        w = _f32(weights)
+        assert w.shape == views.shape
+        xs = _f32(backprojectors) if backprojectors is not None else None
+        rc = _load().mvd_oracle_w(W, H, V, _ptr(psfs, ctypes.c_float), K,
+                                  _ptr(xs, ctypes.c_float) if xs is not None else None,
+                                  xs.shape[1] if xs is not None else 0, int(T), float(np.float32(eps)),
+                                  _ptr(views, ctypes.c_uint16), _ptr(w, ctypes.c_float),
+                                  _ptr(out, ctypes.c_double), N, int(nt), int(bool(literal)))
+        if rc != 0:
+            raise ValueError(f"mvd_oracle_w rejected its arguments (rc={rc})")
+        return out
     if backprojectors is not None:
         xs = _f32(backprojectors)
         assert xs.ndim == 3 and xs.shape[0] == V and xs.shape[1] == xs.shape[2]

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libmvd.so")
 
 MVD_OK, MVD_ERR_INVALID, MVD_ERR_UNSUPPORTED, MVD_ERR_CUDA, MVD_ERR_NOMEM, MVD_ERR_BUSY = 0, -1, -2, -3, -4, -5
 PATH_AUTO, PATH_DIRECT, PATH_FFT = 0, 1, 2
-N_KERNEL_CLASSES = 8
+N_KERNEL_CLASSES = 10
 PATH_NAMES = {PATH_AUTO: "auto", PATH_DIRECT: "direct", PATH_FFT: "fft"}
 
 # name -> (restype, argtypes): the symbols include/mvd.h declares (tests check the two agree)
@@ -37,6 +37,7 @@ SIGNATURES = {
     "mvd_last_cuda_error": (_i, [_vp]),
     "mvd_get_path": (_i, [_vp]),
     "mvd_path_supported": (_i, [_i, _i, _i, _i]),
+    "mvd_guard_flagged": (_ll, [_vp]),
     "mvd_reserve": (_i, [_vp, _i]),
     "mvd_get_batch_planes": (_i, [_vp, _i]),
     "mvd_set_chunk_planes": (_i, [_vp, _i]),
@@ -163,6 +164,10 @@ class Mvd:
     @property
     def path(self) -> int:
         return lib().mvd_get_path(self._h)
+
+    def guard_flagged(self) -> int:
+        """Plane pairs the FFT engine's guard has handed to the direct engine so far (synchronises)."""
+        return int(lib().mvd_guard_flagged(self._h))
 
     def reserve(self, max_planes: int) -> None:
         self._raise(lib().mvd_reserve(self._h, max_planes), "mvd_reserve")

@@ -56,15 +56,17 @@ static int grow(mvd_handle* h, float** p, size_t* have, size_t want) {
     return MVD_OK;
 }
 
-int ws_reserve(mvd_handle* h, Workspace& ws, size_t a_bytes, size_t b_bytes) {
+int ws_reserve(mvd_handle* h, Workspace& ws, size_t a_bytes, size_t b_bytes, size_t g_bytes) {
     int rc = grow(h, &ws.a, &ws.a_bytes, a_bytes);
-    if (rc != MVD_OK) return rc;
-    return grow(h, &ws.b, &ws.b_bytes, b_bytes);
+    if (rc == MVD_OK) rc = grow(h, &ws.b, &ws.b_bytes, b_bytes);
+    if (rc == MVD_OK) rc = grow(h, reinterpret_cast<float**>(&ws.g), &ws.g_bytes, g_bytes);
+    return rc;
 }
 
 static void ws_free(Workspace& ws) {
     if (ws.a) cudaFree(ws.a);
     if (ws.b) cudaFree(ws.b);
+    if (ws.g) cudaFree(ws.g);
     ws = Workspace();
 }
 
@@ -91,7 +93,9 @@ int mvd_path_supported(int path, int plane_w, int plane_h, int psf_size) {
 static int choose_path(int W, int H, int K) {
     const bool fft_ok = mvd_path_supported(MVD_PATH_FFT, W, H, K) != 0;
     const bool dir_ok = mvd_path_supported(MVD_PATH_DIRECT, W, H, K) != 0;
-    (void)K;   // measured on config 2's shape: the FFT engine wins at every K, even K = 3
+    // planes small enough to stay on chip for the whole run (one launch) beat the FFT engine's
+    // 4 V T + 1 launches up to K ~ 9; everywhere else the FFT engine wins at every K, even K = 3 (section 7)
+    if (dir_ok && K <= 9 && direct_small_fits(W, H, K)) return MVD_PATH_DIRECT;
     if (fft_ok) return MVD_PATH_FFT;
     if (dir_ok) return MVD_PATH_DIRECT;
     return -1;
@@ -234,6 +238,7 @@ void mvd_destroy(mvd_handle* h) {
     }
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     if (h->d_coef) cudaFree(h->d_coef);
+    if (h->d_guard_total) cudaFree(h->d_guard_total);
     if (h->d_otf) cudaFree(h->d_otf);
     if (h->d_otf_b) cudaFree(h->d_otf_b);
     fft_teardown(h);
@@ -249,7 +254,7 @@ void mvd_destroy(mvd_handle* h) {
 static int even_up(int n) { return n + (n & 1); }
 
 static int default_chunk(const mvd_handle* h) {
-    if (h->chunk_planes > 0) return h->path == MVD_PATH_FFT ? even_up(h->chunk_planes) : h->chunk_planes;
+    if (h->chunk_planes > 0) return h->path == MVD_PATH_FFT ? even_up(std::min(h->chunk_planes, 1024)) : h->chunk_planes;
     if (h->path == MVD_PATH_FFT) return fft_default_chunk(h);
     // direct: bound the scratch (one fp32 plane per plane) to ~1 GiB
     const size_t npx = (size_t)h->W * h->H;
@@ -285,13 +290,14 @@ static int ensure_streams(mvd_handle* h) {
 }
 
 // Scratch of one workspace that runs n planes at a time (FFT: Z and S, 8 B per voxel each; direct: r).
-static void scratch_bytes(const mvd_handle* h, int n, size_t* a, size_t* b) {
+static void scratch_bytes(const mvd_handle* h, int n, size_t* a, size_t* b, size_t* g) {
     const size_t npx = (size_t)h->W * h->H;
     if (h->path == MVD_PATH_FFT) {
         *a = *b = sizeof(float2) * (size_t)((n + 1) / 2) * npx;
+        *g = fft_guard_bytes(n);
     } else {
         *a = h->T > 0 ? sizeof(float) * (size_t)n * npx : 0;
-        *b = 0;
+        *b = *g = 0;
     }
 }
 
@@ -318,12 +324,12 @@ int mvd_reserve(mvd_handle* h, int max_planes) {
     int rc = ensure_streams(h);
     if (rc != MVD_OK) return rc;
     const int B = default_batch(h, max_planes), chunk = default_chunk(h);
-    size_t a, b;
-    scratch_bytes(h, std::min(chunk, max_planes), &a, &b);
-    if ((rc = ws_reserve(h, h->ws_main, a, b)) != MVD_OK) return rc;
-    scratch_bytes(h, std::min(chunk, B), &a, &b);
+    size_t a, b, g;
+    scratch_bytes(h, std::min(chunk, max_planes), &a, &b, &g);
+    if ((rc = ws_reserve(h, h->ws_main, a, b, g)) != MVD_OK) return rc;
+    scratch_bytes(h, std::min(chunk, B), &a, &b, &g);
     for (int s = 0; s < mvd_handle::kSlots; ++s)
-        if ((rc = ws_reserve(h, h->ws_slot[s], a, b)) != MVD_OK) return rc;
+        if ((rc = ws_reserve(h, h->ws_slot[s], a, b, g)) != MVD_OK) return rc;
     return reserve_slots(h, B);
 }
 
@@ -342,9 +348,9 @@ static int run_resident(mvd_handle* h, const uint16_t* views, ViewLayout lay, fl
     if (ns <= 1 || h->profiling || n_planes < 2 * B) return run_core(h, h->ws_main, views, lay, out, n_planes, stream);
     int rc = ensure_streams(h);
     {
-        size_t a, b;
-        scratch_bytes(h, std::min(default_chunk(h), B), &a, &b);
-        for (int s = 0; s < ns && rc == MVD_OK; ++s) rc = ws_reserve(h, h->ws_slot[s], a, b);
+        size_t a, b, g;
+        scratch_bytes(h, std::min(default_chunk(h), B), &a, &b, &g);
+        for (int s = 0; s < ns && rc == MVD_OK; ++s) rc = ws_reserve(h, h->ws_slot[s], a, b, g);
     }
     if (rc != MVD_OK) return rc;
     MVD_TRY(h, cudaEventRecord(h->ev_fork, stream));
@@ -414,9 +420,9 @@ static int host_pipeline(mvd_handle* h, const uint16_t* host_views_u16, float* h
     {   // everything the batches need is sized before the first copy is enqueued: nothing below allocates
         int rc0 = ensure_streams(h);
         if (rc0 == MVD_OK) rc0 = reserve_slots(h, B);
-        size_t a, b;
-        scratch_bytes(h, std::min(default_chunk(h), B), &a, &b);
-        for (int s = 0; s < mvd_handle::kSlots && rc0 == MVD_OK; ++s) rc0 = ws_reserve(h, h->ws_slot[s], a, b);
+        size_t a, b, g;
+        scratch_bytes(h, std::min(default_chunk(h), B), &a, &b, &g);
+        for (int s = 0; s < mvd_handle::kSlots && rc0 == MVD_OK; ++s) rc0 = ws_reserve(h, h->ws_slot[s], a, b, g);
         if (rc0 != MVD_OK) return rc0;
     }
 
@@ -509,6 +515,15 @@ const char* mvd_strerror(int code) {
 }
 
 int mvd_last_cuda_error(const mvd_handle* h) { return h ? h->last_cuda : 0; }
+
+long long mvd_guard_flagged(mvd_handle* h) {
+    if (!h) return MVD_ERR_INVALID;
+    if (!h->d_guard_total) return 0;
+    unsigned n = 0;
+    if (mvd_check(h, cudaDeviceSynchronize()) != MVD_OK) return MVD_ERR_CUDA;
+    if (mvd_check(h, cudaMemcpy(&n, h->d_guard_total, sizeof n, cudaMemcpyDeviceToHost)) != MVD_OK) return MVD_ERR_CUDA;
+    return (long long)n;
+}
 int mvd_get_path(const mvd_handle* h) { return h ? h->path : MVD_ERR_INVALID; }
 
 int mvd_set_chunk_planes(mvd_handle* h, int planes) {
@@ -558,7 +573,7 @@ int mvd_profile_read(mvd_handle* h, float* ms, long long* n) {
 const char* mvd_kernel_class_name(int k) {
     static const char* names[MVD_N_KERNEL_CLASSES] = {
         "init_mean", "direct_blur_ratio", "direct_backproject_update", "fft_rows_first",
-        "fft_cols_otf", "fft_rows_ratio", "fft_rows_update", "setup"};
+        "fft_cols_otf", "fft_rows_ratio", "fft_rows_update", "setup", "guard_repair", "small_resident"};
     return (k >= 0 && k < MVD_N_KERNEL_CLASSES) ? names[k] : nullptr;
 }
 

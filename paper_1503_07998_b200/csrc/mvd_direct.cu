@@ -11,6 +11,8 @@
 // registers: for one PSF column i it reads a (RY+JC-1)-tall window of the staged column (one
 // conflict-free LDS per value, lanes along x) and issues JC*RY FFMAs on it.  The FP32 FMA pipe is
 // the bound (4 K^2 flop against 22 B of HBM traffic per voxel-view-iteration).
+#include <algorithm>
+
 #include "mvd_internal.cuh"
 
 namespace {
@@ -130,13 +132,15 @@ __device__ __forceinline__ float2 ffma2_bcast(float g, float2 w, float2 c) {
     return r;
 }
 
-template <int KT, int JC, int MODE>
-__global__ void __launch_bounds__(BX* BY)
-direct_corr2_kernel(const float* __restrict__ src, const float* __restrict__ G,
-                    const uint16_t* __restrict__ phi, float* __restrict__ dst, int W, int H, int Krt,
-                    int Kp, float eps, int tiles_x, int tiles_y, size_t phi_plane, size_t phi_row,
-                    int n_planes) {
-    extern __shared__ __align__(16) float smem[];
+// One 64 x 64 output tile (tile_x, tile_y) of the plane pair (pa, pa + 1): stage, correlate, epilogue.
+// `stage_G`: copy the coefficient array into shared memory first (false when the caller already did).
+// CG: read src and the read-modify-write of dst through L2 only (ld.global.cg) -- the persistent repair kernel
+// reads what other SMs wrote earlier in the SAME launch, which a stale L1 line must not serve.
+template <int KT, int JC, int MODE, bool CG = false>
+__device__ __forceinline__ void corr2_tile(float* smem, const float* __restrict__ src, const float* __restrict__ G,
+                                           const uint16_t* __restrict__ phi, float* __restrict__ dst, int W, int H,
+                                           int Krt, int Kp, float eps, int tile_x, int tile_y, int pa, bool has_b,
+                                           size_t phi_plane, size_t phi_row, bool stage_G) {
     const int K = KT > 0 ? KT : Krt;
     const int c = (K - 1) / 2;
     const int SW = (KT > 0 ? KT : Krt) + BX - 1;   // staged tile width (= pitch)
@@ -144,16 +148,12 @@ direct_corr2_kernel(const float* __restrict__ src, const float* __restrict__ G,
     float* sG = smem;                              // [K][Kp]  G transposed: sG[i * Kp + j]
     float2* s = reinterpret_cast<float2*>(smem + ((K * Kp + 1) & ~1));   // [SH][SW] (a, b)
 
-    int t = blockIdx.x;
-    const int tile_x = t % tiles_x; t /= tiles_x;
-    const int tile_y = t % tiles_y; t /= tiles_y;   // t: pair index
-    const int pa = 2 * t;
-    const bool has_b = pa + 1 < n_planes;
     const size_t offa = (size_t)pa * W * H, offb = has_b ? offa + (size_t)W * H : offa;
     const int x0 = tile_x * BX, y0 = tile_y * TILE_H;
     const int tid = threadIdx.y * BX + threadIdx.x;
 
-    for (int k = tid; k < K * Kp; k += BX * BY) sG[k] = G[k];
+    if (stage_G)
+        for (int k = tid; k < K * Kp; k += BX * BY) sG[k] = G[k];
 
     {   // stage the tile with periodic wrap: s[ty][tx] = src(y0 - c + ty, x0 - c + tx) of both planes
         const float* spa = src + offa;
@@ -164,8 +164,9 @@ direct_corr2_kernel(const float* __restrict__ src, const float* __restrict__ G,
             const int gx = pmod(x0 - c + tx, W);
             int gy = pmod(y0 - c + warp, H);
             for (int ty = warp; ty < SH; ty += (BX * BY) / 32) {
-                s[ty * SW + tx] = ty < real_rows ? make_float2(spa[(size_t)gy * W + gx], spb[(size_t)gy * W + gx])
-                                                 : make_float2(0.f, 0.f);
+                const size_t g = (size_t)gy * W + gx;
+                s[ty * SW + tx] = ty >= real_rows ? make_float2(0.f, 0.f)
+                                  : CG ? make_float2(__ldcg(spa + g), __ldcg(spb + g)) : make_float2(spa[g], spb[g]);
                 gy += (BX * BY) / 32;
                 while (gy >= H) gy -= H;
             }
@@ -207,11 +208,184 @@ direct_corr2_kernel(const float* __restrict__ src, const float* __restrict__ G,
                     dst[offa + q] = (float)phi[f] / fmaxf(acc[m].x, eps);
                     if (has_b) dst[offb + q] = (float)phi[f + phi_plane] / fmaxf(acc[m].y, eps);
                 } else {                                                      // a4
-                    dst[offa + q] = dst[offa + q] * acc[m].x;
-                    if (has_b) dst[offb + q] = dst[offb + q] * acc[m].y;
+                    dst[offa + q] = (CG ? __ldcg(dst + offa + q) : dst[offa + q]) * acc[m].x;
+                    if (has_b) dst[offb + q] = (CG ? __ldcg(dst + offb + q) : dst[offb + q]) * acc[m].y;
                 }
             }
         }
+    }
+}
+
+template <int KT, int JC, int MODE>
+__global__ void __launch_bounds__(BX* BY)
+direct_corr2_kernel(const float* __restrict__ src, const float* __restrict__ G,
+                    const uint16_t* __restrict__ phi, float* __restrict__ dst, int W, int H, int Krt,
+                    int Kp, float eps, int tiles_x, int tiles_y, size_t phi_plane, size_t phi_row,
+                    int n_planes) {
+    extern __shared__ __align__(16) float smem[];
+    int t = blockIdx.x;
+    const int tile_x = t % tiles_x; t /= tiles_x;
+    const int tile_y = t % tiles_y; t /= tiles_y;   // t: pair index
+    corr2_tile<KT, JC, MODE>(smem, src, G, phi, dst, W, H, Krt, Kp, eps, tile_x, tile_y, 2 * t,
+                             2 * t + 1 < n_planes, phi_plane, phi_row, true);
+}
+
+// ---------------------------------------------------------------------------------------------
+// Guard of the FFT engine: the plane pairs that the FFT engine flagged as
+// ill-conditioned for fp32 transforms (a pixel with phi_v > 0 whose blur fell below the engine's noise
+// threshold: step a2 then divides by round-off) are recomputed here from scratch, a0..a5, with the direct
+// engine's arithmetic.  ONE persistent cooperative launch per chunk: every CTA reads the flags, returns at
+// once when none is set (the normal case: one empty launch), and otherwise all CTAs share the tiles of the
+// flagged pairs with a grid-wide barrier after every pass (the halo dependency between a2 and a3, and
+// between a4 and the next a1).
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void grid_barrier(unsigned* counter, unsigned target) {
+    __syncthreads();
+    if (threadIdx.x == 0 && threadIdx.y == 0) {
+        __threadfence();
+        atomicAdd(counter, 1u);
+        while (*(volatile unsigned*)counter < target) {}
+        __threadfence();
+    }
+    __syncthreads();
+}
+
+struct RepairArgs {
+    const uint16_t* views;      // view 0 of plane 0 of the chunk
+    ViewLayout lay;
+    float* out;                 // [n_planes][H][W]: psi, iterated in place
+    float* r;                   // ratio scratch, [n_planes][H][W] (the FFT engine's Z buffer, free by now)
+    const float* coef;          // [V][2][K][Kp]
+    const unsigned* flags;      // [pairs]
+    unsigned* barrier;          // zeroed before the launch
+    unsigned* total;            // per-handle count of pairs ever handed over (mvd_guard_flagged)
+    int n_planes, W, H, K, Kp, V, T;
+    float eps;
+};
+
+template <int KT, int JC>
+__global__ void __launch_bounds__(BX* BY) direct_repair_kernel(RepairArgs a) {
+    extern __shared__ __align__(16) float smem[];
+    __shared__ int s_list[512];
+    __shared__ int s_n;
+    const int pairs = (a.n_planes + 1) / 2;
+    const int tid = threadIdx.y * BX + threadIdx.x;
+    if (tid == 0) {
+        int n = 0;
+        for (int p = 0; p < pairs; ++p)
+            if (a.flags[p]) {
+                if (n < 512) s_list[n] = p;
+                ++n;
+            }
+        s_n = n;
+    }
+    __syncthreads();
+    const int nf = s_n < 512 ? s_n : 512;   // more than 512 flagged pairs per chunk cannot happen (chunks hold <= 512 pairs)
+    if (nf == 0) return;
+    if (blockIdx.x == 0 && tid == 0) atomicAdd(a.total, (unsigned)nf);
+
+    const size_t npx = (size_t)a.W * a.H;
+    const int tiles_x = (a.W + BX - 1) / BX, tiles_y = (a.H + TILE_H - 1) / TILE_H;
+    const int tiles = tiles_x * tiles_y;
+    unsigned epoch = 0;
+
+    // a0 on the flagged pairs
+    for (int k = 0; k < nf; ++k) {
+        const int pa = 2 * s_list[k];
+        const int np = pa + 1 < a.n_planes ? 2 : 1;
+        for (size_t q = (size_t)blockIdx.x * (BX * BY) + tid; q < np * npx; q += (size_t)gridDim.x * (BX * BY)) {
+            const size_t pl = q / npx, rem = q % npx;
+            const size_t src = (pa + pl) * a.lay.plane + (rem / a.W) * a.lay.row + rem % a.W;
+            float s = 0.f;
+            for (int v = 0; v < a.V; ++v) s += (float)a.views[(size_t)v * a.lay.view + src];
+            a.out[(size_t)(pa + pl) * npx + rem] = s / (float)a.V;
+        }
+    }
+    grid_barrier(a.barrier, ++epoch * gridDim.x);
+
+    const size_t per = (size_t)a.K * a.Kp;
+    for (int t = 0; t < a.T; ++t)
+        for (int v = 0; v < a.V; ++v) {
+            const float* Gblur = a.coef + ((size_t)v * 2 + 0) * per;
+            const float* Gback = a.coef + ((size_t)v * 2 + 1) * per;
+            const uint16_t* phi = a.views + (size_t)v * a.lay.view;
+            for (int w = blockIdx.x; w < nf * tiles; w += gridDim.x) {
+                const int pa = 2 * s_list[w / tiles], tl = w % tiles;
+                __syncthreads();   // the previous tile's shared memory is no longer read
+                corr2_tile<KT, JC, 0, true>(smem, a.out, Gblur, phi, a.r, a.W, a.H, a.K, a.Kp, a.eps, tl % tiles_x,
+                                      tl / tiles_x, pa, pa + 1 < a.n_planes, a.lay.plane, a.lay.row, true);
+            }
+            grid_barrier(a.barrier, ++epoch * gridDim.x);
+            for (int w = blockIdx.x; w < nf * tiles; w += gridDim.x) {
+                const int pa = 2 * s_list[w / tiles], tl = w % tiles;
+                __syncthreads();
+                corr2_tile<KT, JC, 1, true>(smem, a.r, Gback, nullptr, a.out, a.W, a.H, a.K, a.Kp, a.eps, tl % tiles_x,
+                                      tl / tiles_x, pa, pa + 1 < a.n_planes, 0, 0, true);
+            }
+            grid_barrier(a.barrier, ++epoch * gridDim.x);
+        }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Planes that fit on chip: the WHOLE RL run (a0, T x V view updates, final store) of a plane pair in one CTA
+// and one launch.  psi and r of the pair live in shared memory (4 fp32 planes), every pass stages its wrapped
+// tile from there and runs the same register-blocked FFMA2 correlation as above, so the result is the direct
+// engine's bit for bit; HBM sees the uint16 views and the final psi only ((2 V + 4) B per voxel per step instead
+// of 22 B per voxel-view-iteration), and the 2 V T + 1 launches of the tiled kernels -- which bound small stacks
+// such as config 1 (81 launches of ~4 us on 32 768 voxels) -- become one.
+// ---------------------------------------------------------------------------------------------
+struct SmallArgs {
+    const uint16_t* views;
+    ViewLayout lay;
+    float* out;
+    const float* coef;          // [V][2][K][Kp]
+    int n_planes, W, H, K, Kp, V, T;
+    float eps;
+    int tile_floats;            // floats of the staging area (coefficients + wrapped float2 tile)
+};
+
+template <int KT, int JC>
+__global__ void __launch_bounds__(BX* BY) direct_small_kernel(SmallArgs a) {
+    extern __shared__ __align__(16) float smem[];
+    const size_t npx = (size_t)a.W * a.H;
+    float* psi = smem + a.tile_floats;          // [2][H][W]
+    float* r = psi + 2 * npx;                   // [2][H][W]
+    const int tid = threadIdx.y * BX + threadIdx.x;
+    const int pairs = (a.n_planes + 1) / 2;
+    const int tiles_x = (a.W + BX - 1) / BX, tiles_y = (a.H + TILE_H - 1) / TILE_H;
+    const size_t per = (size_t)a.K * a.Kp;
+    for (int pair = blockIdx.x; pair < pairs; pair += gridDim.x) {
+        const int pa = 2 * pair;
+        const bool has_b = pa + 1 < a.n_planes;
+        const uint16_t* v0 = a.views + (size_t)pa * a.lay.plane;
+        for (size_t q = tid; q < (has_b ? 2 : 1) * npx; q += BX * BY) {      // a0
+            const size_t pl = q / npx, rem = q % npx;
+            const size_t src = pl * a.lay.plane + (rem / a.W) * a.lay.row + rem % a.W;
+            float s = 0.f;
+            for (int v = 0; v < a.V; ++v) s += (float)v0[(size_t)v * a.lay.view + src];
+            psi[q] = s / (float)a.V;
+        }
+        __syncthreads();
+        for (int t = 0; t < a.T; ++t)
+            for (int v = 0; v < a.V; ++v) {
+                const float* Gblur = a.coef + ((size_t)v * 2 + 0) * per;
+                const float* Gback = a.coef + ((size_t)v * 2 + 1) * per;
+                const uint16_t* phi = v0 + (size_t)v * a.lay.view;
+                for (int tl = 0; tl < tiles_x * tiles_y; ++tl) {
+                    if (tl) __syncthreads();      // the staging area is no longer read
+                    corr2_tile<KT, JC, 0>(smem, psi, Gblur, phi, r, a.W, a.H, a.K, a.Kp, a.eps, tl % tiles_x,
+                                          tl / tiles_x, 0, has_b, a.lay.plane, a.lay.row, true);
+                }
+                __syncthreads();
+                for (int tl = 0; tl < tiles_x * tiles_y; ++tl) {
+                    if (tl) __syncthreads();
+                    corr2_tile<KT, JC, 1>(smem, r, Gback, nullptr, psi, a.W, a.H, a.K, a.Kp, a.eps, tl % tiles_x,
+                                          tl / tiles_x, 0, has_b, 0, 0, true);
+                }
+                __syncthreads();
+            }
+        for (size_t q = tid; q < (has_b ? 2 : 1) * npx; q += BX * BY) a.out[(size_t)pa * npx + q] = psi[q];
+        __syncthreads();
     }
 }
 
@@ -288,8 +462,8 @@ int launch_corr(int mode, const mvd_handle* h, const float* src, const float* G,
     // parameter for the config sizes
     if (h->direct_pair) {
 #define MVD_DIRECT_CASE(KT_, JC_)                                                                 \
-    if (h->K == (KT_) && h->JC == (JC_))                                                          \
-        return launch_pair2<KT_, JC_>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp,             \
+    if (h->dK == (KT_) && h->JC == (JC_))                                                         \
+        return launch_pair2<KT_, JC_>(mode, src, G, phi, dst, h->W, h->H, h->dK, h->Kp,            \
                                       h->eps, n_planes, st, phi_plane, phi_row);
         MVD_DIRECT_CASE(9, 9)
         MVD_DIRECT_CASE(21, 7)
@@ -298,10 +472,10 @@ int launch_corr(int mode, const mvd_handle* h, const float* src, const float* G,
         MVD_DIRECT_CASE(51, 17)
 #undef MVD_DIRECT_CASE
         if (h->JC == 8)
-            return launch_pair2<0, 8>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp, h->eps, n_planes, st,
+            return launch_pair2<0, 8>(mode, src, G, phi, dst, h->W, h->H, h->dK, h->Kp, h->eps, n_planes, st,
                                       phi_plane, phi_row);
     }
-    return launch_pair_member<0, 8>(mode, src, G, phi, dst, h->W, h->H, h->K, h->Kp, h->eps,
+    return launch_pair_member<0, 8>(mode, src, G, phi, dst, h->W, h->H, h->dK, h->Kp, h->eps,
                                     n_planes, st, phi_plane, phi_row);
 }
 
@@ -326,7 +500,7 @@ int direct_choose_chunk(int K, int* JC, int* Kp) {
 // Upload both coefficient arrays per view, transposed and zero-padded: G[v][which][i][j], j < Kp.
 // host_xs (nullable): explicit back-projectors X_v, [V][KX][KX].  Step a3 is then the convolution with
 // X_v, i.e. the correlation this kernel computes with the FLIPPED X_v.  Both kernels are laid, centred,
-// into arrays of Kd = max(K, KX) taps (zero outside their support); h->K becomes Kd for this engine.
+// into arrays of Kd = max(K, KX) taps (zero outside their support): h->dK taps.
 int direct_setup(mvd_handle* h, const float* host_psfs, const float* host_xs) {
     const int K0 = h->K, KX = host_xs ? h->KX : h->K;
     const int Kd = K0 > KX ? K0 : KX;
@@ -345,17 +519,17 @@ int direct_setup(mvd_handle* h, const float* host_psfs, const float* host_xs) {
                     pad_b[((size_t)v * Kd + (Kd - 1 - (j + ox))) * Kd + (Kd - 1 - (i + ox))] =
                         host_xs[((size_t)v * KX + j) * KX + i];
     }
-    h->K = Kd;
+    h->dK = Kd;
     host_psfs = pad_p.data();
     const float* host_back = pad_b.data();
-    direct_choose_chunk(h->K, &h->JC, &h->Kp);
+    direct_choose_chunk(h->dK, &h->JC, &h->Kp);
     // two planes per thread whenever the float2 tile fits; the single-plane kernel works in row chunks of 8
-    h->direct_pair = pair_smem_bytes(h->K, h->Kp) <= 227u * 1024u;
+    h->direct_pair = pair_smem_bytes(h->dK, h->Kp) <= 227u * 1024u;
     if (!h->direct_pair) {
         h->JC = 8;
-        h->Kp = (h->K + 7) / 8 * 8;
+        h->Kp = (h->dK + 7) / 8 * 8;
     }
-    const int K = h->K, Kp = h->Kp;
+    const int K = h->dK, Kp = h->Kp;
     const size_t per = (size_t)K * Kp;
     // shared memory needed by one CTA must fit the 227 KB limit
     const size_t smem = sizeof(float) * (per + (size_t)(TILE_H + Kp - 1) * (K + BX - 1));
@@ -377,6 +551,54 @@ int direct_setup(mvd_handle* h, const float* host_psfs, const float* host_xs) {
     return MVD_OK;
 }
 
+namespace {
+size_t small_smem_bytes(const mvd_handle* h) {
+    return pair_smem_bytes(h->dK, h->Kp) + sizeof(float) * 4 * (size_t)h->W * h->H;
+}
+
+template <int KT, int JC>
+int launch_small(const mvd_handle* h, SmallArgs& a, cudaStream_t st) {
+    const size_t smem = small_smem_bytes(h);
+    static size_t opted = 0;
+    auto k = direct_small_kernel<KT, JC>;
+    if (smem > opted) {
+        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return (int)e;
+        opted = smem;
+    }
+    const int pairs = (a.n_planes + 1) / 2;
+    const int per_sm = (int)std::max<size_t>(1, (size_t)(228 * 1024) / (smem + 1024));
+    const int grid = std::min(pairs, h->n_sm * per_sm);
+    k<<<grid, dim3(BX, BY), smem, st>>>(a);
+    return (int)cudaGetLastError();
+}
+}  // namespace
+
+// The on-chip path serves a plan when psi, r (4 fp32 planes of the pair) and the staging tile fit one CTA.
+bool direct_small_available(const mvd_handle* h) {
+    return h->direct_pair && small_smem_bytes(h) <= 227u * 1024u;
+}
+bool direct_small_fits(int W, int H, int K) {
+    int JC, Kp;
+    direct_choose_chunk(K, &JC, &Kp);
+    return pair_smem_bytes(K, Kp) + sizeof(float) * 4 * (size_t)W * H <= 227u * 1024u;
+}
+
+static int direct_run_small(mvd_handle* h, const uint16_t* views, ViewLayout lay, float* out, int n_planes,
+                            cudaStream_t stream) {
+    SmallArgs a;
+    a.views = views; a.lay = lay; a.out = out; a.coef = h->d_coef;
+    a.n_planes = n_planes; a.W = h->W; a.H = h->H; a.K = h->dK; a.Kp = h->Kp; a.V = h->V; a.T = h->T; a.eps = h->eps;
+    a.tile_floats = (int)(pair_smem_bytes(h->dK, h->Kp) / sizeof(float));
+    int e;
+    LaunchScope ls(h, KC_SMALL_RESIDENT, stream);
+    if (h->dK == 9 && h->JC == 9) e = launch_small<9, 9>(h, a, stream);
+    else if (h->dK == 21 && h->JC == 7) e = launch_small<21, 7>(h, a, stream);
+    else if (h->dK == 31 && h->JC == 8) e = launch_small<31, 8>(h, a, stream);
+    else e = launch_small<0, 8>(h, a, stream);
+    return mvd_check(h, (cudaError_t)e);
+}
+
 size_t direct_scratch_bytes(const mvd_handle* h, int n_planes) {
     return sizeof(float) * (size_t)n_planes * h->W * h->H;
 }
@@ -385,6 +607,7 @@ int direct_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout l
                int n_planes, cudaStream_t stream) {
     const size_t npx = (size_t)h->W * h->H;
     const size_t n = npx * n_planes;
+    if (h->T > 0 && direct_small_available(h)) return direct_run_small(h, views, lay, out, n_planes, stream);
     {
         LaunchScope ls(h, KC_INIT_MEAN, stream);
         const int threads = 256;
@@ -397,7 +620,7 @@ int direct_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout l
     int rc = ws_reserve(h, ws, direct_scratch_bytes(h, n_planes), 0);
     if (rc != MVD_OK) return rc;
     float* r = ws.a;
-    const size_t per = (size_t)h->K * h->Kp;
+    const size_t per = (size_t)h->dK * h->Kp;
     for (int t = 0; t < h->T; ++t)
         for (int v = 0; v < h->V; ++v) {
             const float* Gblur = h->d_coef + ((size_t)v * 2 + 0) * per;
@@ -416,4 +639,43 @@ int direct_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout l
             MVD_TRY(h, (cudaError_t)e);
         }
     return MVD_OK;
+}
+
+// ---------------------------------------------------------------------------------------------
+// guard repair (called by the FFT engine after a chunk's last pass)
+// ---------------------------------------------------------------------------------------------
+namespace {
+template <int KT, int JC>
+int launch_repair(const mvd_handle* h, RepairArgs& a, cudaStream_t st) {
+    const size_t smem = pair_smem_bytes(a.K, a.Kp);
+    static size_t opted = 0;
+    auto k = direct_repair_kernel<KT, JC>;
+    if (smem > opted) {
+        cudaError_t e = cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return (int)e;
+        opted = smem;
+    }
+    void* args[] = {&a};
+    // cooperative: all CTAs are resident at once, so the grid-wide barrier cannot deadlock
+    return (int)cudaLaunchCooperativeKernel((void*)k, dim3(h->n_sm), dim3(BX, BY), args, smem, st);
+}
+}  // namespace
+
+bool direct_repair_available(const mvd_handle* h) { return h->d_coef != nullptr && h->direct_pair; }
+
+int direct_repair_launch(mvd_handle* h, const uint16_t* views, ViewLayout lay, float* out, float* r_scratch,
+                         const unsigned* flags, unsigned* barrier, int n_planes, cudaStream_t stream) {
+    RepairArgs a;
+    a.views = views; a.lay = lay; a.out = out; a.r = r_scratch; a.coef = h->d_coef; a.flags = flags;
+    a.barrier = barrier; a.total = h->d_guard_total;
+    a.n_planes = n_planes; a.W = h->W; a.H = h->H; a.K = h->dK; a.Kp = h->Kp; a.V = h->V; a.T = h->T; a.eps = h->eps;
+    int e;
+    LaunchScope ls(h, KC_GUARD_REPAIR, stream);
+    if (h->dK == 9 && h->JC == 9) e = launch_repair<9, 9>(h, a, stream);
+    else if (h->dK == 21 && h->JC == 7) e = launch_repair<21, 7>(h, a, stream);
+    else if (h->dK == 31 && h->JC == 8) e = launch_repair<31, 8>(h, a, stream);
+    else if (h->dK == 41 && h->JC == 7) e = launch_repair<41, 7>(h, a, stream);
+    else if (h->dK == 51 && h->JC == 17) e = launch_repair<51, 17>(h, a, stream);
+    else e = launch_repair<0, 8>(h, a, stream);
+    return mvd_check(h, (cudaError_t)e);
 }

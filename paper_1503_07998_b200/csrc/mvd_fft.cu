@@ -242,15 +242,27 @@ int fft_setup(mvd_handle* h, const float* host_psfs, const float* host_xs) {
                 rc = make_otf_tensor_map(h, fs, h->d_otf_b + (size_t)v * npx, &fs->otf_b_maps[v]);
         }
     }
+    // guard: the direct engine's coefficient arrays for the repair pass (PSFs too large for its two-plane kernel
+    // leave the FFT engine without one: direct_repair_available), and the counter behind mvd_guard_flagged
+    if (rc == MVD_OK) {
+        const int rd = direct_setup(h, host_psfs, host_xs);
+        if (rd != MVD_OK && rd != MVD_ERR_UNSUPPORTED) rc = rd;
+        h->guard_rel = 1.0f / 8192.0f;
+    }
+    if (rc == MVD_OK) rc = mvd_check(h, cudaMalloc((void**)&h->d_guard_total, sizeof(unsigned)));
+    if (rc == MVD_OK) rc = mvd_check(h, cudaMemset(h->d_guard_total, 0, sizeof(unsigned)));
     h->launches = 0;
     return rc;
 }
+
+// Guard words of a chunk of n planes: [pairs] max bits, [pairs] flags, [1] barrier of the repair kernel.
+size_t fft_guard_bytes(int n_planes) { return sizeof(unsigned) * (2 * (size_t)((n_planes + 1) / 2) + 1); }
 
 // Planes per internal pass: bound the two scratch buffers (8 B per voxel) to about 1 GiB.
 int fft_default_chunk(const mvd_handle* h) {
     const size_t npx = (size_t)h->W * h->H;
     size_t c = ((size_t)1 << 30) / (npx * 8);
-    c = std::max<size_t>(2, std::min<size_t>(c, 1 << 20));
+    c = std::max<size_t>(2, std::min<size_t>(c, 1024));   // <= 512 pairs: the repair kernel's list
     return (int)(c & ~(size_t)1);
 }
 
@@ -265,8 +277,10 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay,
     if (((uintptr_t)views & 15u) != 0 || ((lay.view * sizeof(uint16_t)) & 15u) != 0 ||
         ((lay.plane * sizeof(uint16_t)) & 15u) != 0 || ((lay.row * sizeof(uint16_t)) & 15u) != 0)
         return MVD_ERR_INVALID;
-    int rc = ws_reserve(h, ws, bytes, bytes);
+    int rc = ws_reserve(h, ws, bytes, bytes, fft_guard_bytes(n_planes));
     if (rc != MVD_OK) return rc;
+    if (pairs > 512) return MVD_ERR_INVALID;   // chunks are bounded by fft_default_chunk / mvd_set_chunk_planes
+    MVD_TRY(h, cudaMemsetAsync(ws.g, 0, fft_guard_bytes(n_planes), stream));
     CUtensorMap tmap;
     memset(&tmap, 0, sizeof(tmap));
     if (st->col->col_box_h > 0) {
@@ -289,6 +303,9 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay,
     a.eps = h->eps;
     a.final = 0;
     a.total_rows = pairs * H;
+    a.gmax = ws.g;
+    a.gflag = ws.g + pairs;
+    a.guard_rel = h->guard_rel;
 
     const int rp = st->row->row_threads / st->row->row.TPF;          // rows per CTA pass
     const int row_ctas = (a.total_rows + rp - 1) / rp;
@@ -347,5 +364,9 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay,
             }
             if (rc != MVD_OK) return rc;
         }
+    // guard: pairs flagged by the ratio passes are recomputed with the direct engine's arithmetic (one empty
+    // cooperative launch when nothing is flagged); Z is free by now and serves as its ratio scratch
+    if (h->T > 0 && direct_repair_available(h))
+        return direct_repair_launch(h, views, lay, out, ws.a, ws.g + pairs, ws.g + 2 * pairs, n_planes, stream);
     return MVD_OK;
 }

@@ -1,4 +1,7 @@
 // FFT engine, generation-2 (team-synchronous) kernels: 256, 512, 1024, 2048.
+#include <stdio.h>
+#include <stdlib.h>
+
 #include "mvd_fft_v2.cuh"
 using namespace mvdfft;
 
@@ -13,6 +16,21 @@ const SizeOps* mvd_fft_ops_v2(int N) {
     static const SizeOps o2048 = OpsFor2<P2048, 128, P2048, 256, false, 2, false, 4, 3>::make();   // rows: 3 CTAs of 2 teams, 168 registers
     using P800C = Plan<800, 40, 40, 20>;     // columns only: eight columns per team of 160 threads
     static const SizeOps o800 = ColsOnly2<P800C, 160, false, 2, 8>::make();
+#ifdef MVD_DEV
+    {   // experiment variants of a dev build (_work/devbuild.py): MVD_DEV_V<N>=<letter>
+        char name[32];
+        snprintf(name, sizeof name, "MVD_DEV_V%d", N);
+        const char* v = getenv(name);
+        if (v) {
+            if (N == 800 && v[0] == 'a') { static const SizeOps o = ColsOnly2<P800C, 320, false, 1, 8>::make(); return &o; }
+            if (N == 2048 && v[0] == 'a') { static const SizeOps o = OpsFor2<Plan<2048, 16, 16, 16, 8>, 256, P2048, 256, false, 2, false, 4, 3>::make(); return &o; }
+            if (N == 2048 && v[0] == 'b') { static const SizeOps o = OpsFor2<Plan<2048, 16, 16, 16, 8>, 512, P2048, 256, false, 2, false, 4, 2>::make(); return &o; }
+            if (N == 1024 && v[0] == 'a') { static const SizeOps o = OpsFor2<P1024, 256, Plan<1024, 16, 16, 16, 4>, 256, false, 2>::make(); return &o; }
+            if (N == 512 && v[0] == 'a') { static const SizeOps o = OpsFor2<P512, 256, Plan<512, 16, 16, 8, 4>, 128, false, 5>::make(); return &o; }
+            if (N == 512 && v[0] == 'b') { static const SizeOps o = OpsFor2<P512, 256, Plan<512, 16, 16, 16, 2>, 128, false, 5>::make(); return &o; }
+        }
+    }
+#endif
     switch (N) {
         case 256: return &o256;
         case 512: return &o512;

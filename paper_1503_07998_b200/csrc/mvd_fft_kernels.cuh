@@ -472,7 +472,19 @@ struct RowArgs {
     int final;               // ROWS_UPDATE: last update -> write `out`, skip the forward FFT
                              // ROWS_FIRST : iterations == 0 -> write `out` only
     int total_rows;          // pairs * H
+    // guard: ROWS_FIRST records max(psi_0) of every pair (float bits; psi_0 >= 0), ROWS_RATIO flags
+    // the pairs in which some pixel has phi_v > 0 and blur < guard_rel * that maximum
+    unsigned* gmax;          // [pairs]
+    unsigned* gflag;         // [pairs]
+    float guard_rel;
 };
+
+// ROWS_FIRST: fold this thread's maximum of psi_0 into the pair's word.  The plain read is only a filter
+// (a stale value costs an extra atomic, never a wrong result).
+__device__ __forceinline__ void guard_note_max(unsigned* gmax, int pair, float m) {
+    const unsigned bits = __float_as_uint(m);
+    if (bits > *(volatile unsigned*)(gmax + pair)) atomicMax(gmax + pair, bits);
+}
 
 template <class P, int MODE, int NT>
 __global__ void __launch_bounds__(NT) fft_rows_kernel(RowArgs a, const float2* __restrict__ tw_g) {
@@ -499,6 +511,7 @@ __global__ void __launch_bounds__(NT) fft_rows_kernel(RowArgs a, const float2* _
         float2 x[E];
 
         if (MODE == ROWS_FIRST) {
+            float gm = 0.f;
 #pragma unroll
             for (int e = 0; e < E; ++e) {
                 const int pos = t + TPF * e;
@@ -510,6 +523,7 @@ __global__ void __launch_bounds__(NT) fft_rows_kernel(RowArgs a, const float2* _
                         if (has_b) sb += (float)__ldg(vp + vxb + pos);
                     }
                 x[e] = make_float2(sa / (float)a.V, sb / (float)a.V);       // a0
+                gm = fmaxf(gm, fmaxf(x[e].x, x[e].y));
                 if (valid) {
                     if (a.final) {
                         a.out[pxa + pos] = x[e].x;
@@ -520,6 +534,7 @@ __global__ void __launch_bounds__(NT) fft_rows_kernel(RowArgs a, const float2* _
                 }
             }
             if (a.final) continue;   // uniform over the block
+            if (valid) guard_note_max(a.gmax, pair, gm);
         } else {
             uint32_t ph[E];          // phi_a | phi_b << 16, fetched before the inverse transform
             if (MODE == ROWS_RATIO) {
@@ -659,14 +674,18 @@ __global__ void __launch_bounds__(NT) fft_rows_tma_kernel(RowArgs a, const float
         fft_run<P, +1>(x, buf, tw, t, addr);
         if (MODE == ROWS_RATIO) {
             const uint16_t* pa = reinterpret_cast<const uint16_t*>(ax);
+            const float tau = a.guard_rel * __uint_as_float(a.gmax[pair]);
+            float bmin = 3.0e38f;
 #pragma unroll
             for (int e = 0; e < E; ++e) {                                 // a2
                 const int pos = t + TPF * e;
                 const float fa = valid ? (float)pa[pos] : 0.f;
                 const float fb = (valid && has_b) ? (float)pa[W + pos] : 0.f;
+                bmin = fminf(bmin, fminf(fa > 0.f ? x[e].x : 3.0e38f, fb > 0.f ? x[e].y : 3.0e38f));
                 x[e].x = __fdividef(fa, fmaxf(x[e].x, a.eps));
                 x[e].y = __fdividef(fb, fmaxf(x[e].y, a.eps));
             }
+            if (bmin < tau) a.gflag[pair] = 1u;
         } else {
             const float2* zr = reinterpret_cast<const float2*>(ax);
 #pragma unroll

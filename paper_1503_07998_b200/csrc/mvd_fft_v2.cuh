@@ -141,8 +141,13 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
                 }
             }
             const float fv = (float)a.V;
+            float gm = 0.f;
 #pragma unroll
-            for (int e = 0; e < E; ++e) x[e] = make_float2(x[e].x / fv, x[e].y / fv);       // a0
+            for (int e = 0; e < E; ++e) {
+                x[e] = make_float2(x[e].x / fv, x[e].y / fv);       // a0
+                gm = fmaxf(gm, fmaxf(x[e].x, x[e].y));
+            }
+            if (valid && !a.final) guard_note_max(a.gmax, pair, gm);
             if (a.final) {   // iterations == 0: the mean is the result (uniform over the grid)
 #pragma unroll
                 for (int e = 0; e < E; ++e) {
@@ -187,12 +192,17 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
             sync();
             if (MODE == ROWS_RATIO) {
                 const uint16_t* lu = reinterpret_cast<const uint16_t*>(land);
+                const float tau = a.guard_rel * __uint_as_float(a.gmax[pair]);
+                float bmin = 3.0e38f;    // smallest blur at a pixel that holds photons (guard)
 #pragma unroll
                 for (int e = 0; e < E; ++e) {                                 // a2
                     const int pos = t + TPF * e;
-                    x[e].x = __fdividef((float)lu[pos], fmaxf(x[e].x, a.eps));
-                    x[e].y = __fdividef((float)lu[W + pos], fmaxf(x[e].y, a.eps));
+                    const float fa = (float)lu[pos], fb = (float)lu[W + pos];
+                    bmin = fminf(bmin, fminf(fa > 0.f ? x[e].x : 3.0e38f, fb > 0.f ? x[e].y : 3.0e38f));
+                    x[e].x = __fdividef(fa, fmaxf(x[e].x, a.eps));
+                    x[e].y = __fdividef(fb, fmaxf(x[e].y, a.eps));
                 }
+                if (valid && bmin < tau) a.gflag[pair] = 1u;
                 sync();
             } else {
 #pragma unroll

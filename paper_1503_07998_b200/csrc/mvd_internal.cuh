@@ -17,9 +17,11 @@ enum KernelClass {
     KC_FFT_COLS,             // column FFT . OTF . inverse column FFT (a1 / a3 middle part)
     KC_FFT_ROWS_RATIO,       // inverse row FFT -> b, a2 ratio, forward row FFT of r
     KC_FFT_ROWS_UPDATE,      // inverse row FFT -> q, a4 update, forward row FFT of the new psi
-    KC_SETUP                 // mvd_create-time kernels (OTF construction)
+    KC_SETUP,                // mvd_create-time kernels (OTF construction)
+    KC_GUARD_REPAIR,         // FFT engine's guard: flagged plane pairs recomputed with the direct engine's arithmetic
+    KC_SMALL_RESIDENT        // whole RL run of a small plane pair on chip, one launch
 };
-static_assert(KC_SETUP + 1 == MVD_N_KERNEL_CLASSES, "kernel class table and mvd.h disagree");
+static_assert(KC_SMALL_RESIDENT + 1 == MVD_N_KERNEL_CLASSES, "kernel class table and mvd.h disagree");
 
 struct ProfRecord {
     int kc;
@@ -31,6 +33,8 @@ struct Workspace {
     float* a = nullptr;      // direct: r [chunk][H][W];   fft: Z (psi pairs, float2 [pairs][H][W])
     float* b = nullptr;      // direct: unused;            fft: S (spectrum, float2 [pairs][H][W])
     size_t a_bytes = 0, b_bytes = 0;
+    unsigned* g = nullptr;   // fft: guard words of the chunk in flight: [pairs] max bits of psi_0, [pairs] flags, [1] barrier
+    size_t g_bytes = 0;
 };
 
 struct mvd_handle {
@@ -43,6 +47,7 @@ struct mvd_handle {
     // direct path: per view two coefficient arrays, transposed and row-padded: G[v][which][K][Kp]
     // which = 0: blur (flipped PSF), 1: back-projection (PSF as given)
     float* d_coef = nullptr;
+    int dK = 0;   // taps per axis of the direct engine's coefficient arrays: max(K, KX)
     int Kp = 0;   // padded number of PSF rows (multiple of the kernel's row chunk)
     int JC = 0;   // row chunk of the direct kernel chosen for K
     bool direct_pair = false;   // the two-plane FFMA2 kernel serves this plan (its float2 tile fits in shared memory)
@@ -52,6 +57,10 @@ struct mvd_handle {
     float2* d_otf_b = nullptr;   // explicit back-projectors' transfer functions (nullptr: a3 uses conj d_otf)
     int KX = 0;                  // size of the caller's back-projectors (0: Independent variant, X = P_v^*)
     void* fft = nullptr;   // FftState (mvd_fft.cu)
+    // fft path, guard: plane pairs with a pixel phi_v > 0 whose blur is below guard_rel x max(psi_0)
+    // are recomputed by direct_repair_launch; d_guard_total counts them over the handle's life
+    float guard_rel = 0.f;
+    unsigned* d_guard_total = nullptr;
 
     Workspace ws_main;
     // host pipeline (mvd_deconvolve_host): three slots, one stream each
@@ -102,7 +111,7 @@ int mvd_check(mvd_handle* h, cudaError_t e);
         if (rc__ != MVD_OK) return rc__;        \
     } while (0)
 
-int ws_reserve(mvd_handle* h, Workspace& ws, size_t a_bytes, size_t b_bytes);
+int ws_reserve(mvd_handle* h, Workspace& ws, size_t a_bytes, size_t b_bytes, size_t g_bytes = 0);
 
 // ---- direct path (mvd_direct.cu) ------------------------------------------------------------
 int direct_choose_chunk(int K, int* JC, int* Kp);
@@ -112,10 +121,17 @@ size_t direct_scratch_bytes(const mvd_handle* h, int n_planes);
 int direct_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay, float* out,
                int n_planes, cudaStream_t stream);
 
+bool direct_small_available(const mvd_handle* h);
+bool direct_small_fits(int W, int H, int K);
+bool direct_repair_available(const mvd_handle* h);
+int direct_repair_launch(mvd_handle* h, const uint16_t* views, ViewLayout lay, float* out, float* r_scratch,
+                         const unsigned* flags, unsigned* barrier, int n_planes, cudaStream_t stream);
+
 // ---- fft path (mvd_fft.cu) --------------------------------------------------------------------
 int fft_supported(int W, int H);
 int fft_setup(mvd_handle* h, const float* host_psfs, const float* host_xs);
 int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay, float* out,
             int n_planes, cudaStream_t stream);
 int fft_default_chunk(const mvd_handle* h);
+size_t fft_guard_bytes(int n_planes);
 void fft_teardown(mvd_handle* h);

@@ -36,7 +36,8 @@ def _name(path):
 @pytest.mark.parametrize("T", [1, 3])
 def test_centred_delta_with_zero_pixels(path, T):
     """P1 with zeros: 0 / max(0, eps) = 0 and psi stays phi.  Bit-exact on the direct engine; the FFT engine
-    returns exact zeros where phi == 0 (0 . q) and phi to rounding elsewhere."""
+    returns exact zeros where phi == 0 (0 . q) and phi elsewhere up to its transform round-off, which is relative
+    to the plane's MAXIMUM (fp32 FFT: ~1e-7 x 65535 on every pixel), not to the pixel."""
     W, H, N = 64, 32, 3
     views = synth.random_views(1, N, W, H, seed=41, lo=0, hi=65536)
     views[0, 0, :7, :9] = 0
@@ -49,7 +50,7 @@ def test_centred_delta_with_zero_pixels(path, T):
         assert np.array_equal(out, want.astype(np.float32))
     else:
         assert (out[want == 0] == 0).all()
-        np.testing.assert_allclose(out, want, rtol=2e-5)
+        np.testing.assert_allclose(out, want, rtol=2e-5, atol=4e-7 * 65535)
 
 
 @pytest.mark.parametrize("path", PATHS)
@@ -82,20 +83,53 @@ def test_zero_background_blocks_in_every_view(path, psf):
     assert_parity(out, ref, f"zero background {psf} {_name(path)}")
 
 
+def _missing_view_problem():
+    V, N, W, H, K, T = 2, 6, 128, 64, 9, 3
+    pr = synth.make_problem(V, N, W, H, K, T, seed=4400, psf="gauss")
+    views = pr.views.copy()
+    views[0, 1:3, 16:48, 40:100] = 0          # planes 1 and 2: pairs (0, 1) and (2, 3) are hit, pair (4, 5) is not
+    return views, pr.psfs, T, pr.eps
+
+
 @pytest.mark.parametrize("path", PATHS)
 def test_view_that_is_zero_where_the_others_are_not(path):
     """View 0 is zero-filled in a block (a registered view that does not cover it) where view 1 has signal:
     view 0's update drives psi to 0 inside the block, view 1 then finds phi > 0 with b < eps at the pixels the
     PSF cannot reach from outside.  The direct engine keeps this local, like the oracle.  On the FFT engine the
-    ratio plane then holds values of phi / eps ~ 1e9 whose fp32 transform round-off (~1e2) reaches every pixel of
-    the plane: the engine detects such planes and hands them to the direct engine."""
-    V, N, W, H, K, T = 2, 4, 128, 64, 9, 3
-    pr = synth.make_problem(V, N, W, H, K, T, seed=4400, psf="gauss")
-    views = pr.views.copy()
-    views[0, 1:3, 16:48, 40:100] = 0
-    ref = mvd_oracle.deconvolve(views, pr.psfs, T, pr.eps)
-    out = _run(views, pr.psfs, T, path)
+    ratio plane would hold values of phi / eps ~ 1e9 whose fp32 transform round-off (~1e2) reaches every pixel of
+    the plane PAIR (measured without the guard: output ~1e20): the engine flags such pairs and recomputes them
+    with the direct engine's arithmetic."""
+    views, psfs, T, eps = _missing_view_problem()
+    ref = mvd_oracle.deconvolve(views, psfs, T, eps)
+    out = _run(views, psfs, T, path)
     assert_parity(out, ref, f"missing view block {_name(path)}")
+
+
+def test_fft_guard_hands_over_exactly_the_ill_conditioned_pairs():
+    """The guard flags pairs (0, 1) and (2, 3) of the case above and leaves pair (4, 5) to the FFT engine; the
+    handed-over planes carry the direct engine's bits; ordinary stacks (config 2's planes) flag nothing."""
+    import torch
+    views, psfs, T, eps = _missing_view_problem()
+    V, N, H, W = views.shape
+    direct = _run(views, psfs, T, binding.PATH_DIRECT)
+    with binding.Mvd(W, H, V, psfs, psfs.shape[-1], T, eps, binding.PATH_FFT) as m:
+        dv = torch.from_numpy(views.view(np.int16)).cuda()
+        do = torch.empty((N, H, W), dtype=torch.float32, device="cuda")
+        m.deconvolve_planes(dv, do, N)
+        assert m.guard_flagged() == 2
+        out = do.cpu().numpy()
+        assert np.array_equal(out[:4], direct[:4])
+        assert not np.array_equal(out[4:], direct[4:])           # the untouched pair is the FFT engine's result
+        m.deconvolve_planes(dv, do, N)                           # the counter accumulates over calls
+        assert m.guard_flagged() == 4
+        assert np.array_equal(do.cpu().numpy(), out)
+    cfg = synth.config(2)
+    cpsfs, cviews = synth.config_psfs(2), synth.views(cfg, [0, 1, 300, 301])
+    with binding.Mvd(cfg.W, cfg.H, cfg.V, cpsfs, cfg.K, cfg.T, cfg.eps, binding.PATH_FFT) as m:
+        dv = torch.from_numpy(cviews.view(np.int16)).cuda()
+        do = torch.empty((4, cfg.H, cfg.W), dtype=torch.float32, device="cuda")
+        m.deconvolve_planes(dv, do, 4)
+        assert m.guard_flagged() == 0
 
 
 @pytest.mark.parametrize("path", PATHS)

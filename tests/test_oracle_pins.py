@@ -385,3 +385,83 @@ def test_backprojector_builders_arithmetic():
     np.testing.assert_allclose(out, 777.0, rtol=1e-5)
     with pytest.raises(ValueError):
         orc.backprojectors(psfs, "optimization2")
+
+
+# ---------------------------------------------------------------------------------------------
+# Per-view weights (mvd_oracle_w; PAPER.md:88 lists a "weights" buffer and never defines it).
+# READING W1 (parity unpinned): a4 becomes psi <- psi . (w_v q + 1 - w_v).
+# What is pinned here is the arithmetic of that reading and the cases any reading must satisfy.
+# ---------------------------------------------------------------------------------------------
+def test_PW1_unit_weights_are_the_unweighted_run_bit_for_bit():
+    views = synth.random_views(3, 2, 14, 10, seed=201)
+    psfs = rand_psfs(3, 5, 202)
+    a = orc.deconvolve(views, psfs, 4)
+    b = orc.deconvolve(views, psfs, 4, weights=np.ones(views.shape, np.float32))
+    assert np.array_equal(a, b)
+    c = orc.deconvolve(views, psfs, 4, weights=np.ones(views.shape, np.float32), literal=True)
+    assert np.array_equal(a, c)
+
+
+def test_PW2_a_view_with_zero_weight_is_never_applied():
+    # all weights zero: nothing is ever applied, psi stays the mean of the views
+    views = synth.random_views(2, 2, 12, 9, seed=203)
+    psfs = rand_psfs(2, 5, 204)
+    out = orc.deconvolve(views, psfs, 5, weights=np.zeros(views.shape, np.float32))
+    assert np.array_equal(out, views.astype(np.float64).sum(0) / 2)
+    # two identical views, the second with weight 0: psi_0 = phi, and the run is the single-view run
+    one = synth.random_views(1, 2, 12, 9, seed=205)
+    two = np.concatenate([one, one])
+    P = rand_psfs(1, 5, 206)
+    w = np.ones(two.shape, np.float32)
+    w[1] = 0.0
+    assert np.array_equal(orc.deconvolve(two, np.concatenate([P, P]), 4, weights=w), orc.deconvolve(one, P, 4))
+    # a pixel mask: pixels whose weight is 0 in every view keep psi_0 for ever, the others move
+    views = synth.random_views(2, 1, 12, 9, seed=207)
+    w = np.ones(views.shape, np.float32)
+    w[:, 0, 2:5, 3:8] = 0.0
+    out = orc.deconvolve(views, psfs, 3, weights=w)[0]
+    psi0 = views[:, 0].astype(np.float64).sum(0) / 2
+    assert np.array_equal(out[2:5, 3:8], psi0[2:5, 3:8])
+    assert not np.allclose(out[6:, :], psi0[6:, :], rtol=1e-3)
+
+
+def test_PW3_constants_stay_fixed_under_any_weights():
+    views = np.full((2, 1, 10, 8), 321, dtype=np.uint16)
+    rng = np.random.default_rng(208)
+    w = rng.random(views.shape).astype(np.float32)
+    out = orc.deconvolve(views, rand_psfs(2, 5, 209), 6, weights=w)
+    np.testing.assert_allclose(out, 321.0, rtol=1e-12)
+
+
+@pytest.mark.parametrize("W,H,K", [(8, 8, 3), (12, 8, 5), (6, 5, 9)])
+def test_PW4_dense_matrix_brute_force_with_random_weights(W, H, K):
+    V, T = 3, 4
+    views = synth.random_views(V, 2, W, H, seed=210 + K)
+    psfs = rand_psfs(V, K, 211 + W)
+    rng = np.random.default_rng(212)
+    w = rng.random(views.shape).astype(np.float32)
+    w[0, :, :2] = 0.0
+    w[1, :, -2:] = 1.0
+    out = orc.deconvolve(views, psfs, T, weights=w)
+    eps = float(np.float32(1e-6))
+    for p in range(2):
+        phi = views[:, p].reshape(V, -1).astype(np.float64)
+        psi = phi.sum(0) / V
+        ops = [dense_operator(psfs[v], H, W) for v in range(V)]
+        for _ in range(T):
+            for v in range(V):
+                q = ops[v].T @ (phi[v] / np.maximum(ops[v] @ psi, eps))
+                wv = w[v, p].reshape(-1).astype(np.float64)
+                psi = psi * (wv * q + (1.0 - wv))
+        np.testing.assert_allclose(out[p], psi.reshape(H, W), rtol=1e-11, atol=1e-11)
+
+
+def test_PW_argument_validation():
+    views = synth.random_views(1, 1, 8, 8, seed=213)
+    w = np.ones(views.shape, np.float32)
+    w[0, 0, 0, 0] = 1.5
+    with pytest.raises(ValueError):
+        orc.deconvolve(views, synth.delta_psf(3)[None], 1, weights=w)
+    w[0, 0, 0, 0] = np.nan
+    with pytest.raises(ValueError):
+        orc.deconvolve(views, synth.delta_psf(3)[None], 1, weights=w)
