@@ -154,6 +154,46 @@ MVD_API int mvd_deconvolve_host_camera(mvd_handle* h, const uint16_t* host_frame
                                int n_planes);
 
 /*
+ * The general form of both calls: one request structure instead of one entry point per combination.
+ *   views          as in mvd_deconvolve_planes (DEVICE) / mvd_deconvolve_host (HOST, pinned for overlap).
+ *   view_stride, plane_stride, row_stride
+ *                  all 0: dense uint16 [n_views][n_planes][plane_h][plane_w]; otherwise the strided layout of
+ *                  mvd_deconvolve_planes_strided (device calls only).
+ *   weights        NULL, or float [n_views][n_planes][plane_h][plane_w] in the same memory space as `views`:
+ *                  per-view, per-pixel weights in [0, 1] (PAPER.md:88 lists "weights, float, 4 v bytes/pixel" and
+ *                  never defines them; READING W1 of DESIGN.md section 2): step a4 becomes
+ *                      psi <- psi . (w_v q + (1 - w_v)),
+ *                  so w_v = 1 is the unweighted update bit for bit and w_v = 0 leaves the pixel untouched by view
+ *                  v (a registered view that does not cover it).  Values outside [0, 1] are not checked.
+ *   out, out_type  MVD_OUT_F32: float [n_planes][plane_h][plane_w] (as above);
+ *                  MVD_OUT_U16: uint16_t, same shape: psi rounded to nearest (ties to even) and saturated at
+ *                  65535 in the final store (the data are uint16) -- halves the output and its D2H copy.
+ *   camera_order   mvd_deconvolve_host_ex only: non-zero = `views` is [n_views][plane_h][n_planes][plane_w] as in
+ *                  mvd_deconvolve_host_camera (weights and output stay plane-major).
+ * Everything else (asynchrony, ownership, errors) as for mvd_deconvolve_planes / mvd_deconvolve_host.
+ */
+enum { MVD_OUT_F32 = 0, MVD_OUT_U16 = 1 };
+typedef struct mvd_io {
+    const uint16_t* views;
+    size_t view_stride, plane_stride, row_stride;
+    const float* weights;
+    void* out;
+    int out_type;
+    int camera_order;
+} mvd_io;
+MVD_API int mvd_deconvolve_planes_ex(mvd_handle* h, const mvd_io* io, int n_planes, void* stream);
+MVD_API int mvd_deconvolve_host_ex(mvd_handle* h, const mvd_io* io, int n_planes);
+
+/* Shorthands: per-view weights and uint16 output. */
+MVD_API int mvd_deconvolve_planes_weighted(mvd_handle* h, const uint16_t* dev_views_u16, const float* dev_weights_f32,
+                                           float* dev_out_f32, int n_planes, void* stream);
+MVD_API int mvd_deconvolve_host_weighted(mvd_handle* h, const uint16_t* host_views_u16, const float* host_weights_f32,
+                                         float* host_out_f32, int n_planes);
+MVD_API int mvd_deconvolve_planes_u16(mvd_handle* h, const uint16_t* dev_views_u16, uint16_t* dev_out_u16,
+                                      int n_planes, void* stream);
+MVD_API int mvd_deconvolve_host_u16(mvd_handle* h, const uint16_t* host_views_u16, uint16_t* host_out_u16, int n_planes);
+
+/*
  * mvd_reserve -- size everything a later call on up to max_planes planes needs (scratch of the engine, the
  * internal streams and events, the pipeline's device slots) now.  After it, mvd_deconvolve_planes* with
  * n_planes <= max_planes only enqueues: no allocation, no synchronisation, so the call can be captured into a

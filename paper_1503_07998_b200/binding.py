@@ -52,6 +52,25 @@ SIGNATURES = {
     "mvd_measure_fp32_peak": (_i, [ctypes.POINTER(ctypes.c_double), ctypes.POINTER(ctypes.c_double)]),
 }
 
+
+
+class MvdIO(ctypes.Structure):
+    """struct mvd_io of include/mvd.h."""
+    _fields_ = [("views", _vp), ("view_stride", ctypes.c_size_t), ("plane_stride", ctypes.c_size_t),
+                ("row_stride", ctypes.c_size_t), ("weights", _vp), ("out", _vp), ("out_type", _i),
+                ("camera_order", _i)]
+
+
+OUT_F32, OUT_U16 = 0, 1
+SIGNATURES.update({
+    "mvd_deconvolve_planes_ex": (_i, [_vp, ctypes.POINTER(MvdIO), _i, _vp]),
+    "mvd_deconvolve_host_ex": (_i, [_vp, ctypes.POINTER(MvdIO), _i]),
+    "mvd_deconvolve_planes_weighted": (_i, [_vp, _vp, _vp, _vp, _i, _vp]),
+    "mvd_deconvolve_host_weighted": (_i, [_vp, _vp, _vp, _vp, _i]),
+    "mvd_deconvolve_planes_u16": (_i, [_vp, _vp, _vp, _i, _vp]),
+    "mvd_deconvolve_host_u16": (_i, [_vp, _vp, _vp, _i]),
+})
+
 _lib: Optional[ctypes.CDLL] = None
 
 
@@ -150,6 +169,35 @@ class Mvd:
         rc = lib().mvd_deconvolve_host_camera(self._h, _ptr(host_frames_u16), _ptr(host_out_f32), n_planes)
         if rc != MVD_OK:
             self._raise(rc, "mvd_deconvolve_host_camera")
+
+    def deconvolve_planes_ex(self, views, out, n_planes: int, stream=None, weights=None, out_u16: bool = False,
+                             strides: Tuple[int, int, int] = (0, 0, 0)) -> None:
+        io = MvdIO(_ptr(views), strides[0], strides[1], strides[2], _ptr(weights), _ptr(out),
+                   OUT_U16 if out_u16 else OUT_F32, 0)
+        self._raise(lib().mvd_deconvolve_planes_ex(self._h, ctypes.byref(io), n_planes, _stream(stream)),
+                    "mvd_deconvolve_planes_ex")
+
+    def deconvolve_host_ex(self, views, out, n_planes: int, weights=None, out_u16: bool = False,
+                           camera_order: bool = False) -> None:
+        io = MvdIO(_ptr(views), 0, 0, 0, _ptr(weights), _ptr(out), OUT_U16 if out_u16 else OUT_F32, int(camera_order))
+        self._raise(lib().mvd_deconvolve_host_ex(self._h, ctypes.byref(io), n_planes), "mvd_deconvolve_host_ex")
+
+    def deconvolve_planes_weighted(self, dev_views_u16, dev_weights_f32, dev_out_f32, n_planes: int, stream=None) -> None:
+        self._raise(lib().mvd_deconvolve_planes_weighted(self._h, _ptr(dev_views_u16), _ptr(dev_weights_f32),
+                                                         _ptr(dev_out_f32), n_planes, _stream(stream)),
+                    "mvd_deconvolve_planes_weighted")
+
+    def deconvolve_host_weighted(self, host_views_u16, host_weights_f32, host_out_f32, n_planes: int) -> None:
+        self._raise(lib().mvd_deconvolve_host_weighted(self._h, _ptr(host_views_u16), _ptr(host_weights_f32),
+                                                       _ptr(host_out_f32), n_planes), "mvd_deconvolve_host_weighted")
+
+    def deconvolve_planes_u16(self, dev_views_u16, dev_out_u16, n_planes: int, stream=None) -> None:
+        self._raise(lib().mvd_deconvolve_planes_u16(self._h, _ptr(dev_views_u16), _ptr(dev_out_u16), n_planes,
+                                                    _stream(stream)), "mvd_deconvolve_planes_u16")
+
+    def deconvolve_host_u16(self, host_views_u16, host_out_u16, n_planes: int) -> None:
+        self._raise(lib().mvd_deconvolve_host_u16(self._h, _ptr(host_views_u16), _ptr(host_out_u16), n_planes),
+                    "mvd_deconvolve_host_u16")
 
     def deconvolve_host(self, host_views_u16, host_out_f32, n_planes: int) -> None:
         """host buffers: pinned torch tensors, numpy arrays or raw host pointers.  Blocks."""
@@ -263,7 +311,7 @@ def build_backprojectors(variant: int, psfs: np.ndarray) -> np.ndarray:
 def deconvolve(views: np.ndarray, psfs: np.ndarray, iterations: int, eps: float = 1e-6,
                path: Optional[int] = None, host: bool = False, chunk_planes: int = 0,
                batch_planes: int = 0, backprojectors: Optional[np.ndarray] = None,
-               resident_streams: int = 0) -> np.ndarray:
+               resident_streams: int = 0, weights: Optional[np.ndarray] = None, out_u16: bool = False) -> np.ndarray:
     """Convenience for tests: numpy uint16 `[V][N][H][W]` in, numpy float32 `[N][H][W]` out, through
     mvd_deconvolve_planes (host=False) or mvd_deconvolve_host (host=True, pinned buffers)."""
     import torch
@@ -280,13 +328,25 @@ def deconvolve(views: np.ndarray, psfs: np.ndarray, iterations: int, eps: float 
         if resident_streams:
             m.set_resident_streams(resident_streams)
         tv = torch.from_numpy(views.view(np.int16))
+        tw = None if weights is None else torch.from_numpy(np.ascontiguousarray(weights, dtype=np.float32))
+        odt = torch.int16 if out_u16 else torch.float32
         if host:
             hv = tv.pin_memory()
-            ho = torch.empty((N, H, W), dtype=torch.float32).pin_memory()
-            m.deconvolve_host(hv, ho, N)
-            return ho.numpy().copy()
-        dv = tv.cuda()
-        do = torch.empty((N, H, W), dtype=torch.float32, device="cuda")
-        m.deconvolve_planes(dv, do, N)
-        torch.cuda.synchronize()
-        return do.cpu().numpy()
+            hw = None if tw is None else tw.pin_memory()
+            ho = torch.empty((N, H, W), dtype=odt).pin_memory()
+            if tw is None and not out_u16:
+                m.deconvolve_host(hv, ho, N)
+            else:
+                m.deconvolve_host_ex(hv, ho, N, weights=hw, out_u16=out_u16)
+            res = ho.numpy().copy()
+        else:
+            dv = tv.cuda()
+            dw = None if tw is None else tw.cuda()
+            do = torch.empty((N, H, W), dtype=odt, device="cuda")
+            if tw is None and not out_u16:
+                m.deconvolve_planes(dv, do, N)
+            else:
+                m.deconvolve_planes_ex(dv, do, N, weights=dw, out_u16=out_u16)
+            torch.cuda.synchronize()
+            res = do.cpu().numpy()
+        return res.view(np.uint16) if out_u16 else res

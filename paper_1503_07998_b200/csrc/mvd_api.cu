@@ -93,9 +93,10 @@ int mvd_path_supported(int path, int plane_w, int plane_h, int psf_size) {
 static int choose_path(int W, int H, int K) {
     const bool fft_ok = mvd_path_supported(MVD_PATH_FFT, W, H, K) != 0;
     const bool dir_ok = mvd_path_supported(MVD_PATH_DIRECT, W, H, K) != 0;
-    // planes small enough to stay on chip for the whole run (one launch) beat the FFT engine's
-    // 4 V T + 1 launches up to K ~ 9; everywhere else the FFT engine wins at every K, even K = 3 (section 7)
-    if (dir_ok && K <= 9 && direct_small_fits(W, H, K)) return MVD_PATH_DIRECT;
+    // Measured: the FFT engine wins at every K, even K = 3, on large stacks; on config 1 its
+    // 81 short launches (0.41 ms) still beat the direct engine's one-launch on-chip kernel (0.50 ms), which keeps
+    // only one SM per plane pair busy.
+    (void)K;
     if (fft_ok) return MVD_PATH_FFT;
     if (dir_ok) return MVD_PATH_DIRECT;
     return -1;
@@ -233,6 +234,7 @@ void mvd_destroy(mvd_handle* h) {
         ws_free(h->ws_slot[s]);
         if (h->d_in[s]) cudaFree(h->d_in[s]);
         if (h->d_out[s]) cudaFree(h->d_out[s]);
+        if (h->d_w[s]) cudaFree(h->d_w[s]);
         if (h->streams[s]) cudaStreamDestroy(h->streams[s]);
         if (h->ev_join[s]) cudaEventDestroy(h->ev_join[s]);
     }
@@ -262,16 +264,14 @@ static int default_chunk(const mvd_handle* h) {
     return (int)std::max<size_t>(1, std::min<size_t>(c, 1 << 20));
 }
 
-// All T iterations on planes [0, n) of `views`, in chunks (each chunk runs to completion).
-static int run_core(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay,
-                    float* out, int n_planes, cudaStream_t stream) {
+// All T iterations on planes [0, n) of `io`, in chunks (each chunk runs to completion).
+static int run_core(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cudaStream_t stream) {
     const size_t npx = (size_t)h->W * h->H;
     const int chunk = default_chunk(h);
     for (int p0 = 0; p0 < n_planes; p0 += chunk) {
         const int n = std::min(chunk, n_planes - p0);
-        int rc = h->path == MVD_PATH_FFT
-                     ? fft_run(h, ws, views + (size_t)p0 * lay.plane, lay, out + (size_t)p0 * npx, n, stream)
-                     : direct_run(h, ws, views + (size_t)p0 * lay.plane, lay, out + (size_t)p0 * npx, n, stream);
+        const PlaneIO sub = io.at(p0, npx);
+        int rc = h->path == MVD_PATH_FFT ? fft_run(h, ws, sub, n, stream) : direct_run(h, ws, sub, n, stream);
         if (rc != MVD_OK) return rc;
     }
     return MVD_OK;
@@ -338,14 +338,13 @@ int mvd_get_batch_planes(const mvd_handle* h, int n_planes) {
     return default_batch(h, n_planes);
 }
 
-// Device-resident work on `lay`: one stream, or batches dealt round-robin to internal streams that fork
-// from and join the caller's stream (planes are independent; results do not depend on the split).
-static int run_resident(mvd_handle* h, const uint16_t* views, ViewLayout lay, float* out, int n_planes,
-                        cudaStream_t stream) {
+// Device-resident work: one stream, or batches dealt round-robin to internal streams that fork from and
+// join the caller's stream (planes are independent; results do not depend on the split).
+static int run_resident(mvd_handle* h, const PlaneIO& io, int n_planes, cudaStream_t stream) {
     const size_t npx = (size_t)h->W * h->H;
     const int B = default_batch(h, n_planes);
     const int ns = std::min(h->resident_streams, mvd_handle::kSlots);
-    if (ns <= 1 || h->profiling || n_planes < 2 * B) return run_core(h, h->ws_main, views, lay, out, n_planes, stream);
+    if (ns <= 1 || h->profiling || n_planes < 2 * B) return run_core(h, h->ws_main, io, n_planes, stream);
     int rc = ensure_streams(h);
     {
         size_t a, b, g;
@@ -358,8 +357,7 @@ static int run_resident(mvd_handle* h, const uint16_t* views, ViewLayout lay, fl
     int k = 0;
     for (int p0 = 0; p0 < n_planes && rc == MVD_OK; p0 += B, ++k) {
         const int s = k % ns;
-        rc = run_core(h, h->ws_slot[s], views + (size_t)p0 * lay.plane, lay, out + (size_t)p0 * npx,
-                      std::min(B, n_planes - p0), h->streams[s]);
+        rc = run_core(h, h->ws_slot[s], io.at(p0, npx), std::min(B, n_planes - p0), h->streams[s]);
     }
     for (int s = 0; s < ns; ++s) {   // join even after an error so that the caller's stream stays ordered
         int rj = mvd_check(h, cudaEventRecord(h->ev_join[s], h->streams[s]));
@@ -369,25 +367,61 @@ static int run_resident(mvd_handle* h, const uint16_t* views, ViewLayout lay, fl
     return rc;
 }
 
-int mvd_deconvolve_planes(mvd_handle* h, const uint16_t* dev_views_u16, float* dev_out_f32,
-                          int n_planes, void* stream) {
+// mvd_io -> PlaneIO for n_planes device-resident planes; MVD_ERR_INVALID on a malformed request
+static int io_from(const mvd_handle* h, const mvd_io* io, int n_planes, PlaneIO* out) {
+    if (!io || !io->views || !io->out) return MVD_ERR_INVALID;
+    if (io->out_type != MVD_OUT_F32 && io->out_type != MVD_OUT_U16) return MVD_ERR_INVALID;
+    const size_t npx = (size_t)h->W * h->H;
+    PlaneIO p;
+    p.views = io->views;
+    if (io->view_stride == 0 && io->plane_stride == 0 && io->row_stride == 0) {
+        p.lay = ViewLayout{(size_t)n_planes * npx, npx, (size_t)h->W};
+    } else {
+        if (io->row_stride < (size_t)h->W || io->plane_stride < 1 || (h->V > 1 && io->view_stride < 1)) return MVD_ERR_INVALID;
+        p.lay = ViewLayout{io->view_stride, io->plane_stride, io->row_stride};
+    }
+    p.weights = io->weights;
+    p.w_view = (size_t)n_planes * npx;
+    if (io->out_type == MVD_OUT_U16) p.out16 = static_cast<uint16_t*>(io->out);
+    else p.out = static_cast<float*>(io->out);
+    *out = p;
+    return MVD_OK;
+}
+
+int mvd_deconvolve_planes_ex(mvd_handle* h, const mvd_io* io, int n_planes, void* stream) {
     if (!h || n_planes < 0) return MVD_ERR_INVALID;
     if (n_planes == 0) return MVD_OK;
-    if (!dev_views_u16 || !dev_out_f32) return MVD_ERR_INVALID;
-    const size_t npx = (size_t)h->W * h->H;
-    return run_resident(h, dev_views_u16, ViewLayout{(size_t)n_planes * npx, npx, (size_t)h->W},
-                        dev_out_f32, n_planes, (cudaStream_t)stream);
+    PlaneIO p;
+    const int rc = io_from(h, io, n_planes, &p);
+    if (rc != MVD_OK) return rc;
+    return run_resident(h, p, n_planes, (cudaStream_t)stream);
+}
+
+int mvd_deconvolve_planes(mvd_handle* h, const uint16_t* dev_views_u16, float* dev_out_f32,
+                          int n_planes, void* stream) {
+    const mvd_io io = {dev_views_u16, 0, 0, 0, nullptr, dev_out_f32, MVD_OUT_F32, 0};
+    return mvd_deconvolve_planes_ex(h, &io, n_planes, stream);
 }
 
 int mvd_deconvolve_planes_strided(mvd_handle* h, const uint16_t* dev_views_u16, size_t view_stride,
                                   size_t plane_stride, size_t row_stride, float* dev_out_f32,
                                   int n_planes, void* stream) {
-    if (!h || n_planes < 0) return MVD_ERR_INVALID;
-    if (n_planes == 0) return MVD_OK;
-    if (!dev_views_u16 || !dev_out_f32) return MVD_ERR_INVALID;
-    if (row_stride < (size_t)h->W || plane_stride < 1 || (h->V > 1 && view_stride < 1)) return MVD_ERR_INVALID;
-    return run_resident(h, dev_views_u16, ViewLayout{view_stride, plane_stride, row_stride},
-                        dev_out_f32, n_planes, (cudaStream_t)stream);
+    if (view_stride == 0 && plane_stride == 0 && row_stride == 0) return MVD_ERR_INVALID;
+    const mvd_io io = {dev_views_u16, view_stride, plane_stride, row_stride, nullptr, dev_out_f32, MVD_OUT_F32, 0};
+    return mvd_deconvolve_planes_ex(h, &io, n_planes, stream);
+}
+
+int mvd_deconvolve_planes_weighted(mvd_handle* h, const uint16_t* dev_views_u16, const float* dev_weights_f32,
+                                   float* dev_out_f32, int n_planes, void* stream) {
+    if (!dev_weights_f32) return MVD_ERR_INVALID;
+    const mvd_io io = {dev_views_u16, 0, 0, 0, dev_weights_f32, dev_out_f32, MVD_OUT_F32, 0};
+    return mvd_deconvolve_planes_ex(h, &io, n_planes, stream);
+}
+
+int mvd_deconvolve_planes_u16(mvd_handle* h, const uint16_t* dev_views_u16, uint16_t* dev_out_u16,
+                              int n_planes, void* stream) {
+    const mvd_io io = {dev_views_u16, 0, 0, 0, nullptr, dev_out_u16, MVD_OUT_U16, 0};
+    return mvd_deconvolve_planes_ex(h, &io, n_planes, stream);
 }
 
 static int default_batch(const mvd_handle* h, int n_planes) {
@@ -409,17 +443,32 @@ static int default_batch(const mvd_handle* h, int n_planes) {
 // camera_order: the host stack is [V][H][n_planes][W] (z-stacks of camera frames; plane p = camera line p
 // of every frame).  A batch of B planes is then H row-blocks of B*W contiguous uint16 per view: one
 // cudaMemcpy2DAsync, landing as [V][H][B][W]; the kernels read it in place with ViewLayout{H B W, W, B W}.
-static int host_pipeline(mvd_handle* h, const uint16_t* host_views_u16, float* host_out_f32,
-                         int n_planes, bool camera_order) {
+int mvd_deconvolve_host_ex(mvd_handle* h, const mvd_io* io, int n_planes) {
     if (!h || n_planes < 0) return MVD_ERR_INVALID;
     if (n_planes == 0) return MVD_OK;
-    if (!host_views_u16 || !host_out_f32) return MVD_ERR_INVALID;
+    if (!io || !io->views || !io->out) return MVD_ERR_INVALID;
+    if (io->out_type != MVD_OUT_F32 && io->out_type != MVD_OUT_U16) return MVD_ERR_INVALID;
+    if (io->view_stride || io->plane_stride || io->row_stride) return MVD_ERR_INVALID;   // host stacks are dense
+    const bool camera_order = io->camera_order != 0, u16 = io->out_type == MVD_OUT_U16;
+    const uint16_t* host_views_u16 = io->views;
+    const float* host_w = io->weights;
     const size_t npx = (size_t)h->W * h->H;
+    const size_t out_elem = u16 ? sizeof(uint16_t) : sizeof(float);
     const int B = default_batch(h, n_planes);
 
     {   // everything the batches need is sized before the first copy is enqueued: nothing below allocates
         int rc0 = ensure_streams(h);
         if (rc0 == MVD_OK) rc0 = reserve_slots(h, B);
+        if (rc0 == MVD_OK && host_w && (size_t)B > h->slot_w_planes) {
+            rc0 = mvd_check(h, cudaDeviceSynchronize());
+            for (int s = 0; s < mvd_handle::kSlots; ++s) {
+                if (h->d_w[s]) { cudaFree(h->d_w[s]); h->d_w[s] = nullptr; }
+            }
+            h->slot_w_planes = 0;
+            for (int s = 0; s < mvd_handle::kSlots && rc0 == MVD_OK; ++s)
+                rc0 = mvd_check(h, cudaMalloc((void**)&h->d_w[s], sizeof(float) * npx * B * h->V));
+            if (rc0 == MVD_OK) h->slot_w_planes = (size_t)B;
+        }
         size_t a, b, g;
         scratch_bytes(h, std::min(default_chunk(h), B), &a, &b, &g);
         for (int s = 0; s < mvd_handle::kSlots && rc0 == MVD_OK; ++s) rc0 = ws_reserve(h, h->ws_slot[s], a, b, g);
@@ -430,7 +479,7 @@ static int host_pipeline(mvd_handle* h, const uint16_t* host_views_u16, float* h
     // host memory instead of disk: batch k goes to stream k mod 3; within a stream H2D, the RL
     // steps and D2H are ordered, across streams they overlap.  Nothing blocks until the end.
     // Batch sizes: B, with a ramp B/4, B/2 at both ends of a long stack so that the first H2D copy and the
-    // last D2H copy -- the only ones that overlap no compute -- are short (sizes stay even: plane pairs)
+    // last D2H copy -- the only ones that overlap no compute -- are short.
     // Every batch except the very last holds an EVEN number of planes: the FFT engine pairs planes (2m, 2m+1)
     // counted from the start of its batch, so a batch that started on an odd plane would pair differently
     // from mvd_deconvolve_planes and the output bits would differ.  An odd stack is split as if it had one
@@ -457,30 +506,41 @@ static int host_pipeline(mvd_handle* h, const uint16_t* host_views_u16, float* h
         const int s = k % mvd_handle::kSlots;
         const int n = sizes[bi];
         cudaStream_t st = h->streams[s];
-        ViewLayout lay;
+        PlaneIO p;
+        p.views = h->d_in[s];
         if (camera_order) {
-            lay = ViewLayout{(size_t)h->H * B * h->W, (size_t)h->W, (size_t)B * h->W};
+            p.lay = ViewLayout{(size_t)h->H * B * h->W, (size_t)h->W, (size_t)B * h->W};
             for (int v = 0; v < h->V && rc == MVD_OK; ++v)
-                rc = mvd_check(h, cudaMemcpy2DAsync(h->d_in[s] + (size_t)v * lay.view, sizeof(uint16_t) * B * h->W,
+                rc = mvd_check(h, cudaMemcpy2DAsync(h->d_in[s] + (size_t)v * p.lay.view, sizeof(uint16_t) * B * h->W,
                                                    host_views_u16 + ((size_t)v * h->H * n_planes + p0) * h->W,
                                                    sizeof(uint16_t) * (size_t)n_planes * h->W,
                                                    sizeof(uint16_t) * (size_t)n * h->W, (size_t)h->H,
                                                    cudaMemcpyHostToDevice, st));
         } else {
-            lay = ViewLayout{(size_t)B * npx, npx, (size_t)h->W};
+            p.lay = ViewLayout{(size_t)B * npx, npx, (size_t)h->W};
             for (int v = 0; v < h->V && rc == MVD_OK; ++v)
                 rc = mvd_check(h, cudaMemcpyAsync(h->d_in[s] + (size_t)v * B * npx,
                                                  host_views_u16 + ((size_t)v * n_planes + p0) * npx,
                                                  sizeof(uint16_t) * npx * n, cudaMemcpyHostToDevice, st));
         }
+        if (host_w) {
+            p.weights = h->d_w[s];
+            p.w_view = (size_t)B * npx;
+            for (int v = 0; v < h->V && rc == MVD_OK; ++v)
+                rc = mvd_check(h, cudaMemcpyAsync(h->d_w[s] + (size_t)v * B * npx,
+                                                 host_w + ((size_t)v * n_planes + p0) * npx,
+                                                 sizeof(float) * npx * n, cudaMemcpyHostToDevice, st));
+        }
+        if (u16) p.out16 = reinterpret_cast<uint16_t*>(h->d_out[s]);
+        else p.out = h->d_out[s];
         // at most two batches compute at a time (measured: two concurrent batches fill each other's kernel
         // tails, a third only adds contention), while the copies of all three streams overlap freely
         if (rc == MVD_OK && k >= 2) rc = mvd_check(h, cudaStreamWaitEvent(st, h->ev_join[(k - 2) % mvd_handle::kSlots], 0));
-        if (rc == MVD_OK) rc = run_core(h, h->ws_slot[s], h->d_in[s], lay, h->d_out[s], n, st);
+        if (rc == MVD_OK) rc = run_core(h, h->ws_slot[s], p, n, st);
         if (rc == MVD_OK) rc = mvd_check(h, cudaEventRecord(h->ev_join[s], st));
         if (rc == MVD_OK)
-            rc = mvd_check(h, cudaMemcpyAsync(host_out_f32 + (size_t)p0 * npx, h->d_out[s],
-                                             sizeof(float) * npx * n, cudaMemcpyDeviceToHost, st));
+            rc = mvd_check(h, cudaMemcpyAsync(static_cast<char*>(io->out) + (size_t)p0 * npx * out_elem, h->d_out[s],
+                                             out_elem * npx * n, cudaMemcpyDeviceToHost, st));
     }
     for (int s = 0; s < mvd_handle::kSlots; ++s) {
         int rs = mvd_check(h, cudaStreamSynchronize(h->streams[s]));
@@ -491,12 +551,26 @@ static int host_pipeline(mvd_handle* h, const uint16_t* host_views_u16, float* h
 
 int mvd_deconvolve_host(mvd_handle* h, const uint16_t* host_views_u16, float* host_out_f32,
                         int n_planes) {
-    return host_pipeline(h, host_views_u16, host_out_f32, n_planes, false);
+    const mvd_io io = {host_views_u16, 0, 0, 0, nullptr, host_out_f32, MVD_OUT_F32, 0};
+    return mvd_deconvolve_host_ex(h, &io, n_planes);
 }
 
 int mvd_deconvolve_host_camera(mvd_handle* h, const uint16_t* host_frames_u16, float* host_out_f32,
                                int n_planes) {
-    return host_pipeline(h, host_frames_u16, host_out_f32, n_planes, true);
+    const mvd_io io = {host_frames_u16, 0, 0, 0, nullptr, host_out_f32, MVD_OUT_F32, 1};
+    return mvd_deconvolve_host_ex(h, &io, n_planes);
+}
+
+int mvd_deconvolve_host_weighted(mvd_handle* h, const uint16_t* host_views_u16, const float* host_weights_f32,
+                                 float* host_out_f32, int n_planes) {
+    if (!host_weights_f32) return MVD_ERR_INVALID;
+    const mvd_io io = {host_views_u16, 0, 0, 0, host_weights_f32, host_out_f32, MVD_OUT_F32, 0};
+    return mvd_deconvolve_host_ex(h, &io, n_planes);
+}
+
+int mvd_deconvolve_host_u16(mvd_handle* h, const uint16_t* host_views_u16, uint16_t* host_out_u16, int n_planes) {
+    const mvd_io io = {host_views_u16, 0, 0, 0, nullptr, host_out_u16, MVD_OUT_U16, 0};
+    return mvd_deconvolve_host_ex(h, &io, n_planes);
 }
 
 // ---------------------------------------------------------------------------------------------

@@ -48,7 +48,8 @@ template <int KT, int JC, int MODE>
 __global__ void __launch_bounds__(BX* BY)
 direct_corr_kernel(const float* __restrict__ src, const float* __restrict__ G,
                    const uint16_t* __restrict__ phi, float* __restrict__ dst, int W, int H, int Krt,
-                   int Kp, float eps, int tiles_x, int tiles_y, size_t phi_plane, size_t phi_row) {
+                   int Kp, float eps, int tiles_x, int tiles_y, size_t phi_plane, size_t phi_row,
+                   const float* __restrict__ wgt) {
     extern __shared__ float smem[];
     const int K = KT > 0 ? KT : Krt;
     const int c = (K - 1) / 2;
@@ -112,7 +113,11 @@ direct_corr_kernel(const float* __restrict__ src, const float* __restrict__ G,
             if (y < H) {
                 const size_t p = plane_off + (size_t)y * W + x;
                 if (MODE == 0) dst[p] = (float)phi[(size_t)t * phi_plane + (size_t)y * phi_row + x] / fmaxf(acc[m], eps);   // a2
-                else           dst[p] = dst[p] * acc[m];                      // a4
+                else {                                                        // a4 / a4w
+                    float q = acc[m];
+                    if (wgt) { const float w0 = __ldg(wgt + p); q = fmaf(w0, q, 1.f - w0); }
+                    dst[p] = dst[p] * q;
+                }
             }
         }
     }
@@ -136,11 +141,13 @@ __device__ __forceinline__ float2 ffma2_bcast(float g, float2 w, float2 c) {
 // `stage_G`: copy the coefficient array into shared memory first (false when the caller already did).
 // CG: read src and the read-modify-write of dst through L2 only (ld.global.cg) -- the persistent repair kernel
 // reads what other SMs wrote earlier in the SAME launch, which a stale L1 line must not serve.
+// MODE 1 extras: wgt (nullable) = weights of this view, same layout as dst (a4w: q <- w q + 1 - w, reading W1).
 template <int KT, int JC, int MODE, bool CG = false>
 __device__ __forceinline__ void corr2_tile(float* smem, const float* __restrict__ src, const float* __restrict__ G,
                                            const uint16_t* __restrict__ phi, float* __restrict__ dst, int W, int H,
                                            int Krt, int Kp, float eps, int tile_x, int tile_y, int pa, bool has_b,
-                                           size_t phi_plane, size_t phi_row, bool stage_G) {
+                                           size_t phi_plane, size_t phi_row, bool stage_G,
+                                           const float* __restrict__ wgt = nullptr) {
     const int K = KT > 0 ? KT : Krt;
     const int c = (K - 1) / 2;
     const int SW = (KT > 0 ? KT : Krt) + BX - 1;   // staged tile width (= pitch)
@@ -208,8 +215,14 @@ __device__ __forceinline__ void corr2_tile(float* smem, const float* __restrict_
                     dst[offa + q] = (float)phi[f] / fmaxf(acc[m].x, eps);
                     if (has_b) dst[offb + q] = (float)phi[f + phi_plane] / fmaxf(acc[m].y, eps);
                 } else {                                                      // a4
-                    dst[offa + q] = (CG ? __ldcg(dst + offa + q) : dst[offa + q]) * acc[m].x;
-                    if (has_b) dst[offb + q] = (CG ? __ldcg(dst + offb + q) : dst[offb + q]) * acc[m].y;
+                    float qa = acc[m].x, qb = acc[m].y;
+                    if (wgt) {                                                // a4w
+                        const float w0 = __ldg(wgt + offa + q), w1 = has_b ? __ldg(wgt + offb + q) : 0.f;
+                        qa = fmaf(w0, qa, 1.f - w0);
+                        qb = fmaf(w1, qb, 1.f - w1);
+                    }
+                    dst[offa + q] = (CG ? __ldcg(dst + offa + q) : dst[offa + q]) * qa;
+                    if (has_b) dst[offb + q] = (CG ? __ldcg(dst + offb + q) : dst[offb + q]) * qb;
                 }
             }
         }
@@ -221,13 +234,13 @@ __global__ void __launch_bounds__(BX* BY)
 direct_corr2_kernel(const float* __restrict__ src, const float* __restrict__ G,
                     const uint16_t* __restrict__ phi, float* __restrict__ dst, int W, int H, int Krt,
                     int Kp, float eps, int tiles_x, int tiles_y, size_t phi_plane, size_t phi_row,
-                    int n_planes) {
+                    int n_planes, const float* __restrict__ wgt) {
     extern __shared__ __align__(16) float smem[];
     int t = blockIdx.x;
     const int tile_x = t % tiles_x; t /= tiles_x;
     const int tile_y = t % tiles_y; t /= tiles_y;   // t: pair index
     corr2_tile<KT, JC, MODE>(smem, src, G, phi, dst, W, H, Krt, Kp, eps, tile_x, tile_y, 2 * t,
-                             2 * t + 1 < n_planes, phi_plane, phi_row, true);
+                             2 * t + 1 < n_planes, phi_plane, phi_row, true, wgt);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -239,6 +252,8 @@ direct_corr2_kernel(const float* __restrict__ src, const float* __restrict__ G,
 // flagged pairs with a grid-wide barrier after every pass (the halo dependency between a2 and a3, and
 // between a4 and the next a1).
 // ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint16_t to_u16(float x) { return (uint16_t)__float2uint_rn(fminf(x, 65535.f)); }
+
 __device__ __forceinline__ void grid_barrier(unsigned* counter, unsigned target) {
     __syncthreads();
     if (threadIdx.x == 0 && threadIdx.y == 0) {
@@ -259,6 +274,9 @@ struct RepairArgs {
     const unsigned* flags;      // [pairs]
     unsigned* barrier;          // zeroed before the launch
     unsigned* total;            // per-handle count of pairs ever handed over (mvd_guard_flagged)
+    const float* weights;       // nullptr or [V][n][H][W] (a4w)
+    size_t w_view;
+    uint16_t* out16;            // nullptr, or the uint16 output that receives the repaired planes (out is then scratch)
     int n_planes, W, H, K, Kp, V, T;
     float eps;
 };
@@ -320,9 +338,17 @@ __global__ void __launch_bounds__(BX* BY) direct_repair_kernel(RepairArgs a) {
                 const int pa = 2 * s_list[w / tiles], tl = w % tiles;
                 __syncthreads();
                 corr2_tile<KT, JC, 1, true>(smem, a.r, Gback, nullptr, a.out, a.W, a.H, a.K, a.Kp, a.eps, tl % tiles_x,
-                                      tl / tiles_x, pa, pa + 1 < a.n_planes, 0, 0, true);
+                                      tl / tiles_x, pa, pa + 1 < a.n_planes, 0, 0, true,
+                                      a.weights ? a.weights + (size_t)v * a.w_view : nullptr);
             }
             grid_barrier(a.barrier, ++epoch * gridDim.x);
+        }
+    if (a.out16)
+        for (int k = 0; k < nf; ++k) {
+            const int pa = 2 * s_list[k];
+            const int np = pa + 1 < a.n_planes ? 2 : 1;
+            for (size_t q = (size_t)blockIdx.x * (BX * BY) + tid; q < np * npx; q += (size_t)gridDim.x * (BX * BY))
+                a.out16[(size_t)pa * npx + q] = to_u16(__ldcg(a.out + (size_t)pa * npx + q));
         }
 }
 
@@ -342,6 +368,9 @@ struct SmallArgs {
     int n_planes, W, H, K, Kp, V, T;
     float eps;
     int tile_floats;            // floats of the staging area (coefficients + wrapped float2 tile)
+    const float* weights;       // nullptr or [V][n][H][W] (a4w)
+    size_t w_view;
+    uint16_t* out16;            // set instead of out for uint16 output
 };
 
 template <int KT, int JC>
@@ -380,11 +409,15 @@ __global__ void __launch_bounds__(BX* BY) direct_small_kernel(SmallArgs a) {
                 for (int tl = 0; tl < tiles_x * tiles_y; ++tl) {
                     if (tl) __syncthreads();
                     corr2_tile<KT, JC, 1>(smem, r, Gback, nullptr, psi, a.W, a.H, a.K, a.Kp, a.eps, tl % tiles_x,
-                                          tl / tiles_x, 0, has_b, 0, 0, true);
+                                          tl / tiles_x, 0, has_b, 0, 0, true,
+                                          a.weights ? a.weights + (size_t)v * a.w_view + (size_t)pa * npx : nullptr);
                 }
                 __syncthreads();
             }
-        for (size_t q = tid; q < (has_b ? 2 : 1) * npx; q += BX * BY) a.out[(size_t)pa * npx + q] = psi[q];
+        for (size_t q = tid; q < (has_b ? 2 : 1) * npx; q += BX * BY) {
+            if (a.out16) a.out16[(size_t)pa * npx + q] = to_u16(psi[q]);
+            else a.out[(size_t)pa * npx + q] = psi[q];
+        }
         __syncthreads();
     }
 }
@@ -396,7 +429,7 @@ inline size_t pair_smem_bytes(int K, int Kp) {
 template <int KT, int JC>
 int launch_pair2(int mode, const float* src, const float* G, const uint16_t* phi, float* dst,
                  int W, int H, int K, int Kp, float eps, int n_planes, cudaStream_t st,
-                 size_t phi_plane, size_t phi_row) {
+                 size_t phi_plane, size_t phi_row, const float* wgt) {
     const int tiles_x = (W + BX - 1) / BX, tiles_y = (H + TILE_H - 1) / TILE_H;
     const size_t smem = pair_smem_bytes(K, Kp);
     const long long grid = (long long)((n_planes + 1) / 2) * tiles_x * tiles_y;
@@ -412,7 +445,7 @@ int launch_pair2(int mode, const float* src, const float* G, const uint16_t* phi
             if (e != cudaSuccess) return (int)e;
             opted[0] = smem;
         }
-        k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row, n_planes);
+        k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row, n_planes, wgt);
     } else {
         auto k = direct_corr2_kernel<KT, JC, 1>;
         if (smem > opted[1]) {
@@ -420,7 +453,7 @@ int launch_pair2(int mode, const float* src, const float* G, const uint16_t* phi
             if (e != cudaSuccess) return (int)e;
             opted[1] = smem;
         }
-        k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row, n_planes);
+        k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row, n_planes, wgt);
     }
     return (int)cudaGetLastError();
 }
@@ -428,7 +461,7 @@ int launch_pair2(int mode, const float* src, const float* G, const uint16_t* phi
 template <int KT, int JC>
 int launch_pair_member(int mode, const float* src, const float* G, const uint16_t* phi, float* dst,
                        int W, int H, int K, int Kp, float eps, int n_planes, cudaStream_t st,
-                       size_t phi_plane, size_t phi_row) {
+                       size_t phi_plane, size_t phi_row, const float* wgt) {
     const int tiles_x = (W + BX - 1) / BX, tiles_y = (H + TILE_H - 1) / TILE_H;
     const size_t smem = sizeof(float) * ((size_t)K * Kp + (size_t)(TILE_H + Kp - 1) * (K + BX - 1));
     const long long grid = (long long)n_planes * tiles_x * tiles_y;
@@ -443,7 +476,7 @@ int launch_pair_member(int mode, const float* src, const float* G, const uint16_
             if (e != cudaSuccess) return (int)e;
             opted[0] = smem;
         }
-        k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row);
+        k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row, wgt);
     } else {
         auto k = direct_corr_kernel<KT, JC, 1>;
         if (smem > opted[1]) {
@@ -451,20 +484,20 @@ int launch_pair_member(int mode, const float* src, const float* G, const uint16_
             if (e != cudaSuccess) return (int)e;
             opted[1] = smem;
         }
-        k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row);
+        k<<<(unsigned)grid, block, smem, st>>>(src, G, phi, dst, W, H, K, Kp, eps, tiles_x, tiles_y, phi_plane, phi_row, wgt);
     }
     return (int)cudaGetLastError();
 }
 
 int launch_corr(int mode, const mvd_handle* h, const float* src, const float* G, const uint16_t* phi,
-                float* dst, int n_planes, cudaStream_t st, size_t phi_plane, size_t phi_row) {
+                float* dst, int n_planes, cudaStream_t st, size_t phi_plane, size_t phi_row, const float* wgt) {
     // two planes per thread whenever the float2 tile fits in shared memory; K as a template
     // parameter for the config sizes
     if (h->direct_pair) {
 #define MVD_DIRECT_CASE(KT_, JC_)                                                                 \
     if (h->dK == (KT_) && h->JC == (JC_))                                                         \
         return launch_pair2<KT_, JC_>(mode, src, G, phi, dst, h->W, h->H, h->dK, h->Kp,            \
-                                      h->eps, n_planes, st, phi_plane, phi_row);
+                                      h->eps, n_planes, st, phi_plane, phi_row, wgt);
         MVD_DIRECT_CASE(9, 9)
         MVD_DIRECT_CASE(21, 7)
         MVD_DIRECT_CASE(31, 8)
@@ -473,10 +506,10 @@ int launch_corr(int mode, const mvd_handle* h, const float* src, const float* G,
 #undef MVD_DIRECT_CASE
         if (h->JC == 8)
             return launch_pair2<0, 8>(mode, src, G, phi, dst, h->W, h->H, h->dK, h->Kp, h->eps, n_planes, st,
-                                      phi_plane, phi_row);
+                                      phi_plane, phi_row, wgt);
     }
     return launch_pair_member<0, 8>(mode, src, G, phi, dst, h->W, h->H, h->dK, h->Kp, h->eps,
-                                    n_planes, st, phi_plane, phi_row);
+                                    n_planes, st, phi_plane, phi_row, wgt);
 }
 
 }  // namespace
@@ -578,16 +611,10 @@ int launch_small(const mvd_handle* h, SmallArgs& a, cudaStream_t st) {
 bool direct_small_available(const mvd_handle* h) {
     return h->direct_pair && small_smem_bytes(h) <= 227u * 1024u;
 }
-bool direct_small_fits(int W, int H, int K) {
-    int JC, Kp;
-    direct_choose_chunk(K, &JC, &Kp);
-    return pair_smem_bytes(K, Kp) + sizeof(float) * 4 * (size_t)W * H <= 227u * 1024u;
-}
-
-static int direct_run_small(mvd_handle* h, const uint16_t* views, ViewLayout lay, float* out, int n_planes,
-                            cudaStream_t stream) {
+static int direct_run_small(mvd_handle* h, const PlaneIO& io, int n_planes, cudaStream_t stream) {
     SmallArgs a;
-    a.views = views; a.lay = lay; a.out = out; a.coef = h->d_coef;
+    a.views = io.views; a.lay = io.lay; a.out = io.out; a.coef = h->d_coef;
+    a.weights = io.weights; a.w_view = io.w_view; a.out16 = io.out16;
     a.n_planes = n_planes; a.W = h->W; a.H = h->H; a.K = h->dK; a.Kp = h->Kp; a.V = h->V; a.T = h->T; a.eps = h->eps;
     a.tile_floats = (int)(pair_smem_bytes(h->dK, h->Kp) / sizeof(float));
     int e;
@@ -603,41 +630,50 @@ size_t direct_scratch_bytes(const mvd_handle* h, int n_planes) {
     return sizeof(float) * (size_t)n_planes * h->W * h->H;
 }
 
-int direct_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay, float* out,
-               int n_planes, cudaStream_t stream) {
+__global__ void convert_u16_kernel(const float* __restrict__ psi, uint16_t* __restrict__ out, size_t n) {
+    for (size_t p = blockIdx.x * (size_t)blockDim.x + threadIdx.x; p < n; p += (size_t)gridDim.x * blockDim.x)
+        out[p] = to_u16(psi[p]);
+}
+
+int direct_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cudaStream_t stream) {
     const size_t npx = (size_t)h->W * h->H;
     const size_t n = npx * n_planes;
-    if (h->T > 0 && direct_small_available(h)) return direct_run_small(h, views, lay, out, n_planes, stream);
+    if (h->T > 0 && direct_small_available(h)) return direct_run_small(h, io, n_planes, stream);
+    // psi is iterated in place in the fp32 output; a uint16 output gets an fp32 scratch and one conversion pass
+    int rc = ws_reserve(h, ws, h->T > 0 ? direct_scratch_bytes(h, n_planes) : 0, io.out16 ? sizeof(float) * n : 0);
+    if (rc != MVD_OK) return rc;
+    float* psi = io.out16 ? ws.b : io.out;
+    const unsigned egrid = (unsigned)std::min<size_t>((n + 255) / 256, (size_t)h->n_sm * 16);
     {
         LaunchScope ls(h, KC_INIT_MEAN, stream);
-        const int threads = 256;
-        const size_t want = (n + threads - 1) / threads;
-        const unsigned grid = (unsigned)(want < (size_t)h->n_sm * 16 ? want : (size_t)h->n_sm * 16);
-        init_mean_kernel<<<grid, threads, 0, stream>>>(views, lay, h->V, h->W, h->H, out, n);
+        init_mean_kernel<<<egrid, 256, 0, stream>>>(io.views, io.lay, h->V, h->W, h->H, psi, n);
     }
     MVD_TRY(h, cudaGetLastError());
-    if (h->T == 0) return MVD_OK;
-    int rc = ws_reserve(h, ws, direct_scratch_bytes(h, n_planes), 0);
-    if (rc != MVD_OK) return rc;
     float* r = ws.a;
     const size_t per = (size_t)h->dK * h->Kp;
     for (int t = 0; t < h->T; ++t)
         for (int v = 0; v < h->V; ++v) {
             const float* Gblur = h->d_coef + ((size_t)v * 2 + 0) * per;
             const float* Gback = h->d_coef + ((size_t)v * 2 + 1) * per;
-            const uint16_t* phi = views + (size_t)v * lay.view;
+            const uint16_t* phi = io.views + (size_t)v * io.lay.view;
             int e;
             {
                 LaunchScope ls(h, KC_DIRECT_BLUR_RATIO, stream);
-                e = launch_corr(0, h, out, Gblur, phi, r, n_planes, stream, lay.plane, lay.row);
+                e = launch_corr(0, h, psi, Gblur, phi, r, n_planes, stream, io.lay.plane, io.lay.row, nullptr);
             }
             MVD_TRY(h, (cudaError_t)e);
             {
                 LaunchScope ls(h, KC_DIRECT_BACK_UPDATE, stream);
-                e = launch_corr(1, h, r, Gback, nullptr, out, n_planes, stream, 0, 0);
+                e = launch_corr(1, h, r, Gback, nullptr, psi, n_planes, stream, 0, 0,
+                                io.weights ? io.weights + (size_t)v * io.w_view : nullptr);
             }
             MVD_TRY(h, (cudaError_t)e);
         }
+    if (io.out16) {
+        LaunchScope ls(h, KC_INIT_MEAN, stream);
+        convert_u16_kernel<<<egrid, 256, 0, stream>>>(psi, io.out16, n);
+        MVD_TRY(h, cudaGetLastError());
+    }
     return MVD_OK;
 }
 
@@ -663,11 +699,12 @@ int launch_repair(const mvd_handle* h, RepairArgs& a, cudaStream_t st) {
 
 bool direct_repair_available(const mvd_handle* h) { return h->d_coef != nullptr && h->direct_pair; }
 
-int direct_repair_launch(mvd_handle* h, const uint16_t* views, ViewLayout lay, float* out, float* r_scratch,
+int direct_repair_launch(mvd_handle* h, const PlaneIO& io, float* psi, float* r_scratch,
                          const unsigned* flags, unsigned* barrier, int n_planes, cudaStream_t stream) {
     RepairArgs a;
-    a.views = views; a.lay = lay; a.out = out; a.r = r_scratch; a.coef = h->d_coef; a.flags = flags;
+    a.views = io.views; a.lay = io.lay; a.out = psi; a.r = r_scratch; a.coef = h->d_coef; a.flags = flags;
     a.barrier = barrier; a.total = h->d_guard_total;
+    a.weights = io.weights; a.w_view = io.w_view; a.out16 = io.out16;
     a.n_planes = n_planes; a.W = h->W; a.H = h->H; a.K = h->dK; a.Kp = h->Kp; a.V = h->V; a.T = h->T; a.eps = h->eps;
     int e;
     LaunchScope ls(h, KC_GUARD_REPAIR, stream);

@@ -266,13 +266,15 @@ int fft_default_chunk(const mvd_handle* h) {
     return (int)(c & ~(size_t)1);
 }
 
-int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay, float* out,
-            int n_planes, cudaStream_t stream) {
+int fft_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cudaStream_t stream) {
+    const uint16_t* views = io.views;
+    const ViewLayout lay = io.lay;
     FftState* st = state_of(h);
     if (!st) return MVD_ERR_INVALID;
     const int W = h->W, H = h->H;
     const int pairs = (n_planes + 1) / 2;
     const size_t bytes = sizeof(float2) * (size_t)pairs * H * W;
+    if (io.weights && (((uintptr_t)io.weights & 15u) != 0 || (W & 3) != 0)) return MVD_ERR_INVALID;
     // the bulk copies of the row kernels need 16-byte aligned rows
     if (((uintptr_t)views & 15u) != 0 || ((lay.view * sizeof(uint16_t)) & 15u) != 0 ||
         ((lay.plane * sizeof(uint16_t)) & 15u) != 0 || ((lay.row * sizeof(uint16_t)) & 15u) != 0)
@@ -295,7 +297,10 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay,
     a.view_stride = lay.view;
     a.view_plane = lay.plane;
     a.view_row = lay.row;
-    a.out = out;
+    a.out = io.out;
+    a.out16 = io.out16;
+    a.weights = io.weights;
+    a.w_view = io.w_view;
     a.n_planes = n_planes;
     a.H = H;
     a.V = h->V;
@@ -311,6 +316,8 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay,
     const int row_ctas = (a.total_rows + rp - 1) / rp;
     // v1: many short-lived CTAs; v2: persistent, two CTAs per SM
     const int row_grid = std::max(1, std::min(row_ctas, h->n_sm * (st->row->generation == 2 ? st->row->row_cps : 16)));
+    const int row_grid_w = st->row->generation == 2 && st->row->row_cps_w > 0
+                               ? std::max(1, std::min(row_ctas, h->n_sm * st->row->row_cps_w)) : row_grid;
     const int tiles = W / st->col->col_tc;
     dim3 col_grid;
     if (st->col->generation == 2) {
@@ -360,13 +367,16 @@ int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay,
             {
                 LaunchScope ls(h, KC_FFT_ROWS_UPDATE, stream);
                 a.final = (t == h->T - 1 && v == h->V - 1);
-                rc = mvd_check(h, st->row->rows(mvdfft::ROWS_UPDATE, a, st->tw_row, row_grid, stream));  // a4
+                rc = io.weights   // a4w: the weighted kernel keeps twice the landing zone, so fewer CTAs are resident
+                         ? mvd_check(h, st->row->rows(mvdfft::ROWS_UPDATE_W, a, st->tw_row, row_grid_w, stream))
+                         : mvd_check(h, st->row->rows(mvdfft::ROWS_UPDATE, a, st->tw_row, row_grid, stream));  // a4
             }
             if (rc != MVD_OK) return rc;
         }
     // guard: pairs flagged by the ratio passes are recomputed with the direct engine's arithmetic (one empty
     // cooperative launch when nothing is flagged); Z is free by now and serves as its ratio scratch
+    // (with uint16 output psi is iterated in S, which is free as well)
     if (h->T > 0 && direct_repair_available(h))
-        return direct_repair_launch(h, views, lay, out, ws.a, ws.g + pairs, ws.g + 2 * pairs, n_planes, stream);
+        return direct_repair_launch(h, io, io.out ? io.out : ws.b, ws.a, ws.g + pairs, ws.g + 2 * pairs, n_planes, stream);
     return MVD_OK;
 }

@@ -26,6 +26,11 @@ const SizeOps* mvd_fft_ops_v2(int N) {
             if (N == 2048 && v[0] == 'a') { static const SizeOps o = OpsFor2<Plan<2048, 16, 16, 16, 8>, 256, P2048, 256, false, 2, false, 4, 3>::make(); return &o; }
             if (N == 2048 && v[0] == 'b') { static const SizeOps o = OpsFor2<Plan<2048, 16, 16, 16, 8>, 512, P2048, 256, false, 2, false, 4, 2>::make(); return &o; }
             if (N == 1024 && v[0] == 'a') { static const SizeOps o = OpsFor2<P1024, 256, Plan<1024, 16, 16, 16, 4>, 256, false, 2>::make(); return &o; }
+            if (N == 512 && v[0] == 'c') { static const SizeOps o = OpsFor2<P512, 256, P512, 128, false, 3, true, 8>::make(); return &o; }
+            if (N == 1024 && v[0] == 'c') { static const SizeOps o = OpsFor2<P1024, 256, P1024, 256, false, 1, true, 8>::make(); return &o; }
+            if (N == 2048 && v[0] == 'c') { static const SizeOps o = OpsFor2<P2048, 128, P2048, 256, false, 2, false, 4, 2>::make(); return &o; }
+            if (N == 2048 && v[0] == 'd') { static const SizeOps o = OpsFor2<P2048, 256, P2048, 256, false, 2, false, 4, 2>::make(); return &o; }
+            if (N == 2048 && v[0] == 'e') { static const SizeOps o = OpsFor2<P2048, 64, P2048, 256, false, 2, false, 4, 6>::make(); return &o; }
             if (N == 512 && v[0] == 'a') { static const SizeOps o = OpsFor2<P512, 256, Plan<512, 16, 16, 8, 4>, 128, false, 5>::make(); return &o; }
             if (N == 512 && v[0] == 'b') { static const SizeOps o = OpsFor2<P512, 256, Plan<512, 16, 16, 16, 2>, 128, false, 5>::make(); return &o; }
         }

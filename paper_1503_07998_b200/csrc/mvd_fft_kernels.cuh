@@ -458,7 +458,12 @@ __device__ __forceinline__ void fft_run_tail(float2 (&x)[P::E], float2* buf, con
 // ---------------------------------------------------------------------------------------------
 // kernels
 // ---------------------------------------------------------------------------------------------
-enum RowMode { ROWS_FIRST = 0, ROWS_RATIO = 1, ROWS_UPDATE = 2 };
+// ROWS_UPDATE_W: ROWS_UPDATE with per-view weights (a4w: psi <- psi . (w q + 1 - w), reading W1); the generation-2
+// kernel gives every team a second landing zone for the two weight rows, generation 1 reads them directly
+enum RowMode { ROWS_FIRST = 0, ROWS_RATIO = 1, ROWS_UPDATE = 2, ROWS_UPDATE_W = 3 };
+
+// final store as uint16: round to nearest even, saturate at 65535; negative round-off and NaN -> 0
+__device__ __forceinline__ uint16_t to_u16(float x) { return (uint16_t)__float2uint_rn(fminf(x, 65535.f)); }
 
 struct RowArgs {
     float2* S;               // [pairs][H][W] spectrum (row pass in / out)
@@ -466,8 +471,11 @@ struct RowArgs {
     const uint16_t* views;   // view 0 of plane 0 of this chunk
     size_t view_stride;      // elements between views
     size_t view_plane, view_row;   // elements between planes / image rows of a view (ViewLayout)
-    float* out;              // [n_planes][H][W]; written when `final`
-    int n_planes, H, V, v;   // v: the view of this update (ROWS_RATIO)
+    float* out;              // [n_planes][H][W]; written when `final` (nullptr when out16 is set)
+    uint16_t* out16;         // the same as uint16 (nullptr when out is set)
+    const float* weights;    // nullptr, or the weights of view 0 of plane 0 of this chunk, dense [V][n][H][W]
+    size_t w_view;           // elements between the weight stacks of two views
+    int n_planes, H, V, v;   // v: the view of this update (ROWS_RATIO, ROWS_UPDATE*)
     float eps;
     int final;               // ROWS_UPDATE: last update -> write `out`, skip the forward FFT
                              // ROWS_FIRST : iterations == 0 -> write `out` only
@@ -526,8 +534,13 @@ __global__ void __launch_bounds__(NT) fft_rows_kernel(RowArgs a, const float2* _
                 gm = fmaxf(gm, fmaxf(x[e].x, x[e].y));
                 if (valid) {
                     if (a.final) {
-                        a.out[pxa + pos] = x[e].x;
-                        if (has_b) a.out[pxb + pos] = x[e].y;
+                        if (a.out16) {
+                            a.out16[pxa + pos] = to_u16(x[e].x);
+                            if (has_b) a.out16[pxb + pos] = to_u16(x[e].y);
+                        } else {
+                            a.out[pxa + pos] = x[e].x;
+                            if (has_b) a.out[pxb + pos] = x[e].y;
+                        }
                     } else {
                         a.Z[rowoff + pos] = x[e];
                     }
@@ -567,8 +580,13 @@ __global__ void __launch_bounds__(NT) fft_rows_kernel(RowArgs a, const float2* _
                     x[e] = make_float2(z.x * x[e].x, z.y * x[e].y);
                     if (valid) {
                         if (a.final) {
-                            a.out[pxa + pos] = x[e].x;
-                            if (has_b) a.out[pxb + pos] = x[e].y;
+                            if (a.out16) {
+                                a.out16[pxa + pos] = to_u16(x[e].x);
+                                if (has_b) a.out16[pxb + pos] = to_u16(x[e].y);
+                            } else {
+                                a.out[pxa + pos] = x[e].x;
+                                if (has_b) a.out[pxb + pos] = x[e].y;
+                            }
                         } else {
                             a.Z[rowoff + pos] = x[e];
                         }
@@ -688,15 +706,25 @@ __global__ void __launch_bounds__(NT) fft_rows_tma_kernel(RowArgs a, const float
             if (bmin < tau) a.gflag[pair] = 1u;
         } else {
             const float2* zr = reinterpret_cast<const float2*>(ax);
+            const float* wa = a.weights ? a.weights + (size_t)a.v * a.w_view + pxa : nullptr;   // weights share out's layout
 #pragma unroll
             for (int e = 0; e < E; ++e) {                                 // a4
                 const int pos = t + TPF * e;
                 const float2 z = valid ? zr[pos] : make_float2(0.f, 0.f);
+                if (wa && valid) {                                        // a4w
+                    const float w0 = __ldg(wa + pos), w1 = has_b ? __ldg(wa + npx + pos) : 0.f;
+                    x[e] = make_float2(fmaf(w0, x[e].x, 1.f - w0), fmaf(w1, x[e].y, 1.f - w1));
+                }
                 x[e] = make_float2(z.x * x[e].x, z.y * x[e].y);
                 if (valid) {
                     if (a.final) {
-                        a.out[pxa + pos] = x[e].x;
-                        if (has_b) a.out[pxb + pos] = x[e].y;
+                        if (a.out16) {
+                            a.out16[pxa + pos] = to_u16(x[e].x);
+                            if (has_b) a.out16[pxb + pos] = to_u16(x[e].y);
+                        } else {
+                            a.out[pxa + pos] = x[e].x;
+                            if (has_b) a.out[pxb + pos] = x[e].y;
+                        }
                     } else {
                         a.Z[rowoff + pos] = x[e];
                     }
@@ -823,6 +851,7 @@ struct SizeOps {
     int col_box_w = 0;               // generation 2: floats per TMA box row (2 x columns per team)
     int col_otf_regs = 0;            // generation 2: the column kernel keeps its tile's OTF in registers
     int row_cps = 0, col_cps = 0;    // generation 2: resident CTAs per SM the persistent grids are sized for
+    int row_cps_w = 0;               // ... of the weighted update kernel (twice the landing zone)
     int generation = 1;              // 1: CTA-synchronous TMA-staged kernels (this file); 2: team kernels (mvd_fft_v2.cuh)
 };
 
@@ -837,7 +866,7 @@ struct OpsFor {
     static cudaError_t rows(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st) {
         if (mode == ROWS_FIRST) fft_rows_kernel<P, ROWS_FIRST, NT><<<grid, NT, kFirstSmem, st>>>(a, tw);
         else if (mode == ROWS_RATIO) fft_rows_tma_kernel<P, ROWS_RATIO, NT><<<grid, NT, kRatioSmem, st>>>(a, tw);
-        else fft_rows_tma_kernel<P, ROWS_UPDATE, NT><<<grid, NT, kUpdateSmem, st>>>(a, tw);
+        else fft_rows_tma_kernel<P, ROWS_UPDATE, NT><<<grid, NT, kUpdateSmem, st>>>(a, tw);   // also ROWS_UPDATE_W
         return cudaGetLastError();
     }
     static cudaError_t cols(const CUtensorMap& tmap, const CUtensorMap& otf_map, float2* S, const float2* otf, int conj_otf, int pairs, int W,

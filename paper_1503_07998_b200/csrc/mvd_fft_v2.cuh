@@ -74,24 +74,28 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 template <class P, int MODE, int NT, int RMINB = 2>
 __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const float2* __restrict__ tw_g) {
     constexpr int E = P::E, TPF = P::TPF, W = P::N, RP = NT / TPF;
+    constexpr bool UPD = MODE == ROWS_UPDATE || MODE == ROWS_UPDATE_W, WT = MODE == ROWS_UPDATE_W;
+    constexpr int RW = WT ? 2 * W : W;   // float2 slots of a team's region: exchange / landing zone (+ the weight rows)
     static_assert(NT % TPF == 0 && (TPF <= 32 ? 32 % TPF == 0 : TPF % 32 == 0), "teams are warp-aligned");
     static_assert(TPF % 16 == 0 && W % 16 == 0, "tile-major addressing assumes whole 16-element groups per team step");
     static_assert(TPF <= 32 || RP <= 15, "one named barrier per team");
     static_assert(E % 8 == 0 && TPF % 8 == 0, "the landing copies split evenly over the team");
+    (void)UPD;
     extern __shared__ __align__(16) float2 smem_rows2[];
     float2* tw = smem_rows2;                                  // [(S-1) E][TPF]
-    float2* buf = smem_rows2 + (P::S - 1) * E * TPF;          // [RP][N]
+    float2* buf = smem_rows2 + (P::S - 1) * E * TPF;          // [RP][RW]
     for (int k = threadIdx.x; k < (P::S - 1) * E * TPF; k += NT) tw[k] = tw_g[k];
     __syncthreads();
     pdl_launch_dependents();
     pdl_wait();
     const int team = threadIdx.x / TPF, t = threadIdx.x % TPF;
-    const RowAddr2<P> addr{team * W};
+    const RowAddr2<P> addr{team * RW};
     const TeamSync<TPF> sync{team};
     const size_t npx = (size_t)a.H * W;
     const int stride = gridDim.x * RP;
     const uint16_t* vp = a.views + (size_t)a.v * a.view_stride;
-    float2* land = buf + team * W;                            // the team's region, used linearly as landing zone
+    float2* land = buf + team * RW;                           // the team's region, used linearly as landing zone
+    const float* wv = WT ? a.weights + (size_t)a.v * a.w_view : nullptr;
     const int last_row = a.total_rows - 1;
 
     // S is tile-major: 16-byte chunk q = t + TPF k of image row `row` (elements 2q, 2q+1) sits in tile q / 8 at
@@ -151,8 +155,13 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
             if (a.final) {   // iterations == 0: the mean is the result (uniform over the grid)
 #pragma unroll
                 for (int e = 0; e < E; ++e) {
-                    if (st_a) a.out[pxa + t + TPF * e] = x[e].x;
-                    if (st_b) a.out[pxb + t + TPF * e] = x[e].y;
+                    if (a.out16) {
+                        if (st_a) a.out16[pxa + t + TPF * e] = to_u16(x[e].x);
+                        if (st_b) a.out16[pxb + t + TPF * e] = to_u16(x[e].y);
+                    } else {
+                        if (st_a) a.out[pxa + t + TPF * e] = x[e].x;
+                        if (st_b) a.out[pxb + t + TPF * e] = x[e].y;
+                    }
                 }
                 continue;
             }
@@ -185,6 +194,16 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
                     const int q = t + TPF * k;
                     cp_async16(land + 2 * q, a.Z + rowoff + 2 * q);
                 }
+                if (WT) {   // the weight rows of the two planes: W floats each, behind the Z row
+                    float* lw = reinterpret_cast<float*>(land + W);
+                    const float* qa = wv + pxa + 4 * t;
+                    const float* qb = wv + pxb + 4 * t;
+#pragma unroll
+                    for (int k = 0; k < E / 4; ++k) {
+                        cp_async16(lw + 4 * (t + TPF * k), qa + 4 * TPF * k);
+                        cp_async16(lw + W + 4 * (t + TPF * k), qb + 4 * TPF * k);
+                    }
+                }
             }
             cp_async_commit();
             fft_run_tail<P, +1>(x, buf, tw, t, addr, sync);
@@ -205,6 +224,14 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
                 if (valid && bmin < tau) a.gflag[pair] = 1u;
                 sync();
             } else {
+                if (WT) {
+                    const float* lw = reinterpret_cast<const float*>(land + W);
+#pragma unroll
+                    for (int e = 0; e < E; ++e) {                             // a4w: q <- w q + (1 - w)
+                        const float w0 = lw[t + TPF * e], w1 = lw[W + t + TPF * e];
+                        x[e] = make_float2(fmaf(w0, x[e].x, 1.f - w0), fmaf(w1, x[e].y, 1.f - w1));
+                    }
+                }
 #pragma unroll
                 for (int e = 0; e < E; ++e) {                                 // a4
                     const float2 z = land[t + TPF * e];
@@ -215,8 +242,13 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
                     if (more) issue_S(next_row);
 #pragma unroll
                     for (int e = 0; e < E; ++e) {
-                        if (st_a) a.out[pxa + t + TPF * e] = x[e].x;
-                        if (st_b) a.out[pxb + t + TPF * e] = x[e].y;
+                        if (a.out16) {
+                            if (st_a) a.out16[pxa + t + TPF * e] = to_u16(x[e].x);
+                            if (st_b) a.out16[pxb + t + TPF * e] = to_u16(x[e].y);
+                        } else {
+                            if (st_a) a.out[pxa + t + TPF * e] = x[e].x;
+                            if (st_b) a.out[pxb + t + TPF * e] = x[e].y;
+                        }
                     }
                     continue;
                 }
@@ -472,6 +504,9 @@ template <class P, int NT, class PC, int NTC, bool OTF_REGS, int MINB, bool TMA 
 struct OpsFor2 {
     static_assert(P::N == PC::N, "row and column plan of one entry describe the same length");
     static constexpr size_t kRowSmem = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * P::N);
+    static constexpr size_t kRowSmemW = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * 2 * P::N);
+    static constexpr int kRowCpsW = (int)((228u * 1024u) / (kRowSmemW + 1024)) < RMINB ? (int)((228u * 1024u) / (kRowSmemW + 1024)) : RMINB;
+    static_assert(kRowSmemW <= 227u * 1024u && kRowCpsW >= 1, "the weighted update kernel fits one CTA");
     static constexpr int kTeam = CPT * PC::TPF, kNTeam = NTC / kTeam, kTC = CPT * kNTeam;
     static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)(TMA ? (EARLY ? 3 : 2) : 1) * kNTeam * PC::N * CPT) +
                                        (TMA ? 2 * sizeof(uint64_t) * kNTeam : 0);
@@ -479,6 +514,7 @@ struct OpsFor2 {
     static cudaError_t rows(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st) {
         if (mode == ROWS_FIRST) return launch_pdl(fft2_rows_kernel<P, ROWS_FIRST, NT, RMINB>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
         if (mode == ROWS_RATIO) return launch_pdl(fft2_rows_kernel<P, ROWS_RATIO, NT, RMINB>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
+        if (mode == ROWS_UPDATE_W) return launch_pdl(fft2_rows_kernel<P, ROWS_UPDATE_W, NT, kRowCpsW>, dim3(grid), dim3(NT), kRowSmemW, st, a, tw);
         return launch_pdl(fft2_rows_kernel<P, ROWS_UPDATE, NT, RMINB>, dim3(grid), dim3(NT), kRowSmem, st, a, tw);
     }
     static cudaError_t cols(const CUtensorMap& tmap, const CUtensorMap& otf_map, float2* S, const float2* otf, int conj_otf, int pairs, int W,
@@ -493,6 +529,8 @@ struct OpsFor2 {
         e = cudaFuncSetAttribute(fft2_rows_kernel<P, ROWS_FIRST, NT, RMINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
         if (e != cudaSuccess) return e;
         e = cudaFuncSetAttribute(fft2_rows_kernel<P, ROWS_RATIO, NT, RMINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(fft2_rows_kernel<P, ROWS_UPDATE_W, NT, kRowCpsW>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmemW);
         if (e != cudaSuccess) return e;
         return cudaFuncSetAttribute(fft2_rows_kernel<P, ROWS_UPDATE, NT, RMINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
     }
@@ -513,6 +551,7 @@ struct OpsFor2 {
         o.rows = &rows; o.cols = &cols; o.prepare_rows = &prepare_rows; o.prepare_cols = &prepare_cols;
         o.generation = 2;
         o.row_cps = RMINB;
+        o.row_cps_w = kRowCpsW;
         o.col_cps = MINB;
         o.col_otf_regs = OTF_REGS ? 1 : 0;
         return o;

@@ -68,6 +68,8 @@ struct mvd_handle {
     cudaStream_t streams[kSlots] = {nullptr, nullptr, nullptr};
     Workspace ws_slot[kSlots];
     uint16_t* d_in[kSlots] = {nullptr, nullptr, nullptr};
+    float* d_w[kSlots] = {nullptr, nullptr, nullptr};      // weights of the batch, allocated at the first weighted call
+    size_t slot_w_planes = 0;
     float* d_out[kSlots] = {nullptr, nullptr, nullptr};
     size_t slot_planes = 0;
 
@@ -103,6 +105,27 @@ struct ViewLayout {
     size_t view, plane, row;
 };
 
+// What one call reads and writes, as the engines see it (device pointers; plane 0 = the first plane of the call
+// or chunk).  weights: nullptr, or per-view per-pixel fp32 weights of step a4w (reading W1), dense [V][n][H][W]
+// with w_view elements between views.  Exactly one of out (fp32) / out16 (uint16, round to nearest even,
+// saturated at 65535) is set.
+struct PlaneIO {
+    const uint16_t* views = nullptr;
+    ViewLayout lay{0, 0, 0};
+    const float* weights = nullptr;
+    size_t w_view = 0;
+    float* out = nullptr;
+    uint16_t* out16 = nullptr;
+    PlaneIO at(int p0, size_t npx) const {     // the same, starting p0 planes further on
+        PlaneIO r = *this;
+        r.views = views + (size_t)p0 * lay.plane;
+        if (weights) r.weights = weights + (size_t)p0 * npx;
+        if (out) r.out = out + (size_t)p0 * npx;
+        if (out16) r.out16 = out16 + (size_t)p0 * npx;
+        return r;
+    }
+};
+
 // Returns MVD_OK or records the CUDA error in h and returns MVD_ERR_CUDA / MVD_ERR_NOMEM.
 int mvd_check(mvd_handle* h, cudaError_t e);
 #define MVD_TRY(h, expr)                        \
@@ -118,20 +141,18 @@ int direct_choose_chunk(int K, int* JC, int* Kp);
 int direct_setup(mvd_handle* h, const float* host_psfs, const float* host_xs);
 size_t direct_scratch_bytes(const mvd_handle* h, int n_planes);
 // views: view v of plane p at views + (v * view_stride + p * H * W); out: [n][H][W]
-int direct_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay, float* out,
-               int n_planes, cudaStream_t stream);
+int direct_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cudaStream_t stream);
 
 bool direct_small_available(const mvd_handle* h);
-bool direct_small_fits(int W, int H, int K);
 bool direct_repair_available(const mvd_handle* h);
-int direct_repair_launch(mvd_handle* h, const uint16_t* views, ViewLayout lay, float* out, float* r_scratch,
+// psi: fp32 [n][H][W] iteration buffer of the repair (io.out itself, or scratch when the output is uint16)
+int direct_repair_launch(mvd_handle* h, const PlaneIO& io, float* psi, float* r_scratch,
                          const unsigned* flags, unsigned* barrier, int n_planes, cudaStream_t stream);
 
 // ---- fft path (mvd_fft.cu) --------------------------------------------------------------------
 int fft_supported(int W, int H);
 int fft_setup(mvd_handle* h, const float* host_psfs, const float* host_xs);
-int fft_run(mvd_handle* h, Workspace& ws, const uint16_t* views, ViewLayout lay, float* out,
-            int n_planes, cudaStream_t stream);
+int fft_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cudaStream_t stream);
 int fft_default_chunk(const mvd_handle* h);
 size_t fft_guard_bytes(int n_planes);
 void fft_teardown(mvd_handle* h);
