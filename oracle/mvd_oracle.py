@@ -145,6 +145,23 @@ def deconvolve(views: np.ndarray, psfs: np.ndarray, T: int, eps: float = 1e-6,
     return out
 
 
+def deconvolve_padded(views: np.ndarray, psfs: np.ndarray, T: int, eps: float = 1e-6,
+                      n_threads: Optional[int] = None, extra: int = 0) -> np.ndarray:
+    """The paper's own boundary (Supp. Table 1 caption: the transformed size is "the sum of the
+    actual data size and the size of PSF"): every plane of every view is embedded in a plane K - 1 (+ `extra`)
+    pixels larger in x and z, the periodic iteration runs on the padded planes, and the result is cropped.
+    READING PD1 (the paper does not say what the padding holds): the padding is ZERO.
+    Then psi_0 and every later psi are zero in it (the update is multiplicative) and so is r (phi = 0), i.e. the
+    result on the plane is the RL iteration with zero boundary conditions -- whatever `extra` is (pin PD1).
+    """
+    views = np.ascontiguousarray(views, dtype=np.uint16)
+    V, N, H, W = views.shape
+    K = np.asarray(psfs).shape[1]
+    padded = np.zeros((V, N, H + K - 1 + extra, W + K - 1 + extra), dtype=np.uint16)
+    padded[:, :, :H, :W] = views
+    return np.ascontiguousarray(deconvolve(padded, psfs, T, eps, n_threads)[:, :H, :W])
+
+
 def trace(views_plane: np.ndarray, psfs: np.ndarray, T: int, eps: float = 1e-6) -> np.ndarray:
     """fp64 `[T*V][H][W]`: psi after every view update of ONE plane (views_plane uint16 `[V][H][W]`)."""
     views_plane = np.ascontiguousarray(views_plane, dtype=np.uint16)

@@ -191,7 +191,20 @@ int fft_setup(mvd_handle* h, const float* host_psfs, const float* host_xs) {
         return MVD_OK;
     };
     int rc = upload(make_twiddles(h->W, st.row->row), &st.tw_row);
-    if (rc == MVD_OK) rc = upload(make_twiddles(h->H, st.col->col), &st.tw_col);
+    if (rc == MVD_OK) {
+        if (st.col->col_tw_custom) {   // two-stage plan with unequal thread counts: [RA][RB], exp(-2 pi i t k / H) at [k][t]
+            const int RA = st.col->col.radices[0], RB = st.col->col.radices[1];
+            std::vector<float2> tw((size_t)RA * RB);
+            for (int k = 0; k < RA; ++k)
+                for (int t = 0; t < RB; ++t) {
+                    const double ang = -2.0 * M_PI * (double)(k * t) / (double)h->H;
+                    tw[(size_t)k * RB + t] = make_float2((float)cos(ang), (float)sin(ang));
+                }
+            rc = upload(tw, &st.tw_col);
+        } else {
+            rc = upload(make_twiddles(h->H, st.col->col), &st.tw_col);
+        }
+    }
     if (rc != MVD_OK) {
         if (st.tw_row) cudaFree(st.tw_row);
         if (st.tw_col) cudaFree(st.tw_col);

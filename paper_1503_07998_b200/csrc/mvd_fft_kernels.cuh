@@ -335,6 +335,51 @@ struct Bfly<20, DIR> : BflyTimes5<4, DIR> {};
 template <int DIR>
 struct Bfly<40, DIR> : BflyTimes5<8, DIR> {};
 
+// cos / sin of 2 pi k / 25 as compile-time constants (k any integer)
+__host__ __device__ constexpr float cos25(int k) {
+    constexpr float C[13] = {1.0f, 0.96858316112863107605f, 0.87630668004386358394f, 0.72896862742141155245f,
+                             0.53582679497899654564f, 0.30901699437494745126f, 0.06279051952931352654f,
+                             -0.18738131458572460097f, -0.42577929156507271502f, -0.63742398974868974548f,
+                             -0.80901699437494734024f, -0.92977648588825134723f, -0.99211470131447776488f};
+    k = ((k % 25) + 25) % 25;
+    return C[k > 12 ? 25 - k : k];
+}
+__host__ __device__ constexpr float sin25(int k) {
+    constexpr float S[13] = {0.0f, 0.24868988716485479484f, 0.48175367410171532345f, 0.68454710592868861507f,
+                             0.84432792550201507531f, 0.95105651629515353118f, 0.99802672842827155897f,
+                             0.98228725072868872115f, 0.90482705246601946580f, 0.77051324277578925326f,
+                             0.58778525229247324813f, 0.36812455268467814129f, 0.12533323356430453588f};
+    k = ((k % 25) + 25) % 25;
+    return k > 12 ? -S[25 - k] : S[k];
+}
+// 25 = 5 x 5: n = n1 + 5 n2, f = f2 + 5 f1; 5-point transforms over n2, twiddles w25^(n1 f2), 5-point transforms over n1
+template <int DIR>
+struct Bfly<25, DIR> {
+    static __device__ __forceinline__ void run(float2* v) {
+        float2 a[5][5];
+#pragma unroll
+        for (int n1 = 0; n1 < 5; ++n1) {
+            float2 t[5] = {v[n1], v[n1 + 5], v[n1 + 10], v[n1 + 15], v[n1 + 20]};
+            Bfly<5, DIR>::run(t);
+#pragma unroll
+            for (int f2 = 0; f2 < 5; ++f2) a[n1][f2] = t[f2];
+        }
+#pragma unroll
+        for (int n1 = 1; n1 < 5; ++n1) {
+#pragma unroll
+            for (int f2 = 1; f2 < 5; ++f2)
+                a[n1][f2] = cmul(a[n1][f2], make_float2(cos25(n1 * f2), (DIR < 0 ? -1.f : 1.f) * sin25(n1 * f2)));
+        }
+#pragma unroll
+        for (int f2 = 0; f2 < 5; ++f2) {
+            float2 t[5] = {a[0][f2], a[1][f2], a[2][f2], a[3][f2], a[4][f2]};
+            Bfly<5, DIR>::run(t);
+#pragma unroll
+            for (int f1 = 0; f1 < 5; ++f1) v[f2 + 5 * f1] = t[f1];
+        }
+    }
+};
+
 // ---------------------------------------------------------------------------------------------
 // plans
 // ---------------------------------------------------------------------------------------------
@@ -356,6 +401,22 @@ struct Plan {
     static_assert(N_ % E_ == 0 && E_ % R0 == 0 && E_ % R1 == 0 && E_ % R2 == 0 && E_ % R3 == 0 && E_ % R4 == 0,
                   "every radix must divide the per-thread element count");
 };
+
+// A plan whose last stage is a radix-2 over elements of the same thread (N = R0 R1 2 with E = R1, TPF = 64):
+// the exchange in front of it goes through warp shuffles when the kernel maps logical thread t of an FFT to
+// lane ((t >> 5) << 4 | t & 15) of warp (t >> 4) & 1 (fft_stage).
+template <class P>
+struct ShflTail : P {
+    static constexpr bool kShflTail = true;
+    static_assert(P::S >= 2 && P::radix(P::S - 1) == 2 && P::radix(P::S - 2) == P::E && P::TPF == 64,
+                  "shuffle exchange: one radix-E butterfly per thread in front of a final radix-2 stage, two warps per FFT");
+};
+template <class P, class = void>
+struct ShflTailOf { static constexpr bool value = false; };
+template <class P>
+struct ShflTailOf<P, decltype((void)P::kShflTail)> { static constexpr bool value = P::kShflTail; };
+template <class P>
+__host__ __device__ constexpr bool shfl_tail() { return ShflTailOf<P>::value; }
 
 // Row layout: one FFT per TPF threads, exchange region of NPAD float2 per FFT, padded against the
 // stride-R0 stores of stage 0.
@@ -397,6 +458,7 @@ __device__ __forceinline__ void fft_stage(float2 (&x)[P::E], float2* buf, const 
                                           const Sync& sync) {
     constexpr int R = P::radix(s), NB = P::E / R, NS = P::ns(s), TPF = P::TPF;
     constexpr bool last = (s == P::S - 1);
+    constexpr bool shfl = shfl_tail<P>() && s == P::S - 2;
 #pragma unroll
     for (int u = 0; u < NB; ++u) {
         float2 v[R];
@@ -413,6 +475,21 @@ __device__ __forceinline__ void fft_stage(float2 (&x)[P::E], float2* buf, const 
         if (last) {
 #pragma unroll
             for (int m = 0; m < R; ++m) x[u + m * NB] = v[m];
+        } else if constexpr (shfl) {
+            // The exchange in front of a final radix-2 stage only swaps half of the data between threads t and
+            // t ^ (N / 2 / R) (here 32): position (t / 32) 1024 + t % 32 + 32 m goes to thread t % 32 + 32 (m & 1),
+            // element 16 (t / 32) + m / 2.  The row kernels map those two threads to lanes l and l ^ 16 of one
+            // warp (ShflTail), so the exchange is 16 shuffles and no shared memory or barrier.
+            const bool hi = (t >> 5) & 1;
+#pragma unroll
+            for (int i = 0; i < R / 2; ++i) {
+                const float2 send = hi ? v[2 * i] : v[2 * i + 1];
+                float2 recv;
+                recv.x = __shfl_xor_sync(0xffffffffu, send.x, 16);
+                recv.y = __shfl_xor_sync(0xffffffffu, send.y, 16);
+                x[i] = hi ? recv : v[2 * i];
+                x[R / 2 + i] = hi ? v[2 * i + 1] : recv;
+            }
         } else {
             const int j = t + u * TPF;
             const int k = j % NS;
@@ -421,7 +498,7 @@ __device__ __forceinline__ void fft_stage(float2 (&x)[P::E], float2* buf, const 
             for (int m = 0; m < R; ++m) buf[addr(base + m * NS)] = v[m];
         }
     }
-    if (!last) {
+    if (!last && !shfl) {
         sync();
 #pragma unroll
         for (int e = 0; e < P::E; ++e) x[e] = buf[addr(t + TPF * e)];
@@ -853,6 +930,7 @@ struct SizeOps {
     int row_cps = 0, col_cps = 0;    // generation 2: resident CTAs per SM the persistent grids are sized for
     int row_cps_w = 0;               // ... of the weighted update kernel (twice the landing zone)
     int generation = 1;              // 1: CTA-synchronous TMA-staged kernels (this file); 2: team kernels (mvd_fft_v2.cuh)
+    int col_tw_custom = 0;           // 1: the column kernel's twiddle table is [R0][N / R0]: exp(-2 pi i t k / N) at [k][t] (two-stage plans with unequal thread counts)
 };
 
 template <class P, int NT, class PC, int TC, bool OTF_REGS>

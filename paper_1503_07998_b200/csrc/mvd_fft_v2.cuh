@@ -88,7 +88,10 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
     __syncthreads();
     pdl_launch_dependents();
     pdl_wait();
-    const int team = threadIdx.x / TPF, t = threadIdx.x % TPF;
+    const int team = threadIdx.x / TPF;
+    // ShflTail plans: threads t and t ^ 32 of an FFT sit in lanes l and l ^ 16 of one warp
+    const int t = shfl_tail<P>() ? ((int)(threadIdx.x & 16) << 1) | ((int)(threadIdx.x & 32) >> 1) | (int)(threadIdx.x & 15)
+                                 : (int)threadIdx.x % TPF;
     const RowAddr2<P> addr{team * RW};
     const TeamSync<TPF> sync{team};
     const size_t npx = (size_t)a.H * W;
@@ -482,6 +485,200 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
     if (l == 0) bulk_wait_read();
 }
 
+// Lean column pass: ONE shared-memory region per team.  The team's slice arrives by TMA in the exchange
+// region (requested when the previous item's inverse transform has done its last exchange), the OTF
+// slice is read straight from L2 into registers (CPT >= 8: whole 64-byte segments per eight lanes) and
+// the results leave by plain stores from registers.  Half the shared memory and ~40 % less shared-memory
+// traffic per element than fft2_cols_tma_kernel, so a third (or fourth) team fits on an SM: the pass is
+// bound by barrier and exchange latency at two teams per SM, not by a pipe (profiles/r2_c4_ncu.md).
+__device__ __forceinline__ float2 ldg_nc_na(const float2* p) {
+    float2 r;
+    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p));
+    return r;
+}
+template <class P, int NT, int MINB, int CPT>
+__global__ void __launch_bounds__(NT, MINB)
+fft2_cols_lean_kernel(const __grid_constant__ CUtensorMap tmap, float2* __restrict__ S, const float2* __restrict__ otf,
+                      int conj_otf, int pairs, int W, const float2* __restrict__ tw_g) {
+    constexpr int E = P::E, TPF = P::TPF, H = P::N, TEAM = CPT * TPF, NTEAM = NT / TEAM, TC = CPT * NTEAM;
+    constexpr int BOXH = H <= 256 ? H : (H % 256 == 0 ? 256 : 200);
+    static_assert(H % BOXH == 0 && (CPT == 4 || CPT == 8 || CPT == 16), "whole boxes; a team owns whole 32-byte sectors of a row");
+    static_assert(NT % TEAM == 0 && TEAM % 32 == 0 && (TEAM == 32 || NTEAM <= 15), "column teams are whole warps");
+    extern __shared__ __align__(128) float2 smem_cols4[];
+    constexpr int TW = (P::S - 1) * E * TPF;
+    static_assert(TW % 16 == 0, "twiddle table keeps the regions aligned");
+    float2* tw = smem_cols4;                                  // [(S-1) E][TPF]
+    float2* buf = smem_cols4 + TW;                            // [NTEAM][H][CPT]  exchange regions = landing zones
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_cols4 + TW + NTEAM * H * CPT);   // [NTEAM]
+    if (threadIdx.x < NTEAM) mbar_init(&bars[threadIdx.x], 1);
+    if (threadIdx.x == 0) fence_mbar_init();
+    for (int k = threadIdx.x; k < TW; k += NT) tw[k] = tw_g[k];
+    __syncthreads();
+    pdl_launch_dependents();
+    const int team = threadIdx.x / TEAM, l = threadIdx.x % TEAM;
+    const int c4 = l % CPT, t = l / CPT;
+    const ColAddr2<P, CPT> addr{team * H * CPT + c4};
+    const TeamSync<TEAM> sync{team};
+    const float sgn = conj_otf ? -1.f : 1.f;
+    float2* land = buf + team * H * CPT;
+    uint64_t* full = &bars[team];
+    const int tiles = W / TC;
+    const int items = tiles * pairs;
+    auto first_col = [&](int item) { return (item % tiles) * TC + team * CPT; };
+    auto plane_off = [&](int x) { return (size_t)(x >> 4) * (H * 16) + (x & 15); };
+    auto box_x = [&](int item) { return 2 * (first_col(item) & 15); };
+    auto box_y = [&](int item) { return ((item / tiles) * (W / 16) + (first_col(item) >> 4)) * H; };
+    auto issue = [&](int item) {   // one lane
+        fence_proxy_async();
+        mbar_arrive_expect_tx(full, (uint32_t)(sizeof(float2) * H * CPT));
+#pragma unroll
+        for (int b = 0; b < H / BOXH; ++b) tma_2d_g2s(land + b * BOXH * CPT, &tmap, box_x(item), box_y(item) + b * BOXH, full);
+    };
+
+    int item = blockIdx.x;
+    pdl_wait();
+    if (item < items && l == 0) issue(item);
+    uint32_t phase = 0;
+    for (; item < items; item += gridDim.x) {
+        const int xg = first_col(item) + c4;
+        const float2* op = otf + plane_off(xg) + (size_t)t * 16;
+        float2* Sp = S + (size_t)(item / tiles) * H * W + plane_off(xg) + (size_t)t * 16;
+        float2 x[E];
+        mbar_wait(full, phase);
+        phase ^= 1;
+#pragma unroll
+        for (int e = 0; e < E; ++e) x[e] = land[(t + TPF * e) * CPT + c4];
+        sync();
+        fft_run<P, -1>(x, buf, tw, t, addr, sync);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            float2 w = ldg_nc_na(op + (size_t)(TPF * e) * 16);
+            w.y *= sgn;
+            x[e] = cmul(x[e], w);
+        }
+        fft_run_head<P, +1>(x, buf, tw, t, addr, sync);
+        if (l == 0 && item + (int)gridDim.x < items) issue(item + gridDim.x);
+        fft_run_tail<P, +1>(x, buf, tw, t, addr, sync);
+#pragma unroll
+        for (int e = 0; e < E; ++e) Sp[(size_t)(TPF * e) * 16] = x[e];
+    }
+}
+
+// Column pass for lengths H = RA x RB whose two radices differ (800 = 25 x 32): a two-stage transform in which the
+// stages use different numbers of threads.  RB threads (one warp's worth per column) each hold rows t + RB e and
+// run one radix-RA butterfly; after the exchange RA of them hold RB elements each and run one radix-RB butterfly
+// (X[k1 + RA k2] in thread k1), multiply by the OTF, run the inverse radix-RB butterfly and hand the data back for
+// the inverse radix-RA stage.  Against the uniform 40 x 20 plan (20 threads x 40 elements, five warps per team of
+// eight columns) a team is FOUR columns x 32 threads = four warps (one per scheduler), holds half the shared memory
+// and at most 64 data registers per thread, so four teams are resident per SM instead of two; the price is that
+// 7 of 32 lanes idle in the middle stage.  Loads, OTF slices and stores go through the TMA unit exactly as in
+// fft2_cols_tma_kernel.  Twiddles: tw[k1 RB + t] = exp(-2 pi i t k1 / H).
+template <int RA, int RB, int NT, int MINB>
+__global__ void __launch_bounds__(NT, MINB)
+fft2_cols_nu_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap omap,
+                    int conj_otf, int pairs, int W, const float2* __restrict__ tw_g) {
+    constexpr int H = RA * RB, TPF = RB, CPT = 4, TEAM = CPT * TPF, NTEAM = NT / TEAM, TC = CPT * NTEAM;
+    constexpr int BOXH = H <= 256 ? H : (H % 256 == 0 ? 256 : 200);
+    static_assert(RB == 32 && RA <= RB, "one warp's worth of threads per column");
+    static_assert(H % BOXH == 0 && NT % TEAM == 0 && NTEAM <= 15, "whole boxes, whole teams");
+    extern __shared__ __align__(128) float2 smem_cols5[];
+    constexpr int TW = RA * RB;
+    static_assert(TW % 16 == 0, "twiddle table keeps the regions aligned");
+    float2* tw = smem_cols5;                                  // [RA][RB]
+    float2* buf = smem_cols5 + TW;                            // [NTEAM][H][CPT]  exchange regions / landing zones
+    float2* obuf = buf + NTEAM * H * CPT;                     // [NTEAM][H][CPT]  OTF slices, then results on their way out
+    uint64_t* bars = reinterpret_cast<uint64_t*>(obuf + NTEAM * H * CPT);   // [2][NTEAM]
+    if (threadIdx.x < 2 * NTEAM) mbar_init(&bars[threadIdx.x], 1);
+    if (threadIdx.x == 0) fence_mbar_init();
+    for (int k = threadIdx.x; k < TW; k += NT) tw[k] = tw_g[k];
+    __syncthreads();
+    pdl_launch_dependents();
+    const int team = threadIdx.x / TEAM, l = threadIdx.x % TEAM;
+    const int c = l % CPT, t = l / CPT;
+    const TeamSync<TEAM> sync{team};
+    const float sgn = conj_otf ? -1.f : 1.f;
+    float2* land = buf + team * H * CPT;
+    float2* outz = obuf + team * H * CPT;
+    uint64_t* full = &bars[team];
+    uint64_t* full_otf = &bars[NTEAM + team];
+    // exchange slot of (k1, t): four consecutive t (stage A stores) and four consecutive k1 (stage B loads) both
+    // spread over the four 32-byte groups of a 128-byte line
+    auto slot = [&](int k1, int tt) { return land + ((k1 * RB + (tt ^ (k1 & 3))) * CPT + c); };
+    const int tiles = W / TC;
+    const int items = tiles * pairs;
+    auto first_col = [&](int item) { return (item % tiles) * TC + team * CPT; };
+    auto box_x = [&](int item) { return 2 * (first_col(item) & 15); };
+    auto box_y = [&](int item) { return ((item / tiles) * (W / 16) + (first_col(item) >> 4)) * H; };
+    auto issue = [&](int item) {   // one lane
+        fence_proxy_async();
+        mbar_arrive_expect_tx(full, (uint32_t)(sizeof(float2) * H * CPT));
+#pragma unroll
+        for (int b = 0; b < H / BOXH; ++b) tma_2d_g2s(land + b * BOXH * CPT, &tmap, box_x(item), box_y(item) + b * BOXH, full);
+    };
+    const bool act = t < RA;    // threads of the radix-RB stage
+
+    int item = blockIdx.x;
+    pdl_wait();
+    if (item < items && l == 0) issue(item);
+    uint32_t phase = 0;
+    for (; item < items; item += gridDim.x) {
+        float2 xa[RA];
+        mbar_wait(full, phase);
+        phase ^= 1;
+#pragma unroll
+        for (int e = 0; e < RA; ++e) xa[e] = land[(t + RB * e) * CPT + c];
+        sync();
+        if (l == 0) {   // this item's OTF slice -> the out region, which the previous item's results have left by now
+            bulk_wait_read();
+            fence_proxy_async();
+            mbar_arrive_expect_tx(full_otf, (uint32_t)(sizeof(float2) * H * CPT));
+            const int oy = (first_col(item) >> 4) * H;
+#pragma unroll
+            for (int b = 0; b < H / BOXH; ++b) tma_2d_g2s(outz + b * BOXH * CPT, &omap, box_x(item), oy + b * BOXH, full_otf);
+        }
+        Bfly<RA, -1>::run(xa);
+#pragma unroll
+        for (int k1 = 1; k1 < RA; ++k1) xa[k1] = cmul(xa[k1], tw[k1 * RB + t]);
+#pragma unroll
+        for (int k1 = 0; k1 < RA; ++k1) *slot(k1, t) = xa[k1];
+        sync();
+        if (act) {      // thread t is k1: it reads, transforms and writes back its own RB slots
+            float2 xb[RB];
+#pragma unroll
+            for (int j = 0; j < RB; ++j) xb[j] = *slot(t, j);
+            Bfly<RB, -1>::run(xb);
+            mbar_wait(full_otf, phase ^ 1);      // same parity sequence as `full`: one completion per item
+#pragma unroll
+            for (int k2 = 0; k2 < RB; ++k2) {
+                float2 w = outz[(t + RA * k2) * CPT + c];
+                w.y *= sgn;
+                xb[k2] = cmul(xb[k2], w);
+            }
+            Bfly<RB, +1>::run(xb);
+#pragma unroll
+            for (int j = 0; j < RB; ++j) *slot(t, j) = xb[j];
+        }
+        sync();
+#pragma unroll
+        for (int k1 = 0; k1 < RA; ++k1) xa[k1] = *slot(k1, t);
+        sync();
+        if (l == 0 && item + (int)gridDim.x < items) issue(item + gridDim.x);
+#pragma unroll
+        for (int k1 = 1; k1 < RA; ++k1) xa[k1] = cmulc(xa[k1], tw[k1 * RB + t]);
+        Bfly<RA, +1>::run(xa);
+#pragma unroll
+        for (int e = 0; e < RA; ++e) outz[(t + RB * e) * CPT + c] = xa[e];
+        fence_proxy_async();
+        sync();
+        if (l == 0) {
+#pragma unroll
+            for (int b = 0; b < H / BOXH; ++b) tma_2d_s2g(&tmap, box_x(item), box_y(item) + b * BOXH, outz + b * BOXH * CPT);
+            bulk_commit();
+        }
+    }
+    if (l == 0) bulk_wait_read();
+}
+
 // ---------------------------------------------------------------------------------------------
 // host-side descriptor of a v2 length
 // ---------------------------------------------------------------------------------------------
@@ -582,6 +779,63 @@ struct ColsOnly2 {
         o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = kBoxH; o.col_box_w = 2 * CPT;
         o.rows = nullptr; o.cols = &cols; o.prepare_rows = nullptr; o.prepare_cols = &prepare_cols;
         o.generation = 2; o.row_cps = 0; o.col_cps = MINB; o.col_otf_regs = OTF_REGS ? 1 : 0;
+        return o;
+    }
+};
+
+// A length served by the lean column kernel (columns only when P has no row kernel here).
+template <class PC, int NTC, int MINB, int CPT>
+struct ColsLean2 {
+    static constexpr int kTeam = CPT * PC::TPF, kNTeam = NTC / kTeam, kTC = CPT * kNTeam;
+    static constexpr int kBoxH = PC::N <= 256 ? PC::N : (PC::N % 256 == 0 ? 256 : 200);
+    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)kNTeam * PC::N * CPT) +
+                                       sizeof(uint64_t) * kNTeam;
+    static cudaError_t cols(const CUtensorMap& tmap, const CUtensorMap&, float2* S, const float2* otf, int conj_otf, int pairs, int W,
+                            const float2* tw, dim3 grid, cudaStream_t st) {
+        return launch_pdl(fft2_cols_lean_kernel<PC, NTC, MINB, CPT>, grid, dim3(NTC), kColSmem, st, tmap, S, otf, conj_otf, pairs, W, tw);
+    }
+    static cudaError_t prepare_cols() {
+        return cudaFuncSetAttribute(fft2_cols_lean_kernel<PC, NTC, MINB, CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
+    }
+    // `base`: the descriptor whose row kernels this length keeps (nullptr: columns only)
+    static SizeOps make(const SizeOps* base = nullptr) {
+        SizeOps o;
+        if (base) o = *base;
+        o.N = PC::N;
+        if (!base) {
+            o.row = PlanInfo{0, 0, 0, {0, 0, 0, 0, 0}};
+            o.row_threads = 0; o.row_smem = 0; o.rows = nullptr; o.prepare_rows = nullptr; o.row_cps = 0;
+        }
+        o.col = PlanInfo{PC::E, PC::TPF, PC::S, {PC::radix(0), PC::radix(1), PC::radix(2), PC::radix(3), PC::radix(4)}};
+        o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = kBoxH; o.col_box_w = 2 * CPT;
+        o.cols = &cols; o.prepare_cols = &prepare_cols;
+        o.generation = 2; o.col_cps = MINB; o.col_otf_regs = 0;
+        return o;
+    }
+};
+
+// A column-only length served by fft2_cols_nu_kernel.
+template <int RA, int RB, int NTC, int MINB>
+struct ColsNu2 {
+    static constexpr int kN = RA * RB, kNTeam = NTC / (4 * RB), kTC = 4 * kNTeam;
+    static constexpr int kBoxH = kN <= 256 ? kN : (kN % 256 == 0 ? 256 : 200);
+    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)RA * RB + (size_t)2 * kNTeam * kN * 4) + 2 * sizeof(uint64_t) * kNTeam;
+    static cudaError_t cols(const CUtensorMap& tmap, const CUtensorMap& otf_map, float2*, const float2*, int conj_otf, int pairs, int W,
+                            const float2* tw, dim3 grid, cudaStream_t st) {
+        return launch_pdl(fft2_cols_nu_kernel<RA, RB, NTC, MINB>, grid, dim3(NTC), kColSmem, st, tmap, otf_map, conj_otf, pairs, W, tw);
+    }
+    static cudaError_t prepare_cols() {
+        return cudaFuncSetAttribute(fft2_cols_nu_kernel<RA, RB, NTC, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
+    }
+    static SizeOps make() {
+        SizeOps o;
+        o.N = kN;
+        o.row = PlanInfo{0, 0, 0, {0, 0, 0, 0, 0}};
+        o.col = PlanInfo{RB, RB, 2, {RA, RB, 1, 1, 1}};
+        o.row_threads = 0; o.row_smem = 0;
+        o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = kBoxH; o.col_box_w = 8;
+        o.rows = nullptr; o.cols = &cols; o.prepare_rows = nullptr; o.prepare_cols = &prepare_cols;
+        o.generation = 2; o.row_cps = 0; o.col_cps = MINB; o.col_otf_regs = 0; o.col_tw_custom = 1;
         return o;
     }
 };

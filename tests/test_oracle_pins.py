@@ -465,3 +465,63 @@ def test_PW_argument_validation():
     w[0, 0, 0, 0] = np.nan
     with pytest.raises(ValueError):
         orc.deconvolve(views, synth.delta_psf(3)[None], 1, weights=w)
+
+
+# ---------------------------------------------------------------------------------------------
+# PD: the paper's padded boundary, READING PD1 = zero padding (oracle.deconvolve_padded)
+# ---------------------------------------------------------------------------------------------
+def _rl_zero_boundary_scipy(views, psfs, T, eps):
+    """RL with ZERO boundary conditions written with scipy's non-periodic routines (independent of the oracle's
+    periodic loops): b = convolve2d(psi, P, 'same', fill 0), q = correlate2d(r, P, 'same', fill 0)."""
+    from scipy.signal import convolve2d, correlate2d
+    V, N, H, W = views.shape
+    out = np.empty((N, H, W))
+    e32 = float(np.float32(eps))
+    for n in range(N):
+        phi = views[:, n].astype(np.float64)
+        psi = phi.mean(axis=0) if V not in (1, 2, 4) else phi.sum(axis=0) / V
+        for _ in range(T):
+            for v in range(V):
+                P = psfs[v].astype(np.float64)
+                b = convolve2d(psi, P, mode="same", boundary="fill", fillvalue=0.0)
+                r = phi[v] / np.maximum(b, e32)
+                psi = psi * correlate2d(r, P, mode="same", boundary="fill", fillvalue=0.0)
+        out[n] = psi
+    return out
+
+
+@pytest.mark.parametrize("W,H,K,V", [(13, 9, 5, 2), (8, 12, 7, 3), (10, 10, 3, 1), (6, 5, 9, 2)])
+def test_PD1_padding_amount_does_not_matter(W, H, K, V):
+    """Zero padding of K - 1 pixels decouples opposite edges; any larger padding gives the same plane."""
+    rng = np.random.default_rng(W * 100 + K)
+    views = rng.integers(0, 500, size=(V, 2, H, W)).astype(np.uint16)
+    psfs = rand_psfs(V, K, K + W)
+    a = orc.deconvolve_padded(views, psfs, 4)
+    for extra in (1, 5):
+        b = orc.deconvolve_padded(views, psfs, 4, extra=extra)
+        np.testing.assert_allclose(b, a, rtol=1e-12, atol=1e-300)
+
+
+@pytest.mark.parametrize("W,H,K,V", [(13, 9, 5, 2), (8, 12, 7, 3), (16, 16, 9, 2)])
+def test_PD2_padded_mode_is_rl_with_zero_boundary(W, H, K, V):
+    """Against scipy.signal.convolve2d / correlate2d with zero fill: a dropped or transposed tap, the wrong flip
+    or a crop at the wrong corner all fail here (asymmetric PSFs, W != H)."""
+    rng = np.random.default_rng(7 * W + K)
+    views = rng.integers(1, 800, size=(V, 2, H, W)).astype(np.uint16)
+    psfs = rand_psfs(V, K, 3 * K + H)
+    ref = _rl_zero_boundary_scipy(views, psfs, 3, 1e-6)
+    got = orc.deconvolve_padded(views, psfs, 3)
+    np.testing.assert_allclose(got, ref, rtol=1e-11, atol=1e-300)
+    # and it is NOT the periodic result (the readings differ wherever the PSF reaches across an edge)
+    per = orc.deconvolve(views, psfs, 3)
+    assert np.abs(per - got).max() > 1e-3 * np.abs(got).max()
+
+
+def test_PD3_interior_of_a_dark_bordered_plane_matches_periodic():
+    """A plane whose outer K - 1 pixels are zero in every view sees no difference between the two boundaries."""
+    K, V, H, W = 5, 2, 20, 24
+    rng = np.random.default_rng(5)
+    views = np.zeros((V, 1, H, W), dtype=np.uint16)
+    views[:, :, K - 1:H - K + 1, K - 1:W - K + 1] = rng.integers(1, 900, size=(V, 1, H - 2 * K + 2, W - 2 * K + 2))
+    psfs = rand_psfs(V, K, 11)
+    np.testing.assert_allclose(orc.deconvolve_padded(views, psfs, 3), orc.deconvolve(views, psfs, 3), rtol=1e-12, atol=1e-300)
