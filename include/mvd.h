@@ -81,6 +81,27 @@ MVD_API int mvd_create_path(int plane_w, int plane_h, int n_views, const float* 
                     int iterations, float eps, int path, mvd_handle** out);
 
 /*
+ * mvd_create_padded -- the paper's own boundary (Supp. Table 1 caption: the transformed sizes are "the
+ * sum of the actual data size and the size of PSF").  The caller's planes stay plane_w x plane_h; inside the library
+ * every plane of every view is embedded in a ZERO-filled plane at least psf_size - 1 pixels larger in x and z
+ * (READING PD1 of DESIGN.md: the paper does not say what the padding holds), the periodic iteration of mvd_create runs
+ * on the padded planes and the result is cropped.  Because psi_0 and r are zero in the padding and the update is
+ * multiplicative, the result is the RL iteration with zero boundary conditions on the caller's plane, whatever the
+ * padded size is.  The FFT engine pads to the next supported transform lengths (so ANY plane_w, plane_h up to
+ * 2048 - psf_size + 1 runs on it), the direct engine to exactly plane + psf_size - 1; mvd_get_engine_plane tells.
+ *   path   MVD_PATH_AUTO (FFT whenever a padded size exists) / MVD_PATH_DIRECT / MVD_PATH_FFT.
+ * Layouts, ownership and errors as for mvd_create.  Calls on a padded handle take dense or row-strided views (planes a
+ * whole number of rows apart); per-view weights and camera-order host stacks return MVD_ERR_UNSUPPORTED.
+ * Cost: one zero-fill + embed copy of the views and one crop copy of the result per chunk (2 V + 8 bytes per padded
+ * pixel against 42 V T for the iterations), plus the iterations on the larger planes.
+ */
+MVD_API int mvd_create_padded(int plane_w, int plane_h, int n_views, const float* psfs, int psf_size,
+                              int iterations, float eps, int path, mvd_handle** out);
+
+/* The planes the engine of this handle works on: plane_w x plane_h of mvd_create, the padded size of mvd_create_padded. */
+MVD_API int mvd_get_engine_plane(const mvd_handle* h, int* w, int* hh);
+
+/*
  * Other back-projectors (Supp. Note 2 s.1: "the implemented variants all used the
  * following formula, but replaced X").  Step a3 becomes the TRUE periodic convolution with X_v,
  *   q = r (*) X_v,   q(x) = sum_u X_v(u) r(x - u),   index (j, i) <-> u = (j - cx, i - cx), cx = (bp_size - 1) / 2;

@@ -26,6 +26,8 @@ _fp = ctypes.POINTER(ctypes.c_float)
 SIGNATURES = {
     "mvd_create": (_i, [_i, _i, _i, _fp, _i, _i, _f, ctypes.POINTER(_vp)]),
     "mvd_create_path": (_i, [_i, _i, _i, _fp, _i, _i, _f, _i, ctypes.POINTER(_vp)]),
+    "mvd_create_padded": (_i, [_i, _i, _i, _fp, _i, _i, _f, _i, ctypes.POINTER(_vp)]),
+    "mvd_get_engine_plane": (_i, [_vp, ctypes.POINTER(_i), ctypes.POINTER(_i)]),
     "mvd_create_backprojectors": (_i, [_i, _i, _i, _fp, _i, _fp, _i, _i, _f, _i, ctypes.POINTER(_vp)]),
     "mvd_build_backprojectors": (_i, [_i, _i, _fp, _i, _fp]),
     "mvd_deconvolve_planes": (_i, [_vp, _vp, _vp, _i, _vp]),
@@ -126,7 +128,7 @@ class Mvd:
 
     def __init__(self, plane_w: int, plane_h: int, n_views: int, psfs: np.ndarray, psf_size: int,
                  iterations: int, eps: float = 1e-6, path: Optional[int] = None,
-                 backprojectors: Optional[np.ndarray] = None):
+                 backprojectors: Optional[np.ndarray] = None, padded: bool = False):
         psfs = np.ascontiguousarray(psfs, dtype=np.float32)
         if psfs.size != n_views * psf_size * psf_size:
             raise ValueError("psfs must hold n_views * psf_size * psf_size floats")
@@ -134,7 +136,12 @@ class Mvd:
         self.plane_w, self.plane_h, self.n_views = plane_w, plane_h, n_views
         self.psf_size, self.iterations = psf_size, iterations
         p = psfs.ctypes.data_as(_fp)
-        if backprojectors is not None:      # mvd_create_backprojectors: explicit X_v for step a3
+        if padded:                          # mvd_create_padded: zero-padded planes, cropped result
+            if backprojectors is not None:
+                raise ValueError("padded plans take the Independent back-projector only")
+            rc = lib().mvd_create_padded(plane_w, plane_h, n_views, p, psf_size, iterations, eps,
+                                         PATH_AUTO if path is None else path, ctypes.byref(self._h))
+        elif backprojectors is not None:    # mvd_create_backprojectors: explicit X_v for step a3
             xs = np.ascontiguousarray(backprojectors, dtype=np.float32)
             if xs.ndim != 3 or xs.shape[0] != n_views or xs.shape[1] != xs.shape[2]:
                 raise ValueError("backprojectors must be [n_views][bp_size][bp_size]")
@@ -212,6 +219,12 @@ class Mvd:
     @property
     def path(self) -> int:
         return lib().mvd_get_path(self._h)
+
+    def engine_plane(self) -> Tuple[int, int]:
+        """(w, h) of the planes the engine works on (the padded size of a padded plan)."""
+        w, hh = _i(0), _i(0)
+        self._raise(lib().mvd_get_engine_plane(self._h, ctypes.byref(w), ctypes.byref(hh)), "mvd_get_engine_plane")
+        return w.value, hh.value
 
     def guard_flagged(self) -> int:
         """Plane pairs the FFT engine's guard has handed to the direct engine so far (synchronises)."""
@@ -311,7 +324,8 @@ def build_backprojectors(variant: int, psfs: np.ndarray) -> np.ndarray:
 def deconvolve(views: np.ndarray, psfs: np.ndarray, iterations: int, eps: float = 1e-6,
                path: Optional[int] = None, host: bool = False, chunk_planes: int = 0,
                batch_planes: int = 0, backprojectors: Optional[np.ndarray] = None,
-               resident_streams: int = 0, weights: Optional[np.ndarray] = None, out_u16: bool = False) -> np.ndarray:
+               resident_streams: int = 0, weights: Optional[np.ndarray] = None, out_u16: bool = False,
+               padded: bool = False) -> np.ndarray:
     """Convenience for tests: numpy uint16 `[V][N][H][W]` in, numpy float32 `[N][H][W]` out, through
     mvd_deconvolve_planes (host=False) or mvd_deconvolve_host (host=True, pinned buffers)."""
     import torch
@@ -320,7 +334,7 @@ def deconvolve(views: np.ndarray, psfs: np.ndarray, iterations: int, eps: float 
     views = np.ascontiguousarray(views, dtype=np.uint16)
     V, N, H, W = views.shape
     K = psfs.shape[-1]
-    with Mvd(W, H, V, psfs, K, iterations, eps, path, backprojectors) as m:
+    with Mvd(W, H, V, psfs, K, iterations, eps, path, backprojectors, padded) as m:
         if chunk_planes:
             m.set_chunk_planes(chunk_planes)
         if batch_planes:

@@ -67,6 +67,8 @@ static void ws_free(Workspace& ws) {
     if (ws.a) cudaFree(ws.a);
     if (ws.b) cudaFree(ws.b);
     if (ws.g) cudaFree(ws.g);
+    if (ws.pin) cudaFree(ws.pin);
+    if (ws.pout) cudaFree(ws.pout);
     ws = Workspace();
 }
 
@@ -103,7 +105,8 @@ static int choose_path(int W, int H, int K) {
 }
 
 static int create_impl(int plane_w, int plane_h, int n_views, const float* psfs, int psf_size,
-                       const float* xs, int bp_size, int iterations, float eps, int path, mvd_handle** out) {
+                       const float* xs, int bp_size, int iterations, float eps, int path, mvd_handle** out,
+                       bool padded = false) {
     if (!out) return MVD_ERR_INVALID;
     *out = nullptr;
     if (xs) {
@@ -122,7 +125,18 @@ static int create_impl(int plane_w, int plane_h, int n_views, const float* psfs,
     for (size_t k = 0; k < ncoef; ++k)
         if (!isfinite(psfs[k]) || psfs[k] < 0.f) return MVD_ERR_INVALID;
     if (path != MVD_PATH_AUTO && path != MVD_PATH_DIRECT && path != MVD_PATH_FFT) return MVD_ERR_INVALID;
-    if (path == MVD_PATH_AUTO) {
+    // Padded plan: the engine works on zero-filled planes at least K - 1 pixels larger -- the next
+    // supported transform lengths for the FFT engine, exactly K - 1 more for the direct engine.
+    int eng_w = plane_w, eng_h = plane_h;
+    if (padded) {
+        const int w_min = plane_w + k_eff - 1, h_min = plane_h + k_eff - 1;
+        int fw = 0, fh = 0;
+        const bool fft_ok = path != MVD_PATH_DIRECT && fft_pad_dims(w_min, h_min, &fw, &fh);
+        if (fft_ok) { path = MVD_PATH_FFT; eng_w = fw; eng_h = fh; }
+        else if (path == MVD_PATH_FFT) return MVD_ERR_UNSUPPORTED;
+        else { path = MVD_PATH_DIRECT; eng_w = w_min; eng_h = h_min; }
+        if ((long long)eng_w * eng_h > (1LL << 30) || !mvd_path_supported(path, eng_w, eng_h, k_eff)) return MVD_ERR_UNSUPPORTED;
+    } else if (path == MVD_PATH_AUTO) {
         path = choose_path(plane_w, plane_h, k_eff);
         if (path < 0) return MVD_ERR_UNSUPPORTED;
     } else if (!mvd_path_supported(path, plane_w, plane_h, k_eff)) {
@@ -131,7 +145,8 @@ static int create_impl(int plane_w, int plane_h, int n_views, const float* psfs,
 
     mvd_handle* h = new (std::nothrow) mvd_handle();
     if (!h) return MVD_ERR_NOMEM;
-    h->W = plane_w; h->H = plane_h; h->V = n_views; h->K = psf_size; h->T = iterations;
+    h->W = eng_w; h->H = eng_h; h->uW = plane_w; h->uH = plane_h; h->padded = padded;
+    h->V = n_views; h->K = psf_size; h->T = iterations;
     h->eps = eps; h->path = path;
     h->KX = xs ? bp_size : 0;
     int rc = mvd_check(h, cudaGetDevice(&h->device));
@@ -149,6 +164,18 @@ static int create_impl(int plane_w, int plane_h, int n_views, const float* psfs,
 int mvd_create_path(int plane_w, int plane_h, int n_views, const float* psfs, int psf_size,
                     int iterations, float eps, int path, mvd_handle** out) {
     return create_impl(plane_w, plane_h, n_views, psfs, psf_size, nullptr, 0, iterations, eps, path, out);
+}
+
+int mvd_create_padded(int plane_w, int plane_h, int n_views, const float* psfs, int psf_size,
+                      int iterations, float eps, int path, mvd_handle** out) {
+    return create_impl(plane_w, plane_h, n_views, psfs, psf_size, nullptr, 0, iterations, eps, path, out, true);
+}
+
+int mvd_get_engine_plane(const mvd_handle* h, int* w, int* hh) {
+    if (!h || !w || !hh) return MVD_ERR_INVALID;
+    *w = h->W;
+    *hh = h->H;
+    return MVD_OK;
 }
 
 int mvd_create_backprojectors(int plane_w, int plane_h, int n_views, const float* psfs, int psf_size,
@@ -264,14 +291,72 @@ static int default_chunk(const mvd_handle* h) {
     return (int)std::max<size_t>(1, std::min<size_t>(c, 1 << 20));
 }
 
+// Padded plans: staging for chunks of n planes.  The input staging is zeroed when it is allocated and only its
+// uW x uH corners are ever rewritten, so the padding stays zero.
+static int pad_reserve(mvd_handle* h, Workspace& ws, int n) {
+    if (!h->padded) return MVD_OK;
+    const size_t npx = (size_t)h->W * h->H;
+    const size_t in_b = sizeof(uint16_t) * npx * n * h->V, out_b = sizeof(float) * npx * n;
+    if (in_b > ws.pin_bytes) {
+        if (ws.pin) { MVD_TRY(h, cudaDeviceSynchronize()); MVD_TRY(h, cudaFree(ws.pin)); ws.pin = nullptr; ws.pin_bytes = 0; }
+        MVD_TRY(h, cudaMalloc((void**)&ws.pin, in_b));
+        ws.pin_bytes = in_b;
+    }
+    // the layout [V][n][H][W] depends on n: the corners move, so the whole buffer is cleared for every new n
+    if (out_b > ws.pout_bytes) {
+        if (ws.pout) { MVD_TRY(h, cudaDeviceSynchronize()); MVD_TRY(h, cudaFree(ws.pout)); ws.pout = nullptr; ws.pout_bytes = 0; }
+        MVD_TRY(h, cudaMalloc((void**)&ws.pout, out_b));
+        ws.pout_bytes = out_b;
+    }
+    return MVD_OK;
+}
+
+// One chunk of a padded plan: embed, run the engine on the padded planes, crop (reading PD1).
+static int run_padded_chunk(mvd_handle* h, Workspace& ws, const PlaneIO& sub, int n, cudaStream_t stream) {
+    if (sub.weights) return MVD_ERR_UNSUPPORTED;
+    if (sub.lay.row < (size_t)h->uW || sub.lay.plane % sub.lay.row != 0 || sub.lay.plane / sub.lay.row < (size_t)h->uH)
+        return MVD_ERR_UNSUPPORTED;   // one pitched 3D copy per view: planes must be whole numbers of rows apart
+    const size_t npx = (size_t)h->W * h->H;
+    int rc = pad_reserve(h, ws, n);
+    if (rc != MVD_OK) return rc;
+    // Rows beyond uW and planes' rows beyond uH hold zeros: cleared here because the corner positions depend on n
+    // (chunks of one call share n except the last) -- 2 V bytes per padded pixel, ~2 % of a 10-iteration step.
+    MVD_TRY(h, cudaMemsetAsync(ws.pin, 0, sizeof(uint16_t) * npx * n * h->V, stream));
+    for (int v = 0; v < h->V; ++v) {
+        cudaMemcpy3DParms c = {};
+        c.srcPtr = make_cudaPitchedPtr(const_cast<uint16_t*>(sub.views + (size_t)v * sub.lay.view), sub.lay.row * sizeof(uint16_t),
+                                       h->uW * sizeof(uint16_t), sub.lay.plane / sub.lay.row);
+        c.dstPtr = make_cudaPitchedPtr(ws.pin + (size_t)v * n * npx, h->W * sizeof(uint16_t), h->W * sizeof(uint16_t), h->H);
+        c.extent = make_cudaExtent(h->uW * sizeof(uint16_t), h->uH, n);
+        c.kind = cudaMemcpyDeviceToDevice;
+        MVD_TRY(h, cudaMemcpy3DAsync(&c, stream));
+    }
+    PlaneIO pio;
+    pio.views = ws.pin;
+    pio.lay = ViewLayout{(size_t)n * npx, npx, (size_t)h->W};
+    if (sub.out16) pio.out16 = reinterpret_cast<uint16_t*>(ws.pout);
+    else pio.out = ws.pout;
+    rc = h->path == MVD_PATH_FFT ? fft_run(h, ws, pio, n, stream) : direct_run(h, ws, pio, n, stream);
+    if (rc != MVD_OK) return rc;
+    const size_t elem = sub.out16 ? sizeof(uint16_t) : sizeof(float);
+    cudaMemcpy3DParms c = {};
+    c.srcPtr = make_cudaPitchedPtr(ws.pout, h->W * elem, h->W * elem, h->H);
+    c.dstPtr = make_cudaPitchedPtr(sub.out16 ? (void*)sub.out16 : (void*)sub.out, h->uW * elem, h->uW * elem, h->uH);
+    c.extent = make_cudaExtent(h->uW * elem, h->uH, n);
+    c.kind = cudaMemcpyDeviceToDevice;
+    MVD_TRY(h, cudaMemcpy3DAsync(&c, stream));
+    return MVD_OK;
+}
+
 // All T iterations on planes [0, n) of `io`, in chunks (each chunk runs to completion).
 static int run_core(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cudaStream_t stream) {
-    const size_t npx = (size_t)h->W * h->H;
+    const size_t npx = (size_t)h->uW * h->uH;
     const int chunk = default_chunk(h);
     for (int p0 = 0; p0 < n_planes; p0 += chunk) {
         const int n = std::min(chunk, n_planes - p0);
         const PlaneIO sub = io.at(p0, npx);
-        int rc = h->path == MVD_PATH_FFT ? fft_run(h, ws, sub, n, stream) : direct_run(h, ws, sub, n, stream);
+        int rc = h->padded ? run_padded_chunk(h, ws, sub, n, stream)
+                           : h->path == MVD_PATH_FFT ? fft_run(h, ws, sub, n, stream) : direct_run(h, ws, sub, n, stream);
         if (rc != MVD_OK) return rc;
     }
     return MVD_OK;
@@ -304,7 +389,7 @@ static void scratch_bytes(const mvd_handle* h, int n, size_t* a, size_t* b, size
 // Pipeline slots (uint16 in, fp32 out) for batches of B planes.
 static int reserve_slots(mvd_handle* h, int B) {
     if ((size_t)B <= h->slot_planes) return MVD_OK;
-    const size_t npx = (size_t)h->W * h->H;
+    const size_t npx = (size_t)h->uW * h->uH;
     MVD_TRY(h, cudaDeviceSynchronize());
     for (int s = 0; s < mvd_handle::kSlots; ++s) {
         if (h->d_in[s]) { cudaFree(h->d_in[s]); h->d_in[s] = nullptr; }
@@ -327,9 +412,12 @@ int mvd_reserve(mvd_handle* h, int max_planes) {
     size_t a, b, g;
     scratch_bytes(h, std::min(chunk, max_planes), &a, &b, &g);
     if ((rc = ws_reserve(h, h->ws_main, a, b, g)) != MVD_OK) return rc;
+    if ((rc = pad_reserve(h, h->ws_main, std::min(chunk, max_planes))) != MVD_OK) return rc;
     scratch_bytes(h, std::min(chunk, B), &a, &b, &g);
-    for (int s = 0; s < mvd_handle::kSlots; ++s)
+    for (int s = 0; s < mvd_handle::kSlots; ++s) {
         if ((rc = ws_reserve(h, h->ws_slot[s], a, b, g)) != MVD_OK) return rc;
+        if ((rc = pad_reserve(h, h->ws_slot[s], std::min(chunk, B))) != MVD_OK) return rc;
+    }
     return reserve_slots(h, B);
 }
 
@@ -341,7 +429,7 @@ int mvd_get_batch_planes(const mvd_handle* h, int n_planes) {
 // Device-resident work: one stream, or batches dealt round-robin to internal streams that fork from and
 // join the caller's stream (planes are independent; results do not depend on the split).
 static int run_resident(mvd_handle* h, const PlaneIO& io, int n_planes, cudaStream_t stream) {
-    const size_t npx = (size_t)h->W * h->H;
+    const size_t npx = (size_t)h->uW * h->uH;
     const int B = default_batch(h, n_planes);
     const int ns = std::min(h->resident_streams, mvd_handle::kSlots);
     if (ns <= 1 || h->profiling || n_planes < 2 * B) return run_core(h, h->ws_main, io, n_planes, stream);
@@ -371,13 +459,13 @@ static int run_resident(mvd_handle* h, const PlaneIO& io, int n_planes, cudaStre
 static int io_from(const mvd_handle* h, const mvd_io* io, int n_planes, PlaneIO* out) {
     if (!io || !io->views || !io->out) return MVD_ERR_INVALID;
     if (io->out_type != MVD_OUT_F32 && io->out_type != MVD_OUT_U16) return MVD_ERR_INVALID;
-    const size_t npx = (size_t)h->W * h->H;
+    const size_t npx = (size_t)h->uW * h->uH;
     PlaneIO p;
     p.views = io->views;
     if (io->view_stride == 0 && io->plane_stride == 0 && io->row_stride == 0) {
-        p.lay = ViewLayout{(size_t)n_planes * npx, npx, (size_t)h->W};
+        p.lay = ViewLayout{(size_t)n_planes * npx, npx, (size_t)h->uW};
     } else {
-        if (io->row_stride < (size_t)h->W || io->plane_stride < 1 || (h->V > 1 && io->view_stride < 1)) return MVD_ERR_INVALID;
+        if (io->row_stride < (size_t)h->uW || io->plane_stride < 1 || (h->V > 1 && io->view_stride < 1)) return MVD_ERR_INVALID;
         p.lay = ViewLayout{io->view_stride, io->plane_stride, io->row_stride};
     }
     p.weights = io->weights;
@@ -429,12 +517,12 @@ static int default_batch(const mvd_handle* h, int n_planes) {
         return h->path == MVD_PATH_FFT ? even_up(h->batch_planes) : std::min(h->batch_planes, n_planes);
     // ~64 MiB of uint16 input per batch, at least 16 batches when the stack allows it so that the
     // pipeline's fill and drain (one H2D and one D2H that overlap nothing) stay a few percent
-    const size_t per_plane = (size_t)h->W * h->H * sizeof(uint16_t) * h->V;
+    const size_t per_plane = (size_t)h->uW * h->uH * sizeof(uint16_t) * h->V;
     size_t b = std::max<size_t>(1, ((size_t)64 << 20) / per_plane);
     b = std::min<size_t>(b, std::max(1, n_planes / 16));
     // ... but never batches so small that a launch has nothing to chew on: at least ~2 Mvoxel
     // (config 1's 8 planes of 64 x 64 stay one batch)
-    const size_t floor_planes = (((size_t)2 << 20) + (size_t)h->W * h->H - 1) / ((size_t)h->W * h->H);
+    const size_t floor_planes = (((size_t)2 << 20) + (size_t)h->uW * h->uH - 1) / ((size_t)h->uW * h->uH);
     b = std::max(b, floor_planes);
     b = std::max<size_t>(1, std::min<size_t>(b, (size_t)n_planes));
     return h->path == MVD_PATH_FFT ? even_up((int)b) : (int)b;
@@ -450,9 +538,10 @@ int mvd_deconvolve_host_ex(mvd_handle* h, const mvd_io* io, int n_planes) {
     if (io->out_type != MVD_OUT_F32 && io->out_type != MVD_OUT_U16) return MVD_ERR_INVALID;
     if (io->view_stride || io->plane_stride || io->row_stride) return MVD_ERR_INVALID;   // host stacks are dense
     const bool camera_order = io->camera_order != 0, u16 = io->out_type == MVD_OUT_U16;
+    if (h->padded && (camera_order || io->weights)) return MVD_ERR_UNSUPPORTED;
     const uint16_t* host_views_u16 = io->views;
     const float* host_w = io->weights;
-    const size_t npx = (size_t)h->W * h->H;
+    const size_t npx = (size_t)h->uW * h->uH;
     const size_t out_elem = u16 ? sizeof(uint16_t) : sizeof(float);
     const int B = default_batch(h, n_planes);
 
@@ -509,15 +598,15 @@ int mvd_deconvolve_host_ex(mvd_handle* h, const mvd_io* io, int n_planes) {
         PlaneIO p;
         p.views = h->d_in[s];
         if (camera_order) {
-            p.lay = ViewLayout{(size_t)h->H * B * h->W, (size_t)h->W, (size_t)B * h->W};
+            p.lay = ViewLayout{(size_t)h->uH * B * h->uW, (size_t)h->uW, (size_t)B * h->uW};
             for (int v = 0; v < h->V && rc == MVD_OK; ++v)
-                rc = mvd_check(h, cudaMemcpy2DAsync(h->d_in[s] + (size_t)v * p.lay.view, sizeof(uint16_t) * B * h->W,
-                                                   host_views_u16 + ((size_t)v * h->H * n_planes + p0) * h->W,
-                                                   sizeof(uint16_t) * (size_t)n_planes * h->W,
-                                                   sizeof(uint16_t) * (size_t)n * h->W, (size_t)h->H,
+                rc = mvd_check(h, cudaMemcpy2DAsync(h->d_in[s] + (size_t)v * p.lay.view, sizeof(uint16_t) * B * h->uW,
+                                                   host_views_u16 + ((size_t)v * h->uH * n_planes + p0) * h->uW,
+                                                   sizeof(uint16_t) * (size_t)n_planes * h->uW,
+                                                   sizeof(uint16_t) * (size_t)n * h->uW, (size_t)h->uH,
                                                    cudaMemcpyHostToDevice, st));
         } else {
-            p.lay = ViewLayout{(size_t)B * npx, npx, (size_t)h->W};
+            p.lay = ViewLayout{(size_t)B * npx, npx, (size_t)h->uW};
             for (int v = 0; v < h->V && rc == MVD_OK; ++v)
                 rc = mvd_check(h, cudaMemcpyAsync(h->d_in[s] + (size_t)v * B * npx,
                                                  host_views_u16 + ((size_t)v * n_planes + p0) * npx,

@@ -157,6 +157,23 @@ int fft_supported(int W, int H) {
     return 1;
 }
 
+int fft_pad_dims(int w_min, int h_min, int* Wp, int* Hp) {
+    std::vector<int> lens;
+    for (int n = 32; n <= 2048; ++n)
+        if (find_ops_v1(n) || mvd_fft_ops_v2(n)) lens.push_back(n);
+    long long best = 0;
+    for (int w : lens) {
+        if (w < w_min) continue;
+        for (int hh : lens) {
+            if (hh < h_min || !fft_supported(w, hh)) continue;
+            const long long area = (long long)w * hh;
+            if (!best || area < best) { best = area; *Wp = w; *Hp = hh; }
+            break;   // lens is ascending: the first supported height is the smallest for this width
+        }
+    }
+    return best ? 1 : 0;
+}
+
 void fft_teardown(mvd_handle* h) {
     FftState* st = state_of(h);
     if (!st) return;

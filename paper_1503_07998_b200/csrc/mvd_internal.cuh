@@ -35,10 +35,19 @@ struct Workspace {
     size_t a_bytes = 0, b_bytes = 0;
     unsigned* g = nullptr;   // fft: guard words of the chunk in flight: [pairs] max bits of psi_0, [pairs] flags, [1] barrier
     size_t g_bytes = 0;
+    // padded plans (mvd_create_padded): the chunk's views embedded in zero planes of the engine's size, uint16
+    // [V][n][H][W] (the padding is written once, when the buffer is allocated), and the engine's output [n][H][W]
+    uint16_t* pin = nullptr;
+    float* pout = nullptr;
+    size_t pin_bytes = 0, pout_bytes = 0;
 };
 
 struct mvd_handle {
-    int W = 0, H = 0, V = 0, K = 0, T = 0;
+    int W = 0, H = 0, V = 0, K = 0, T = 0;   // W x H: the planes the engine works on
+    // the caller's planes: uW x uH = W x H, or smaller for a padded plan: the caller's planes sit in the
+    // corner of zero-filled W x H planes, W >= uW + K - 1 and H >= uH + K - 1, and the result is cropped
+    int uW = 0, uH = 0;
+    bool padded = false;
     float eps = 0.f;
     int path = MVD_PATH_DIRECT;
     int device = 0;
@@ -151,6 +160,8 @@ int direct_repair_launch(mvd_handle* h, const PlaneIO& io, float* psi, float* r_
 
 // ---- fft path (mvd_fft.cu) --------------------------------------------------------------------
 int fft_supported(int W, int H);
+// smallest supported W x H (by area) with W >= w_min and H >= h_min; 0 if there is none
+int fft_pad_dims(int w_min, int h_min, int* W, int* H);
 int fft_setup(mvd_handle* h, const float* host_psfs, const float* host_xs);
 int fft_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cudaStream_t stream);
 int fft_default_chunk(const mvd_handle* h);
