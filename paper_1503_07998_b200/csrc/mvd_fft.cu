@@ -21,6 +21,8 @@ namespace {
 const SizeOps* find_ops_v1(int N) {
     if (const SizeOps* o = mvd_fft_ops_small(N)) return o;
     if (const SizeOps* o = mvd_fft_ops_mid(N)) return o;
+    if (const SizeOps* o = mvd_fft_ops_more_a(N)) return o;
+    if (const SizeOps* o = mvd_fft_ops_more_b(N)) return o;
     return mvd_fft_ops_large(N);
 }
 bool use_v2(int W, int H) {
@@ -161,17 +163,17 @@ int fft_pad_dims(int w_min, int h_min, int* Wp, int* Hp) {
     std::vector<int> lens;
     for (int n = 32; n <= 2048; ++n)
         if (find_ops_v1(n) || mvd_fft_ops_v2(n)) lens.push_back(n);
-    long long best = 0;
+    // cost = padded area, x 1.6 for shapes only the generation-1 kernels take (measured ratio of the two generations)
+    double best = 0.0;
     for (int w : lens) {
         if (w < w_min) continue;
         for (int hh : lens) {
             if (hh < h_min || !fft_supported(w, hh)) continue;
-            const long long area = (long long)w * hh;
-            if (!best || area < best) { best = area; *Wp = w; *Hp = hh; }
-            break;   // lens is ascending: the first supported height is the smallest for this width
+            const double cost = (double)w * hh * (use_v2(w, hh) ? 1.0 : 1.6);
+            if (best == 0.0 || cost < best) { best = cost; *Wp = w; *Hp = hh; }
         }
     }
-    return best ? 1 : 0;
+    return best > 0.0 ? 1 : 0;
 }
 
 void fft_teardown(mvd_handle* h) {

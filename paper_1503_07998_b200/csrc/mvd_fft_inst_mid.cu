@@ -8,9 +8,9 @@ const SizeOps* mvd_fft_ops_mid(int N) {
     using P512 = Plan<512, 8, 8, 8, 8>;
     using P800 = Plan<800, 40, 8, 5, 5, 4>;
     static const SizeOps o256 = OpsFor<P256, 256, P256, 16, true>::make();
-    static const SizeOps o320 = OpsFor<P320, 256, P320, 8, false>::make();
+    static const SizeOps o320 = OpsFor<P320, 64, P320, 8, false>::make();
     static const SizeOps o512 = OpsFor<P512, 256, P512, 8, true>::make();
-    static const SizeOps o800 = OpsFor<P800, 160, P800, 8, false>::make();
+    static const SizeOps o800 = OpsFor<P800, 80, P800, 8, false>::make();
     switch (N) {
         case 256: return &o256;
         case 320: return &o320;

@@ -16,7 +16,7 @@ const SizeOps* mvd_fft_ops_small(int N) {
     static const SizeOps o96 = OpsFor<P96, 128, P96, 16, true>::make();
     static const SizeOps o128 = OpsFor<P128, 256, P128, 16, true>::make();
     static const SizeOps o160 = OpsFor<P160, 128, P160, 16, false>::make();
-    static const SizeOps o192 = OpsFor<P192, 256, P192, 16, true>::make();
+    static const SizeOps o192 = OpsFor<P192, 128, P192, 16, true>::make();
     switch (N) {
         case 32: return &o32;
         case 64: return &o64;

@@ -983,4 +983,6 @@ struct OpsFor {
 const mvdfft::SizeOps* mvd_fft_ops_small(int N);
 const mvdfft::SizeOps* mvd_fft_ops_mid(int N);
 const mvdfft::SizeOps* mvd_fft_ops_large(int N);
+const mvdfft::SizeOps* mvd_fft_ops_more_a(int N);   // 384, 768, 1536
+const mvdfft::SizeOps* mvd_fft_ops_more_b(int N);   // 640, 1280, 1600
 const mvdfft::SizeOps* mvd_fft_ops_v2(int N);      // power-of-two lengths, team kernels

@@ -56,6 +56,16 @@ def test_path_supported_needs_no_device(lib):
         assert binding.path_supported(binding.PATH_AUTO, *cid_shape)
 
 
+def test_fft_engine_length_set(lib):
+    """Every 2^a 3^b 5^c length the kernels are instantiated for, as rows and as columns."""
+    lengths = [32, 64, 80, 96, 128, 160, 192, 256, 320, 384, 512, 640, 768, 800, 1024, 1280, 1536, 1600, 2048]
+    for w in lengths:
+        for h in lengths:
+            assert binding.path_supported(binding.PATH_FFT, w, h, 9), (w, h)
+    for n in (33, 100, 2000, 4096):
+        assert not binding.path_supported(binding.PATH_FFT, n, 256, 9)
+
+
 def test_create_validates_before_touching_the_device(lib):
     """Argument errors are reported as MVD_ERR_INVALID even on a box without a GPU."""
     P = np.full((1, 3, 3), 1 / 9, dtype=np.float32)

@@ -242,6 +242,16 @@ def test_reserved_handle_is_capturable_into_a_cuda_graph(path):
     (2, 2, 1024, 1024, 7, 1, "random"),  # generation 2: config 5's plane with an asymmetric PSF
     (1, 2, 2048, 2048, 5, 1, "random"),  # the largest plane the FFT engine takes
     (2, 3, 64, 32, 1, 3, "random"),      # psf_size 1: a scalar "PSF"
+    (2, 3, 384, 640, 7, 2, "random"),    # lengths 2^a 3 and 2^a 5 (generation 1): rows 384, columns 640
+    (2, 2, 640, 384, 5, 2, "random"),    # ... and the other way round
+    (1, 2, 768, 1280, 5, 1, "random"),
+    (2, 2, 1280, 768, 7, 1, "sparse"),
+    (1, 2, 1536, 1600, 5, 1, "random"),
+    (2, 1, 1600, 1536, 5, 1, "random"),
+    (2, 2, 2048, 1280, 5, 1, "random"),  # a generation-2 length next to a generation-1 one: both run generation 1
+    (2, 2, 800, 160, 7, 2, "random"),    # 800-point ROWS (generation 1)
+    (2, 3, 320, 80, 5, 2, "random"),
+    (1, 2, 800, 2048, 5, 1, "random"),   # generation-1 2048-point columns
 ])
 def test_asymmetric_and_ragged(path, V, N, W, H, K, T, psf):
     _need(path, W, H, K)
