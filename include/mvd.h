@@ -275,7 +275,7 @@ MVD_API int mvd_set_batch_planes(mvd_handle* h, int planes);
  *                         since the last read; both arrays are HOST, length MVD_N_KERNEL_CLASSES.
  *   mvd_kernel_class_name static name of class k (NULL if out of range).
  */
-enum { MVD_N_KERNEL_CLASSES = 10 };
+enum { MVD_N_KERNEL_CLASSES = 12 };
 MVD_API long long mvd_launch_count(const mvd_handle* h);
 MVD_API void mvd_launch_count_reset(mvd_handle* h);
 MVD_API int mvd_profile_enable(mvd_handle* h, int on);

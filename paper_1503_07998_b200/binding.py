@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libmvd.so")
 
 MVD_OK, MVD_ERR_INVALID, MVD_ERR_UNSUPPORTED, MVD_ERR_CUDA, MVD_ERR_NOMEM, MVD_ERR_BUSY = 0, -1, -2, -3, -4, -5
 PATH_AUTO, PATH_DIRECT, PATH_FFT = 0, 1, 2
-N_KERNEL_CLASSES = 10
+N_KERNEL_CLASSES = 12
 PATH_NAMES = {PATH_AUTO: "auto", PATH_DIRECT: "direct", PATH_FFT: "fft"}
 
 # name -> (restype, argtypes): the symbols include/mvd.h declares (tests check the two agree)

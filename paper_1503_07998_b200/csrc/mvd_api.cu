@@ -152,6 +152,7 @@ static int create_impl(int plane_w, int plane_h, int n_views, const float* psfs,
     int rc = mvd_check(h, cudaGetDevice(&h->device));
     if (rc == MVD_OK) rc = mvd_check(h, cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device));
     if (rc == MVD_OK) rc = path == MVD_PATH_FFT ? fft_setup(h, psfs, xs) : direct_setup(h, psfs, xs);
+    if (rc == MVD_OK && path == MVD_PATH_DIRECT && !getenv("MVD_NO_SEPARABLE")) rc = sep_setup(h, psfs);
     if (rc != MVD_OK) {
         // keep the cuda error visible to the caller through the return code only
         mvd_destroy(h);
@@ -267,6 +268,7 @@ void mvd_destroy(mvd_handle* h) {
     }
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
     if (h->d_coef) cudaFree(h->d_coef);
+    if (h->d_sep) cudaFree(h->d_sep);
     if (h->d_guard_total) cudaFree(h->d_guard_total);
     if (h->d_otf) cudaFree(h->d_otf);
     if (h->d_otf_b) cudaFree(h->d_otf_b);
@@ -362,7 +364,7 @@ static int run_core(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_plane
     return MVD_OK;
 }
 
-static int default_batch(const mvd_handle* h, int n_planes);
+static int default_batch(const mvd_handle* h, int n_planes, int min_batches = 16);
 
 // Streams and events of the host pipeline / the forked device-resident batches, created once.
 static int ensure_streams(mvd_handle* h) {
@@ -408,7 +410,7 @@ int mvd_reserve(mvd_handle* h, int max_planes) {
     if (!h || max_planes < 1) return MVD_ERR_INVALID;
     int rc = ensure_streams(h);
     if (rc != MVD_OK) return rc;
-    const int B = default_batch(h, max_planes), chunk = default_chunk(h);
+    const int B = std::max(default_batch(h, max_planes), default_batch(h, max_planes, 4)), chunk = default_chunk(h);
     size_t a, b, g;
     scratch_bytes(h, std::min(chunk, max_planes), &a, &b, &g);
     if ((rc = ws_reserve(h, h->ws_main, a, b, g)) != MVD_OK) return rc;
@@ -430,7 +432,7 @@ int mvd_get_batch_planes(const mvd_handle* h, int n_planes) {
 // join the caller's stream (planes are independent; results do not depend on the split).
 static int run_resident(mvd_handle* h, const PlaneIO& io, int n_planes, cudaStream_t stream) {
     const size_t npx = (size_t)h->uW * h->uH;
-    const int B = default_batch(h, n_planes);
+    const int B = default_batch(h, n_planes, 4);
     const int ns = std::min(h->resident_streams, mvd_handle::kSlots);
     if (ns <= 1 || h->profiling || n_planes < 2 * B) return run_core(h, h->ws_main, io, n_planes, stream);
     int rc = ensure_streams(h);
@@ -512,14 +514,25 @@ int mvd_deconvolve_planes_u16(mvd_handle* h, const uint16_t* dev_views_u16, uint
     return mvd_deconvolve_planes_ex(h, &io, n_planes, stream);
 }
 
-static int default_batch(const mvd_handle* h, int n_planes) {
+// min_batches: 16 for the host pipeline (its fill and drain -- one H2D and one D2H that overlap nothing -- stay a few
+// percent), 4 for device-resident stacks (two batches per internal stream; measured on config 2: 134 vs 128 GVoxel/s)
+static int default_batch(const mvd_handle* h, int n_planes, int min_batches) {
     if (h->batch_planes > 0)
         return h->path == MVD_PATH_FFT ? even_up(h->batch_planes) : std::min(h->batch_planes, n_planes);
-    // ~64 MiB of uint16 input per batch, at least 16 batches when the stack allows it so that the
-    // pipeline's fill and drain (one H2D and one D2H that overlap nothing) stay a few percent
+    // ~64 MiB of uint16 input per batch
     const size_t per_plane = (size_t)h->uW * h->uH * sizeof(uint16_t) * h->V;
     size_t b = std::max<size_t>(1, ((size_t)64 << 20) / per_plane);
-    b = std::min<size_t>(b, std::max(1, n_planes / 16));
+    if (min_batches < 16 && h->path == MVD_PATH_FFT) {
+        // Device-resident stacks on the FFT engine: two batches are in flight, each cycling its Z and S (8 B per
+        // plane-pixel together) through all T x V passes.  When two such working sets fit the 126 MB L2 with at
+        // least five planes per batch the passes run largely from L2 (measured: configs 2 / 3 / 5 best
+        // at 64 / 8-16 / 4-6 planes); when they cannot (config 4: 13 MB per plane), long launches win instead
+        // (~32 Mvoxel per batch: 99 vs 95 GVoxel/s at 10 planes).
+        const size_t npx = (size_t)h->W * h->H;
+        const size_t fit = (size_t)100e6 / (16 * npx);
+        b = fit >= 5 ? fit : std::max<size_t>(1, ((size_t)32 << 20) / npx);
+    }
+    b = std::min<size_t>(b, std::max(1, n_planes / min_batches));
     // ... but never batches so small that a launch has nothing to chew on: at least ~2 Mvoxel
     // (config 1's 8 planes of 64 x 64 stay one batch)
     const size_t floor_planes = (((size_t)2 << 20) + (size_t)h->uW * h->uH - 1) / ((size_t)h->uW * h->uH);
@@ -736,7 +749,8 @@ int mvd_profile_read(mvd_handle* h, float* ms, long long* n) {
 const char* mvd_kernel_class_name(int k) {
     static const char* names[MVD_N_KERNEL_CLASSES] = {
         "init_mean", "direct_blur_ratio", "direct_backproject_update", "fft_rows_first",
-        "fft_cols_otf", "fft_rows_ratio", "fft_rows_update", "setup", "guard_repair", "small_resident"};
+        "fft_cols_otf", "fft_rows_ratio", "fft_rows_update", "setup", "guard_repair", "small_resident",
+        "sep_blur_ratio", "sep_backproject_update"};
     return (k >= 0 && k < MVD_N_KERNEL_CLASSES) ? names[k] : nullptr;
 }
 

@@ -657,15 +657,17 @@ int direct_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cu
             const float* Gback = h->d_coef + ((size_t)v * 2 + 1) * per;
             const uint16_t* phi = io.views + (size_t)v * io.lay.view;
             int e;
+            const float* wv = io.weights ? io.weights + (size_t)v * io.w_view : nullptr;
             {
-                LaunchScope ls(h, KC_DIRECT_BLUR_RATIO, stream);
-                e = launch_corr(0, h, psi, Gblur, phi, r, n_planes, stream, io.lay.plane, io.lay.row, nullptr);
+                LaunchScope ls(h, h->sep ? KC_SEP_BLUR_RATIO : KC_DIRECT_BLUR_RATIO, stream);
+                e = h->sep ? sep_launch(0, h, v, psi, phi, r, n_planes, stream, io.lay.plane, io.lay.row, nullptr)
+                           : launch_corr(0, h, psi, Gblur, phi, r, n_planes, stream, io.lay.plane, io.lay.row, nullptr);
             }
             MVD_TRY(h, (cudaError_t)e);
             {
-                LaunchScope ls(h, KC_DIRECT_BACK_UPDATE, stream);
-                e = launch_corr(1, h, r, Gback, nullptr, psi, n_planes, stream, 0, 0,
-                                io.weights ? io.weights + (size_t)v * io.w_view : nullptr);
+                LaunchScope ls(h, h->sep ? KC_SEP_BACK_UPDATE : KC_DIRECT_BACK_UPDATE, stream);
+                e = h->sep ? sep_launch(1, h, v, r, nullptr, psi, n_planes, stream, 0, 0, wv)
+                           : launch_corr(1, h, r, Gback, nullptr, psi, n_planes, stream, 0, 0, wv);
             }
             MVD_TRY(h, (cudaError_t)e);
         }

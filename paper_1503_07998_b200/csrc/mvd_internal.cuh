@@ -19,9 +19,11 @@ enum KernelClass {
     KC_FFT_ROWS_UPDATE,      // inverse row FFT -> q, a4 update, forward row FFT of the new psi
     KC_SETUP,                // mvd_create-time kernels (OTF construction)
     KC_GUARD_REPAIR,         // FFT engine's guard: flagged plane pairs recomputed with the direct engine's arithmetic
-    KC_SMALL_RESIDENT        // whole RL run of a small plane pair on chip, one launch
+    KC_SMALL_RESIDENT,       // whole RL run of a small plane pair on chip, one launch
+    KC_SEP_BLUR_RATIO,       // a1+a2 with a separable PSF: x pass, z pass, ratio
+    KC_SEP_BACK_UPDATE       // a3+a4 with a separable PSF
 };
-static_assert(KC_SMALL_RESIDENT + 1 == MVD_N_KERNEL_CLASSES, "kernel class table and mvd.h disagree");
+static_assert(KC_SEP_BACK_UPDATE + 1 == MVD_N_KERNEL_CLASSES, "kernel class table and mvd.h disagree");
 
 struct ProfRecord {
     int kc;
@@ -60,6 +62,10 @@ struct mvd_handle {
     int Kp = 0;   // padded number of PSF rows (multiple of the kernel's row chunk)
     int JC = 0;   // row chunk of the direct kernel chosen for K
     bool direct_pair = false;   // the two-plane FFMA2 kernel serves this plan (its float2 tile fits in shared memory)
+    // separable fast path of the direct engine (mvd_sep.cu): every P_v is an outer product u_v w_v^T
+    bool sep = false;
+    float* d_sep = nullptr;     // [V][2 (a1, a3)][2 (z taps, x taps)][sepKp]
+    int sepKp = 0;
 
     // fft path: optical transfer functions, float2 [V][H][W], pre-scaled by 1/(W*H)
     float2* d_otf = nullptr;
@@ -151,6 +157,12 @@ int direct_setup(mvd_handle* h, const float* host_psfs, const float* host_xs);
 size_t direct_scratch_bytes(const mvd_handle* h, int n_planes);
 // views: view v of plane p at views + (v * view_stride + p * H * W); out: [n][H][W]
 int direct_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cudaStream_t stream);
+
+// ---- separable fast path (mvd_sep.cu) -----------------------------------------------------------
+bool sep_psfs_separable(int n_views, const float* psfs, int K);   // host only
+int sep_setup(mvd_handle* h, const float* host_psfs);              // sets h->sep when the plan qualifies
+int sep_launch(int mode, const mvd_handle* h, int v, const float* src, const uint16_t* phi, float* dst, int n_planes,
+               cudaStream_t st, size_t phi_plane, size_t phi_row, const float* wgt);
 
 bool direct_small_available(const mvd_handle* h);
 bool direct_repair_available(const mvd_handle* h);
