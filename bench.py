@@ -273,6 +273,8 @@ def algorithmic_work(cls, cfg, n_planes, K):
         "init_mean": (vox * (2 * cfg.V + 4), "B"),
         "direct_blur_ratio": (vox * 2.0 * K * K, "flop"),          # K^2 FMA per voxel
         "direct_backproject_update": (vox * 2.0 * K * K, "flop"),
+        "sep_blur_ratio": (vox * 2.0 * 2 * K, "flop"),             # separable PSF: K FMA per voxel and pass, two passes
+        "sep_backproject_update": (vox * 2.0 * 2 * K, "flop"),
         "fft_rows_first": (vox * (2 * cfg.V + 4 + 4), "B"),        # phi_v u16 in, psi + row spectrum out
         "fft_cols_otf": (vox * 8, "B"),                            # spectrum in + out (OTF is L2-resident)
         "fft_rows_ratio": (vox * 10, "B"),                         # spectrum in, phi u16 in, spectrum out

@@ -152,7 +152,7 @@ static int create_impl(int plane_w, int plane_h, int n_views, const float* psfs,
     int rc = mvd_check(h, cudaGetDevice(&h->device));
     if (rc == MVD_OK) rc = mvd_check(h, cudaDeviceGetAttribute(&h->n_sm, cudaDevAttrMultiProcessorCount, h->device));
     if (rc == MVD_OK) rc = path == MVD_PATH_FFT ? fft_setup(h, psfs, xs) : direct_setup(h, psfs, xs);
-    if (rc == MVD_OK && path == MVD_PATH_DIRECT && !getenv("MVD_NO_SEPARABLE")) rc = sep_setup(h, psfs);
+    if (rc == MVD_OK && path == MVD_PATH_DIRECT) rc = sep_setup(h, psfs);
     if (rc != MVD_OK) {
         // keep the cuda error visible to the caller through the return code only
         mvd_destroy(h);

@@ -28,7 +28,7 @@ constexpr int NT = 256;      // threads per CTA
 constexpr int RS = 128;      // staged rows per tile (outputs + halo)
 constexpr int TX = 32;       // output columns per tile
 constexpr int RX = 16;       // outputs per thread in the x pass
-constexpr int P1 = RS + 1;   // pitch of the transposed source tile (float2)
+constexpr int P1 = RS + 2;   // pitch of the transposed source tile (float2): 4 P1 = 8 mod 16, see the staging loop
 constexpr int P2 = TX + 1;   // pitch of the intermediate (float2)
 constexpr int NSTRIP = NT / TX;   // strips of the z pass
 
@@ -38,6 +38,13 @@ __device__ __forceinline__ float2 ffma2_b(float g, float2 w, float2 c) {
         "fma.rn.f32x2 rd, ra, rb, rc; mov.b64 {%0,%1}, rd; }"
         : "=f"(r.x), "=f"(r.y) : "f"(g), "f"(w.x), "f"(w.y), "f"(c.x), "f"(c.y));
     return r;
+}
+
+// staged columns of a tile: the alignment shift of the vectorised staging + TX + K - 1, rounded up to whole float4 groups
+__host__ __device__ constexpr int sep_swa(int K) { return ((4 - ((K - 1) / 2) % 4) % 4 + TX + K - 1 + 3) & ~3; }
+
+__device__ __forceinline__ void cp_async4(float* dst, const float* src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"((uint32_t)__cvta_generic_to_shared(dst)), "l"(src) : "memory");
 }
 
 // acc[0 .. N) += sum_{j < JC} g[j] * win[m + j]: a JC-tap chunk of a sliding window, everything in registers
@@ -61,7 +68,7 @@ struct SepArgs {
 };
 
 // KT > 0: K known at compile time, JC == KT (one fully unrolled window); KT == 0: runtime K in chunks of JC taps.
-template <int KT, int JC, int MODE>
+template <int KT, int JC, int MODE, bool VEC, bool WGT>
 __global__ void __launch_bounds__(NT, 2) sep_corr2_kernel(SepArgs a) {
     extern __shared__ __align__(16) float2 sep_smem[];
     const int K = KT > 0 ? KT : a.K, Kp = KT > 0 ? KT : a.Kp;
@@ -72,11 +79,12 @@ __global__ void __launch_bounds__(NT, 2) sep_corr2_kernel(SepArgs a) {
     // The windows of the last strips reach a few rows / columns past the tile: those are zero-filled spares
     // (ZC spare columns of sT for the chunked runtime-K window, ZR spare rows of tt), so no load needs a guard.
     constexpr int ZC = KT > 0 ? 0 : 8, ZR = 16;
-    float2* sT = sep_smem;                            // [SW + ZC][P1]
-    float2* tt = sep_smem + (size_t)(SW + ZC) * P1;   // [RS + ZR][P2]
+    const int SWA = sep_swa(K);                       // staged columns incl. the alignment shift (<= 3) of the VEC path
+    float2* sT = sep_smem;                            // [SWA + ZC][P1]
+    float2* tt = sep_smem + (size_t)(SWA + ZC) * P1;  // [RS + ZR][P2]
     float* sg = reinterpret_cast<float*>(tt + (size_t)(RS + ZR) * P2);   // [2][Kp]
     const int tid = threadIdx.x;
-    for (int k = tid; k < ZC * P1; k += NT) sT[(size_t)SW * P1 + k] = make_float2(0.f, 0.f);
+    for (int k = tid; k < ZC * P1; k += NT) sT[(size_t)SWA * P1 + k] = make_float2(0.f, 0.f);
     for (int k = tid; k < ZR * P2; k += NT) tt[(size_t)RS * P2 + k] = make_float2(0.f, 0.f);
 
     int b = blockIdx.x;
@@ -90,7 +98,51 @@ __global__ void __launch_bounds__(NT, 2) sep_corr2_kernel(SepArgs a) {
     const int x0 = tile_x * TX, y0 = tile_y * TY;
 
     for (int k = tid; k < 2 * Kp; k += NT) sg[k] = a.taps[k];
-    {   // 1. stage, transposed: sT[tx][ty] = src(y0 - c + ty, x0 - c + tx) of both planes, periodic
+    // 1. stage, transposed: sT[shift + tx][ty] = src(y0 - c + ty, x0 - c + tx) of both planes, periodic.
+    // VEC (W a multiple of 4, 16-byte aligned planes): the staged columns start at the multiple of 4 below x0 - c
+    // (`shift` columns earlier; x0 is a multiple of 32), so every row is whole float4 groups that never straddle the
+    // wrap.  A warp takes 8 rows x 4 groups at a time: its loads are 64 contiguous bytes per row, and its transposed
+    // 8-byte stores land in 16 distinct banks per half-warp (rows: 8 consecutive words; groups: 4 P1 words apart =
+    // 8 banks further).  One row block's loads are all issued before its first store.
+    const int shift = VEC ? (4 - c % 4) % 4 : 0;
+    if (VEC) {
+        const int G = (shift + SW + 3) / 4;                       // float4 groups per staged row
+        constexpr int GBMAX = KT > 0 ? ((4 - ((KT - 1) / 2) % 4) % 4 + TX + KT - 1 + 15) / 16 : (TX + 64 + 3 + 15) / 16;
+        const int lane = tid & 31, warp = tid >> 5;
+        const int xa = x0 - c - shift;
+        const float4* spa = reinterpret_cast<const float4*>(a.src + offa);
+        const float4* spb = reinterpret_cast<const float4*>(a.src + offb);
+        constexpr int NRB = RS / 8 / (NT / 32);                 // row blocks per warp (2)
+        float4 va[NRB][GBMAX], vb[NRB][GBMAX];
+#pragma unroll
+        for (int r = 0; r < NRB; ++r) {
+            const int ty = 8 * (warp + r * (NT / 32)) + (lane & 7);
+            int gy = (y0 - c + ty) % H;
+            if (gy < 0) gy += H;
+#pragma unroll
+            for (int gb = 0; gb < GBMAX; ++gb) {   // branch-free: groups past the end repeat the last one
+                const int grp = min(4 * gb + (lane >> 3), G - 1);
+                int gx = (xa + 4 * grp) % W;
+                if (gx < 0) gx += W;
+                const size_t g = ((size_t)gy * W + gx) >> 2;
+                va[r][gb] = spa[g];
+                vb[r][gb] = spb[g];
+            }
+        }
+#pragma unroll
+        for (int r = 0; r < NRB; ++r) {
+            const int ty = 8 * (warp + r * (NT / 32)) + (lane & 7);
+#pragma unroll
+            for (int gb = 0; gb < GBMAX; ++gb) {
+                const int grp = min(4 * gb + (lane >> 3), G - 1);   // (repeated groups store the same values again)
+                float2* d = sT + (size_t)(4 * grp) * P1 + ty;
+                d[0] = make_float2(va[r][gb].x, vb[r][gb].x);
+                d[P1] = make_float2(va[r][gb].y, vb[r][gb].y);
+                d[2 * P1] = make_float2(va[r][gb].z, vb[r][gb].z);
+                d[3 * P1] = make_float2(va[r][gb].w, vb[r][gb].w);
+            }
+        }
+    } else {
         const float* spa = a.src + offa;
         const float* spb = a.src + offb;
         const int lane = tid & 31, warp = tid >> 5;
@@ -99,20 +151,55 @@ __global__ void __launch_bounds__(NT, 2) sep_corr2_kernel(SepArgs a) {
             if (gx < 0) gx += W;
             int gy = (y0 - c + warp) % H;
             if (gy < 0) gy += H;
+#pragma unroll 4
             for (int ty = warp; ty < RS; ty += NT / 32) {
                 const size_t g = (size_t)gy * W + gx;
-                sT[tx * P1 + ty] = make_float2(spa[g], spb[g]);
+                float2* d = sT + tx * P1 + ty;
+                cp_async4(&d->x, spa + g);
+                cp_async4(&d->y, spb + g);
                 gy += NT / 32;
-                while (gy >= H) gy -= H;
+                if (gy >= H) gy = H >= NT / 32 ? gy - H : gy % H;
             }
         }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+        asm volatile("cp.async.wait_group 0;" ::: "memory");
     }
     __syncthreads();
+
+    // The epilogue's operands (phi, or the old psi and the weights) are requested now, so that their latency hides
+    // behind the two passes (and no load has to wait for a store the compiler cannot prove independent).
+    // (Branch-free: coordinates past the plane are clamped, the values discarded later; phi stays uint16 until then.)
+    const int ex = tid % TX, eys = (tid / TX) * RYC, gxo = x0 + ex;
+    const int gxc = min(gxo, W - 1);
+    float ea[MODE == 1 ? RYC : 1], eb[MODE == 1 ? RYC : 1], wa[WGT ? RYC : 1], wb[WGT ? RYC : 1];
+    unsigned short ua[MODE == 0 ? RYC : 1], ub[MODE == 0 ? RYC : 1];
+#pragma unroll
+    for (int m = 0; m < RYC; ++m) {
+        const int yc = min(y0 + eys + m, H - 1);
+        const size_t q = (size_t)yc * W + gxc;
+        if constexpr (MODE == 0) {
+            const size_t f = (size_t)pa * a.phi_plane + (size_t)yc * a.phi_row + gxc;
+            ua[m] = __ldg(a.phi + f);
+            ub[m] = __ldg(a.phi + (has_b ? f + a.phi_plane : f));
+        } else {
+            ea[m] = a.dst[offa + q];
+            eb[m] = a.dst[offb + q];
+        }
+    }
+    if constexpr (WGT) {
+#pragma unroll
+        for (int m = 0; m < RYC; ++m) {
+            const int yc = min(y0 + eys + m, H - 1);
+            const size_t q = (size_t)yc * W + gxc;
+            wa[m] = __ldg(a.wgt + offa + q);
+            wb[m] = __ldg(a.wgt + offb + q);
+        }
+    }
 
     {   // 2. x pass: t(ty, x) = sum_i gx[i] s(ty, x + i)
         const int ty = tid % RS, xs = (tid / RS) * RX;
         const float* gx = sg + Kp;
-        const float2* col = sT + (size_t)xs * P1 + ty;
+        const float2* col = sT + (size_t)(xs + shift) * P1 + ty;
         float2 acc[RX];
 #pragma unroll
         for (int m = 0; m < RX; ++m) acc[m] = make_float2(0.f, 0.f);
@@ -147,26 +234,23 @@ __global__ void __launch_bounds__(NT, 2) sep_corr2_kernel(SepArgs a) {
             for (int j = 0; j < JC; ++j) g[j] = gz[jc + j];
             window_fma<RYC, JC>(acc, win, g);
         }
-        const int gxo = x0 + x;
         if (gxo < W) {
 #pragma unroll
             for (int m = 0; m < RYC; ++m) {
                 const int ly = ys + m, y = y0 + ly;
                 if (ly < TY && y < H) {
                     const size_t q = (size_t)y * W + gxo;
-                    if (MODE == 0) {                                              // a2
-                        const size_t f = (size_t)pa * a.phi_plane + (size_t)y * a.phi_row + gxo;
-                        a.dst[offa + q] = (float)a.phi[f] / fmaxf(acc[m].x, a.eps);
-                        if (has_b) a.dst[offb + q] = (float)a.phi[f + a.phi_plane] / fmaxf(acc[m].y, a.eps);
-                    } else {                                                      // a4
+                    if constexpr (MODE == 0) {                                    // a2
+                        a.dst[offa + q] = __fdividef((float)ua[m], fmaxf(acc[m].x, a.eps));      // 2 ulp, reading A16
+                        if (has_b) a.dst[offb + q] = __fdividef((float)ub[m], fmaxf(acc[m].y, a.eps));
+                    } else {                                                      // a4 (a4w: q <- w q + 1 - w)
                         float qa = acc[m].x, qb = acc[m].y;
-                        if (a.wgt) {                                              // a4w
-                            const float w0 = __ldg(a.wgt + offa + q), w1 = has_b ? __ldg(a.wgt + offb + q) : 0.f;
-                            qa = fmaf(w0, qa, 1.f - w0);
-                            qb = fmaf(w1, qb, 1.f - w1);
+                        if constexpr (WGT) {
+                            qa = fmaf(wa[m], qa, 1.f - wa[m]);
+                            qb = fmaf(wb[m], qb, 1.f - wb[m]);
                         }
-                        a.dst[offa + q] *= qa;
-                        if (has_b) a.dst[offb + q] *= qb;
+                        a.dst[offa + q] = ea[m] * qa;
+                        if (has_b) a.dst[offb + q] = eb[m] * qb;
                     }
                 }
             }
@@ -176,23 +260,29 @@ __global__ void __launch_bounds__(NT, 2) sep_corr2_kernel(SepArgs a) {
 
 size_t sep_smem_bytes(int K, int Kp) {
     const bool templated = Kp == K;
-    return sizeof(float2) * ((size_t)(TX + K - 1 + (templated ? 0 : 8)) * P1 + (size_t)(RS + 16) * P2) + sizeof(float) * 2 * Kp;
+    return sizeof(float2) * ((size_t)(sep_swa(K) + (templated ? 0 : 8)) * P1 + (size_t)(RS + 16) * P2) + sizeof(float) * 2 * Kp;
+}
+
+template <int KT, int JC, int MODE, bool VEC, bool WGT = false>
+int launch_sep_one(const SepArgs& a, size_t smem, unsigned grid, cudaStream_t st) {
+    static size_t opted = 0;
+    if (smem > opted) {
+        cudaError_t e = cudaFuncSetAttribute(sep_corr2_kernel<KT, JC, MODE, VEC, WGT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return (int)e;
+        opted = smem;
+    }
+    sep_corr2_kernel<KT, JC, MODE, VEC, WGT><<<grid, NT, smem, st>>>(a);
+    return (int)cudaGetLastError();
 }
 
 template <int KT, int JC>
 int launch_sep(int mode, const SepArgs& a, cudaStream_t st) {
     const size_t smem = sep_smem_bytes(a.K, a.Kp);
-    static size_t opted[2] = {0, 0};
-    if (smem > opted[mode]) {
-        cudaError_t e = mode == 0 ? cudaFuncSetAttribute(sep_corr2_kernel<KT, JC, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem)
-                                  : cudaFuncSetAttribute(sep_corr2_kernel<KT, JC, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return (int)e;
-        opted[mode] = smem;
-    }
     const unsigned grid = (unsigned)((size_t)a.tiles_x * a.tiles_y * ((a.n_planes + 1) / 2));
-    if (mode == 0) sep_corr2_kernel<KT, JC, 0><<<grid, NT, smem, st>>>(a);
-    else sep_corr2_kernel<KT, JC, 1><<<grid, NT, smem, st>>>(a);
-    return (int)cudaGetLastError();
+    const bool vec = a.W % 4 == 0 && ((uintptr_t)a.src & 15u) == 0;   // planes are W H floats apart: aligned too
+    if (mode == 0) return vec ? launch_sep_one<KT, JC, 0, true>(a, smem, grid, st) : launch_sep_one<KT, JC, 0, false>(a, smem, grid, st);
+    if (a.wgt) return vec ? launch_sep_one<KT, JC, 1, true, true>(a, smem, grid, st) : launch_sep_one<KT, JC, 1, false, true>(a, smem, grid, st);
+    return vec ? launch_sep_one<KT, JC, 1, true>(a, smem, grid, st) : launch_sep_one<KT, JC, 1, false>(a, smem, grid, st);
 }
 
 }  // namespace
