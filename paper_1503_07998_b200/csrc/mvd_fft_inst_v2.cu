@@ -34,6 +34,7 @@ const SizeOps* mvd_fft_ops_v2(int N) {
             if (N == 2048 && v[0] == 'u') { static const SizeOps o = OpsFor2<P2048, 128, P2048, 256, false, 2, false, 4, 3>::make(); return &o; }
             if (N == 800 && v[0] == 'o') { static const SizeOps o = ColsNu2<25, 32, 128, 4>::make(); return &o; }
             if (N == 800 && v[0] == 'a') { static const SizeOps o = ColsOnly2<P800C, 320, false, 1, 8>::make(); return &o; }
+            if (N == 2048 && v[0] == 'f') { static const SizeOps o = OpsFor2<ShflTail<P2048>, 128, P2048, 256, false, 2, false, 4, 4>::make(); return &o; }
             if (N == 2048 && v[0] == 'a') { static const SizeOps o = OpsFor2<Plan<2048, 16, 16, 16, 8>, 256, P2048, 256, false, 2, false, 4, 3>::make(); return &o; }
             if (N == 2048 && v[0] == 'b') { static const SizeOps o = OpsFor2<Plan<2048, 16, 16, 16, 8>, 512, P2048, 256, false, 2, false, 4, 2>::make(); return &o; }
             if (N == 1024 && v[0] == 'a') { static const SizeOps o = OpsFor2<P1024, 256, Plan<1024, 16, 16, 16, 4>, 256, false, 2>::make(); return &o; }
