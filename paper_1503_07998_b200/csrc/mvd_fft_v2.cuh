@@ -37,10 +37,8 @@ __device__ __forceinline__ void prefetch_l2(const void* p, uint32_t bytes) {
 template <class P>
 __device__ __forceinline__ int swz(int p) {
     constexpr int R0 = P::radix(0);
-    static_assert(R0 == 16 || R0 == 32 || R0 == 40, "the XOR swizzle is derived for first radices 16, 32 and 40");
-    // R0 = 40 (length 800, eight columns per team, two positions per half-warp): only the parity has to
-    // differ between neighbouring threads of stage 0 (positions 40 t + m), and p ^ 1 stays inside its block of 40
-    return R0 == 40 ? p ^ ((p / R0) & 1) : p ^ ((p / R0) & 15);
+    static_assert(R0 == 16 || R0 == 32, "the XOR swizzle is derived for first radices 16 and 32");
+    return p ^ ((p / R0) & 15);
 }
 // one FFT per region of N slots
 template <class P>
@@ -370,7 +368,7 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 // box load of the NEXT item into the team's exchange region when the inverse transform has done its
 // last exchange, and the box store of the results from a second region -- no global load or store
 // instruction, and no L1 tag traffic, is left in the loop.
-template <class P, int NT, bool OTF_REGS, int MINB, int CPT = 4, bool EARLY = false>
+template <class P, int NT, bool OTF_REGS, int MINB, int CPT = 4>
 __global__ void __launch_bounds__(NT, MINB)
 fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap omap,
                      const float2* __restrict__ otf, int conj_otf, int pairs, int W, const float2* __restrict__ tw_g) {
@@ -382,12 +380,10 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
     constexpr int TW = (P::S - 1) * E * TPF;                  // a multiple of 16 float2: regions stay 128-byte aligned
     static_assert(TW % 16 == 0, "twiddle table keeps the regions aligned");
     float2* tw = smem_cols3;                                  // [(S-1) E][TPF]
-    // EARLY: a dedicated landing zone per team (the next item is requested a whole item ahead) next to
-    // the exchange region; otherwise the exchange region is the landing zone
-    float2* buf = smem_cols3 + TW;                            // [NTEAM][H][CPT]  exchange regions (/ landing zones)
-    float2* obuf = buf + NTEAM * H * CPT;                     // [NTEAM][H][CPT]  results on their way out
-    float2* lbuf = EARLY ? obuf + NTEAM * H * CPT : buf;      // [NTEAM][H][CPT]  landing zones
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_cols3 + TW + (EARLY ? 3 : 2) * NTEAM * H * CPT);   // [2][NTEAM]
+    // the exchange region is the landing zone of the next item
+    float2* buf = smem_cols3 + TW;                            // [NTEAM][H][CPT]  exchange regions / landing zones
+    float2* obuf = buf + NTEAM * H * CPT;                     // [NTEAM][H][CPT]  OTF slices, then results on their way out
+    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_cols3 + TW + 2 * NTEAM * H * CPT);   // [2][NTEAM]
     if (threadIdx.x < 2 * NTEAM) mbar_init(&bars[threadIdx.x], 1);
     if (threadIdx.x == 0) fence_mbar_init();
     for (int k = threadIdx.x; k < TW; k += NT) tw[k] = tw_g[k];
@@ -398,7 +394,7 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
     const ColAddr2<P, CPT> addr{team * H * CPT + c4};
     const TeamSync<TEAM> sync{team};
     const float sgn = conj_otf ? -1.f : 1.f;
-    float2* land = lbuf + team * H * CPT;
+    float2* land = buf + team * H * CPT;
     float2* outz = obuf + team * H * CPT;
     uint64_t* full = &bars[team];
     uint64_t* full_otf = &bars[NTEAM + team];   // !OTF_REGS: the team's OTF slice lands in the out region
@@ -437,7 +433,6 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
 #pragma unroll
         for (int e = 0; e < E; ++e) x[e] = land[(t + TPF * e) * CPT + c4];
         sync();
-        if (EARLY && l == 0 && item + (int)gridDim.x < items) issue(item + gridDim.x);
         if (!OTF_REGS && l == 0) {
             // The OTF slice of these columns (same tile-major tensor shape as S, one "pair" per view)
             // comes through the TMA unit into the out region, which the previous item's results have
@@ -466,7 +461,7 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
         }
         fft_run_head<P, +1>(x, buf, tw, t, addr, sync);
         if (l == 0) {
-            if (!EARLY && item + (int)gridDim.x < items) issue(item + gridDim.x);
+            if (item + (int)gridDim.x < items) issue(item + gridDim.x);
             if (OTF_REGS) bulk_wait_read();   // the previous item's results have left the out region
         }
         fft_run_tail<P, +1>(x, buf, tw, t, addr, sync);
@@ -483,85 +478,6 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
         }
     }
     if (l == 0) bulk_wait_read();
-}
-
-// Lean column pass: ONE shared-memory region per team.  The team's slice arrives by TMA in the exchange
-// region (requested when the previous item's inverse transform has done its last exchange), the OTF
-// slice is read straight from L2 into registers (CPT >= 8: whole 64-byte segments per eight lanes) and
-// the results leave by plain stores from registers.  Half the shared memory and ~40 % less shared-memory
-// traffic per element than fft2_cols_tma_kernel, so a third (or fourth) team fits on an SM: the pass is
-// bound by barrier and exchange latency at two teams per SM, not by a pipe (profiles/r2_c4_ncu.md).
-__device__ __forceinline__ float2 ldg_nc_na(const float2* p) {
-    float2 r;
-    asm volatile("ld.global.nc.L1::no_allocate.v2.f32 {%0, %1}, [%2];" : "=f"(r.x), "=f"(r.y) : "l"(p));
-    return r;
-}
-template <class P, int NT, int MINB, int CPT>
-__global__ void __launch_bounds__(NT, MINB)
-fft2_cols_lean_kernel(const __grid_constant__ CUtensorMap tmap, float2* __restrict__ S, const float2* __restrict__ otf,
-                      int conj_otf, int pairs, int W, const float2* __restrict__ tw_g) {
-    constexpr int E = P::E, TPF = P::TPF, H = P::N, TEAM = CPT * TPF, NTEAM = NT / TEAM, TC = CPT * NTEAM;
-    constexpr int BOXH = H <= 256 ? H : (H % 256 == 0 ? 256 : 200);
-    static_assert(H % BOXH == 0 && (CPT == 4 || CPT == 8 || CPT == 16), "whole boxes; a team owns whole 32-byte sectors of a row");
-    static_assert(NT % TEAM == 0 && TEAM % 32 == 0 && (TEAM == 32 || NTEAM <= 15), "column teams are whole warps");
-    extern __shared__ __align__(128) float2 smem_cols4[];
-    constexpr int TW = (P::S - 1) * E * TPF;
-    static_assert(TW % 16 == 0, "twiddle table keeps the regions aligned");
-    float2* tw = smem_cols4;                                  // [(S-1) E][TPF]
-    float2* buf = smem_cols4 + TW;                            // [NTEAM][H][CPT]  exchange regions = landing zones
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_cols4 + TW + NTEAM * H * CPT);   // [NTEAM]
-    if (threadIdx.x < NTEAM) mbar_init(&bars[threadIdx.x], 1);
-    if (threadIdx.x == 0) fence_mbar_init();
-    for (int k = threadIdx.x; k < TW; k += NT) tw[k] = tw_g[k];
-    __syncthreads();
-    pdl_launch_dependents();
-    const int team = threadIdx.x / TEAM, l = threadIdx.x % TEAM;
-    const int c4 = l % CPT, t = l / CPT;
-    const ColAddr2<P, CPT> addr{team * H * CPT + c4};
-    const TeamSync<TEAM> sync{team};
-    const float sgn = conj_otf ? -1.f : 1.f;
-    float2* land = buf + team * H * CPT;
-    uint64_t* full = &bars[team];
-    const int tiles = W / TC;
-    const int items = tiles * pairs;
-    auto first_col = [&](int item) { return (item % tiles) * TC + team * CPT; };
-    auto plane_off = [&](int x) { return (size_t)(x >> 4) * (H * 16) + (x & 15); };
-    auto box_x = [&](int item) { return 2 * (first_col(item) & 15); };
-    auto box_y = [&](int item) { return ((item / tiles) * (W / 16) + (first_col(item) >> 4)) * H; };
-    auto issue = [&](int item) {   // one lane
-        fence_proxy_async();
-        mbar_arrive_expect_tx(full, (uint32_t)(sizeof(float2) * H * CPT));
-#pragma unroll
-        for (int b = 0; b < H / BOXH; ++b) tma_2d_g2s(land + b * BOXH * CPT, &tmap, box_x(item), box_y(item) + b * BOXH, full);
-    };
-
-    int item = blockIdx.x;
-    pdl_wait();
-    if (item < items && l == 0) issue(item);
-    uint32_t phase = 0;
-    for (; item < items; item += gridDim.x) {
-        const int xg = first_col(item) + c4;
-        const float2* op = otf + plane_off(xg) + (size_t)t * 16;
-        float2* Sp = S + (size_t)(item / tiles) * H * W + plane_off(xg) + (size_t)t * 16;
-        float2 x[E];
-        mbar_wait(full, phase);
-        phase ^= 1;
-#pragma unroll
-        for (int e = 0; e < E; ++e) x[e] = land[(t + TPF * e) * CPT + c4];
-        sync();
-        fft_run<P, -1>(x, buf, tw, t, addr, sync);
-#pragma unroll
-        for (int e = 0; e < E; ++e) {
-            float2 w = ldg_nc_na(op + (size_t)(TPF * e) * 16);
-            w.y *= sgn;
-            x[e] = cmul(x[e], w);
-        }
-        fft_run_head<P, +1>(x, buf, tw, t, addr, sync);
-        if (l == 0 && item + (int)gridDim.x < items) issue(item + gridDim.x);
-        fft_run_tail<P, +1>(x, buf, tw, t, addr, sync);
-#pragma unroll
-        for (int e = 0; e < E; ++e) Sp[(size_t)(TPF * e) * 16] = x[e];
-    }
 }
 
 // Column pass for lengths H = RA x RB whose two radices differ (800 = 25 x 32): a two-stage transform in which the
@@ -697,7 +613,7 @@ inline cudaError_t launch_pdl(Kern kern, dim3 grid, dim3 block, size_t smem, cud
     return cudaLaunchKernelEx(&cfg, kern, args...);
 }
 
-template <class P, int NT, class PC, int NTC, bool OTF_REGS, int MINB, bool TMA = true, int CPT = 4, int RMINB = 2, bool EARLY = false>
+template <class P, int NT, class PC, int NTC, bool OTF_REGS, int MINB, bool TMA = true, int CPT = 4, int RMINB = 2>
 struct OpsFor2 {
     static_assert(P::N == PC::N, "row and column plan of one entry describe the same length");
     static constexpr size_t kRowSmem = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * P::N);
@@ -705,7 +621,7 @@ struct OpsFor2 {
     static constexpr int kRowCpsW = (int)((228u * 1024u) / (kRowSmemW + 1024)) < RMINB ? (int)((228u * 1024u) / (kRowSmemW + 1024)) : RMINB;
     static_assert(kRowSmemW <= 227u * 1024u && kRowCpsW >= 1, "the weighted update kernel fits one CTA");
     static constexpr int kTeam = CPT * PC::TPF, kNTeam = NTC / kTeam, kTC = CPT * kNTeam;
-    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)(TMA ? (EARLY ? 3 : 2) : 1) * kNTeam * PC::N * CPT) +
+    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)(TMA ? 2 : 1) * kNTeam * PC::N * CPT) +
                                        (TMA ? 2 * sizeof(uint64_t) * kNTeam : 0);
 
     static cudaError_t rows(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st) {
@@ -717,7 +633,7 @@ struct OpsFor2 {
     static cudaError_t cols(const CUtensorMap& tmap, const CUtensorMap& otf_map, float2* S, const float2* otf, int conj_otf, int pairs, int W,
                             const float2* tw, dim3 grid, cudaStream_t st) {
         if constexpr (TMA)
-            return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT, EARLY>, grid, dim3(NTC), kColSmem, st, tmap, otf_map, otf, conj_otf, pairs, W, tw);
+            return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, grid, dim3(NTC), kColSmem, st, tmap, otf_map, otf, conj_otf, pairs, W, tw);
         else
         return launch_pdl(fft2_cols_kernel<PC, NTC, OTF_REGS, MINB>, grid, dim3(NTC), kColSmem, st, S, otf, conj_otf, pairs, W, tw);
     }
@@ -733,7 +649,7 @@ struct OpsFor2 {
     }
     static cudaError_t prepare_cols() {
         if constexpr (TMA)
-            return cudaFuncSetAttribute(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT, EARLY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
+            return cudaFuncSetAttribute(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
         else
         return cudaFuncSetAttribute(fft2_cols_kernel<PC, NTC, OTF_REGS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
     }
@@ -751,65 +667,6 @@ struct OpsFor2 {
         o.row_cps_w = kRowCpsW;
         o.col_cps = MINB;
         o.col_otf_regs = OTF_REGS ? 1 : 0;
-        return o;
-    }
-};
-
-// A length that only has a generation-2 COLUMN kernel (800 = 40 x 20: its 20-thread FFTs are not
-// warp-aligned, so eight columns form a team of five warps).
-template <class PC, int NTC, bool OTF_REGS, int MINB, int CPT>
-struct ColsOnly2 {
-    static constexpr int kTeam = CPT * PC::TPF, kNTeam = NTC / kTeam, kTC = CPT * kNTeam;
-    static constexpr int kBoxH = PC::N <= 256 ? PC::N : (PC::N % 256 == 0 ? 256 : 200);
-    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)2 * kNTeam * PC::N * CPT) +
-                                       2 * sizeof(uint64_t) * kNTeam;
-    static cudaError_t cols(const CUtensorMap& tmap, const CUtensorMap& otf_map, float2*, const float2* otf, int conj_otf, int pairs, int W,
-                            const float2* tw, dim3 grid, cudaStream_t st) {
-        return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, grid, dim3(NTC), kColSmem, st, tmap, otf_map, otf, conj_otf, pairs, W, tw);
-    }
-    static cudaError_t prepare_cols() {
-        return cudaFuncSetAttribute(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
-    }
-    static SizeOps make() {
-        SizeOps o;
-        o.N = PC::N;
-        o.row = PlanInfo{0, 0, 0, {0, 0, 0, 0, 0}};
-        o.col = PlanInfo{PC::E, PC::TPF, PC::S, {PC::radix(0), PC::radix(1), PC::radix(2), PC::radix(3), PC::radix(4)}};
-        o.row_threads = 0; o.row_smem = 0;
-        o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = kBoxH; o.col_box_w = 2 * CPT;
-        o.rows = nullptr; o.cols = &cols; o.prepare_rows = nullptr; o.prepare_cols = &prepare_cols;
-        o.generation = 2; o.row_cps = 0; o.col_cps = MINB; o.col_otf_regs = OTF_REGS ? 1 : 0;
-        return o;
-    }
-};
-
-// A length served by the lean column kernel (columns only when P has no row kernel here).
-template <class PC, int NTC, int MINB, int CPT>
-struct ColsLean2 {
-    static constexpr int kTeam = CPT * PC::TPF, kNTeam = NTC / kTeam, kTC = CPT * kNTeam;
-    static constexpr int kBoxH = PC::N <= 256 ? PC::N : (PC::N % 256 == 0 ? 256 : 200);
-    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)kNTeam * PC::N * CPT) +
-                                       sizeof(uint64_t) * kNTeam;
-    static cudaError_t cols(const CUtensorMap& tmap, const CUtensorMap&, float2* S, const float2* otf, int conj_otf, int pairs, int W,
-                            const float2* tw, dim3 grid, cudaStream_t st) {
-        return launch_pdl(fft2_cols_lean_kernel<PC, NTC, MINB, CPT>, grid, dim3(NTC), kColSmem, st, tmap, S, otf, conj_otf, pairs, W, tw);
-    }
-    static cudaError_t prepare_cols() {
-        return cudaFuncSetAttribute(fft2_cols_lean_kernel<PC, NTC, MINB, CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
-    }
-    // `base`: the descriptor whose row kernels this length keeps (nullptr: columns only)
-    static SizeOps make(const SizeOps* base = nullptr) {
-        SizeOps o;
-        if (base) o = *base;
-        o.N = PC::N;
-        if (!base) {
-            o.row = PlanInfo{0, 0, 0, {0, 0, 0, 0, 0}};
-            o.row_threads = 0; o.row_smem = 0; o.rows = nullptr; o.prepare_rows = nullptr; o.row_cps = 0;
-        }
-        o.col = PlanInfo{PC::E, PC::TPF, PC::S, {PC::radix(0), PC::radix(1), PC::radix(2), PC::radix(3), PC::radix(4)}};
-        o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = kBoxH; o.col_box_w = 2 * CPT;
-        o.cols = &cols; o.prepare_cols = &prepare_cols;
-        o.generation = 2; o.col_cps = MINB; o.col_otf_regs = 0;
         return o;
     }
 };
