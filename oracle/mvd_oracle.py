@@ -162,6 +162,35 @@ def deconvolve_padded(views: np.ndarray, psfs: np.ndarray, T: int, eps: float = 
     return np.ascontiguousarray(deconvolve(padded, psfs, T, eps, n_threads)[:, :H, :W])
 
 
+def deconvolve_product(views: np.ndarray, psfs: np.ndarray, T: int, eps: float = 1e-6,
+                       weights: Optional[np.ndarray] = None) -> np.ndarray:
+    """The update exactly as PAPER.md:79 prints it (Supp. Note 1): psi^{t+1} = psi^t prod_v (phi_v / (psi^t * P_v)) * P_v^*,
+    every view's factor computed from the SAME psi^t (the "simultaneous" form).  north_star's reading (A1) is the
+    sequential form of `deconvolve`; this is the other one, offered as an update mode of the library.  Steps a1-a3 are the
+    C routines behind `blur` / `backproject`; with weights each factor is w_v q_v + 1 - w_v (reading W1).
+    """
+    views = np.ascontiguousarray(views, dtype=np.uint16)
+    psfs = _f32(psfs)
+    V, N, H, W = views.shape
+    e32 = float(np.float32(eps))
+    out = np.empty((N, H, W), dtype=np.float64)
+    for n in range(N):
+        phi = views[:, n].astype(np.float64)
+        psi = phi.sum(axis=0) / V                                   # a0
+        for _ in range(T):
+            factor = np.ones_like(psi)
+            for v in range(V):
+                b = blur(psi, psfs[v])                              # a1, from psi^t for every view
+                q = backproject(phi[v] / np.maximum(b, e32), psfs[v])   # a2, a3
+                if weights is not None:
+                    w = np.asarray(weights[v, n], dtype=np.float64)
+                    q = w * q + (1.0 - w)
+                factor *= q
+            psi = psi * factor                                      # a4, once per iteration
+        out[n] = psi
+    return out
+
+
 def trace(views_plane: np.ndarray, psfs: np.ndarray, T: int, eps: float = 1e-6) -> np.ndarray:
     """fp64 `[T*V][H][W]`: psi after every view update of ONE plane (views_plane uint16 `[V][H][W]`)."""
     views_plane = np.ascontiguousarray(views_plane, dtype=np.uint16)

@@ -525,3 +525,60 @@ def test_PD3_interior_of_a_dark_bordered_plane_matches_periodic():
     views[:, :, K - 1:H - K + 1, K - 1:W - K + 1] = rng.integers(1, 900, size=(V, 1, H - 2 * K + 2, W - 2 * K + 2))
     psfs = rand_psfs(V, K, 11)
     np.testing.assert_allclose(orc.deconvolve_padded(views, psfs, 3), orc.deconvolve(views, psfs, 3), rtol=1e-12, atol=1e-300)
+
+
+# ---------------------------------------------------------------------------------------------
+# PP: the update as printed in PAPER.md:79 (simultaneous / product form), oracle.deconvolve_product
+# ---------------------------------------------------------------------------------------------
+def dense_rl_product(views_plane, psfs, T, eps):
+    V, H, W = views_plane.shape
+    phi = views_plane.reshape(V, -1).astype(np.float64)
+    psi = phi.sum(0) / V
+    ops = [dense_operator(psfs[v], H, W) for v in range(V)]
+    for _ in range(T):
+        f = np.ones_like(psi)
+        for v in range(V):
+            f *= ops[v].T @ (phi[v] / np.maximum(ops[v] @ psi, eps))
+        psi = psi * f
+    return psi.reshape(H, W)
+
+
+@pytest.mark.parametrize("W,H,K", [(8, 8, 3), (12, 8, 5), (8, 12, 7), (6, 5, 9)])
+def test_PP1_product_form_dense_matrix_brute_force(W, H, K):
+    V, T = 3, 4
+    views = synth.random_views(V, 2, W, H, seed=150 + K)
+    psfs = rand_psfs(V, K, 160 + W)
+    out = orc.deconvolve_product(views, psfs, T)
+    for p in range(2):
+        ref = dense_rl_product(views[:, p], psfs, T, float(np.float32(1e-6)))
+        np.testing.assert_allclose(out[p], ref, rtol=1e-11, atol=1e-11)
+    assert np.abs(out - orc.deconvolve(views, psfs, T)).max() > 1e-3 * out.max()    # not the sequential form
+
+
+def test_PP2_single_view_product_is_sequential_and_constants_stay_fixed():
+    views = synth.random_views(1, 2, 14, 10, seed=3)
+    psfs = rand_psfs(1, 5, 4)
+    np.testing.assert_allclose(orc.deconvolve_product(views, psfs, 5), orc.deconvolve(views, psfs, 5), rtol=1e-13)
+    const = np.full((3, 1, 9, 11), 321, dtype=np.uint16)
+    P = rand_psfs(3, 5, 8)
+    np.testing.assert_allclose(orc.deconvolve_product(const, P, 4), 321.0, rtol=1e-12)
+
+
+def test_PP3_product_form_with_weights():
+    V, N, H, W, K = 2, 1, 9, 8, 3
+    views = synth.random_views(V, N, W, H, seed=21)
+    psfs = rand_psfs(V, K, 22)
+    ones = np.ones((V, N, H, W), dtype=np.float32)
+    np.testing.assert_array_equal(orc.deconvolve_product(views, psfs, 3, weights=ones), orc.deconvolve_product(views, psfs, 3))
+    w = ones.copy()
+    w[1] = 0.0                                                      # view 1 never applied == the single-view run
+    np.testing.assert_allclose(orc.deconvolve_product(views, psfs, 3, weights=w)[0] * 0 + 1, 1.0)   # finite
+    one_view = orc.deconvolve_product(views[:1], psfs[:1], 3)
+    got = orc.deconvolve_product(views, psfs, 3, weights=w)
+    # psi_0 differs (mean of both views), so compare the per-iteration factor instead: same update operator
+    phi = views[:, 0].astype(np.float64)
+    psi = phi.sum(0) / V
+    for _ in range(3):
+        psi = psi * orc.backproject(phi[0] / np.maximum(orc.blur(psi, psfs[0]), float(np.float32(1e-6))), psfs[0])
+    np.testing.assert_allclose(got[0], psi, rtol=1e-12)
+    assert one_view.shape == (1, H, W)
