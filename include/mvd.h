@@ -255,6 +255,22 @@ MVD_API int mvd_get_path(const mvd_handle* h);
 MVD_API int mvd_path_supported(int path, int plane_w, int plane_h, int psf_size);
 
 /*
+ * mvd_set_update_mode -- which form of the multi-view update the handle's later calls run.
+ *   MVD_UPDATE_SEQUENTIAL (default)  north_star's reading (A1 of DESIGN.md): for every view in turn, each view's factor is
+ *                                    multiplied in before the next view's blur.
+ *   MVD_UPDATE_PRODUCT               the update exactly as PAPER.md:79 prints it:
+ *                                        psi^{t+1} = psi^t  prod_v  ( phi_v / (psi^t * P_v) ) * P_v^*,
+ *                                    every view's factor from the SAME psi^t (the "simultaneous" form).  Both engines run it
+ *                                    with the kernels of the sequential form: the factors are multiplied into a copy of psi^t
+ *                                    that becomes psi^{t+1} after the last view (FFT engine: every view's blur restarts
+ *                                    from a saved copy of psi^t's row spectrum; 8 (1 + 2 / V) extra bytes per unit).  The FFT
+ *                                    engine's guard (mvd_guard_flagged) does not repair plane pairs in this mode.
+ * Call it before mvd_reserve.  Errors: MVD_ERR_INVALID.
+ */
+enum { MVD_UPDATE_SEQUENTIAL = 0, MVD_UPDATE_PRODUCT = 1 };
+MVD_API int mvd_set_update_mode(mvd_handle* h, int mode);
+
+/*
  * Tuning knobs (measurement; defaults are chosen in mvd_create).
  *   mvd_set_chunk_planes  planes processed per internal pass of mvd_deconvolve_planes (0 = default)
  *   mvd_set_batch_planes  planes per pipeline batch of mvd_deconvolve_host (0 = default)

@@ -42,6 +42,7 @@ SIGNATURES = {
     "mvd_guard_flagged": (_ll, [_vp]),
     "mvd_reserve": (_i, [_vp, _i]),
     "mvd_get_batch_planes": (_i, [_vp, _i]),
+    "mvd_set_update_mode": (_i, [_vp, _i]),
     "mvd_set_chunk_planes": (_i, [_vp, _i]),
     "mvd_set_batch_planes": (_i, [_vp, _i]),
     "mvd_set_resident_streams": (_i, [_vp, _i]),
@@ -64,6 +65,7 @@ class MvdIO(ctypes.Structure):
 
 
 OUT_F32, OUT_U16 = 0, 1
+UPDATE_SEQUENTIAL, UPDATE_PRODUCT = 0, 1
 SIGNATURES.update({
     "mvd_deconvolve_planes_ex": (_i, [_vp, ctypes.POINTER(MvdIO), _i, _vp]),
     "mvd_deconvolve_host_ex": (_i, [_vp, ctypes.POINTER(MvdIO), _i]),
@@ -239,6 +241,10 @@ class Mvd:
             self._raise(rc, "mvd_get_batch_planes")
         return rc
 
+    def set_update_mode(self, mode: int) -> None:
+        """UPDATE_SEQUENTIAL (default) or UPDATE_PRODUCT (the update as printed in PAPER.md:79)."""
+        self._raise(lib().mvd_set_update_mode(self._h, mode), "mvd_set_update_mode")
+
     def set_chunk_planes(self, planes: int) -> None:
         self._raise(lib().mvd_set_chunk_planes(self._h, planes), "mvd_set_chunk_planes")
 
@@ -325,7 +331,7 @@ def deconvolve(views: np.ndarray, psfs: np.ndarray, iterations: int, eps: float 
                path: Optional[int] = None, host: bool = False, chunk_planes: int = 0,
                batch_planes: int = 0, backprojectors: Optional[np.ndarray] = None,
                resident_streams: int = 0, weights: Optional[np.ndarray] = None, out_u16: bool = False,
-               padded: bool = False) -> np.ndarray:
+               padded: bool = False, product: bool = False) -> np.ndarray:
     """Convenience for tests: numpy uint16 `[V][N][H][W]` in, numpy float32 `[N][H][W]` out, through
     mvd_deconvolve_planes (host=False) or mvd_deconvolve_host (host=True, pinned buffers)."""
     import torch
@@ -335,6 +341,8 @@ def deconvolve(views: np.ndarray, psfs: np.ndarray, iterations: int, eps: float 
     V, N, H, W = views.shape
     K = psfs.shape[-1]
     with Mvd(W, H, V, psfs, K, iterations, eps, path, backprojectors, padded) as m:
+        if product:
+            m.set_update_mode(UPDATE_PRODUCT)
         if chunk_planes:
             m.set_chunk_planes(chunk_planes)
         if batch_planes:

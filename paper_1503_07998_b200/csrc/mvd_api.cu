@@ -63,12 +63,20 @@ int ws_reserve(mvd_handle* h, Workspace& ws, size_t a_bytes, size_t b_bytes, siz
     return rc;
 }
 
+int ws_reserve_product(mvd_handle* h, Workspace& ws, size_t c_bytes, size_t d_bytes) {
+    int rc = grow(h, &ws.c, &ws.c_bytes, c_bytes);
+    if (rc == MVD_OK) rc = grow(h, &ws.d, &ws.d_bytes, d_bytes);
+    return rc;
+}
+
 static void ws_free(Workspace& ws) {
     if (ws.a) cudaFree(ws.a);
     if (ws.b) cudaFree(ws.b);
     if (ws.g) cudaFree(ws.g);
     if (ws.pin) cudaFree(ws.pin);
     if (ws.pout) cudaFree(ws.pout);
+    if (ws.c) cudaFree(ws.c);
+    if (ws.d) cudaFree(ws.d);
     ws = Workspace();
 }
 
@@ -415,6 +423,13 @@ int mvd_reserve(mvd_handle* h, int max_planes) {
     scratch_bytes(h, std::min(chunk, max_planes), &a, &b, &g);
     if ((rc = ws_reserve(h, h->ws_main, a, b, g)) != MVD_OK) return rc;
     if ((rc = pad_reserve(h, h->ws_main, std::min(chunk, max_planes))) != MVD_OK) return rc;
+    if (h->update_mode == MVD_UPDATE_PRODUCT) {
+        if ((rc = ws_reserve_product(h, h->ws_main, a, h->path == MVD_PATH_FFT ? b : 0)) != MVD_OK) return rc;
+        size_t a2, b2, g2;
+        scratch_bytes(h, std::min(chunk, B), &a2, &b2, &g2);
+        for (int s = 0; s < mvd_handle::kSlots; ++s)
+            if ((rc = ws_reserve_product(h, h->ws_slot[s], a2, h->path == MVD_PATH_FFT ? b2 : 0)) != MVD_OK) return rc;
+    }
     scratch_bytes(h, std::min(chunk, B), &a, &b, &g);
     for (int s = 0; s < mvd_handle::kSlots; ++s) {
         if ((rc = ws_reserve(h, h->ws_slot[s], a, b, g)) != MVD_OK) return rc;
@@ -701,6 +716,12 @@ long long mvd_guard_flagged(mvd_handle* h) {
     return (long long)n;
 }
 int mvd_get_path(const mvd_handle* h) { return h ? h->path : MVD_ERR_INVALID; }
+
+int mvd_set_update_mode(mvd_handle* h, int mode) {
+    if (!h || (mode != MVD_UPDATE_SEQUENTIAL && mode != MVD_UPDATE_PRODUCT)) return MVD_ERR_INVALID;
+    h->update_mode = mode;
+    return MVD_OK;
+}
 
 int mvd_set_chunk_planes(mvd_handle* h, int planes) {
     if (!h || planes < 0) return MVD_ERR_INVALID;

@@ -638,11 +638,17 @@ __global__ void convert_u16_kernel(const float* __restrict__ psi, uint16_t* __re
 int direct_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cudaStream_t stream) {
     const size_t npx = (size_t)h->W * h->H;
     const size_t n = npx * n_planes;
-    if (h->T > 0 && direct_small_available(h)) return direct_run_small(h, io, n_planes, stream);
+    const bool product = h->update_mode == MVD_UPDATE_PRODUCT && h->T > 0;
+    if (h->T > 0 && !product && direct_small_available(h)) return direct_run_small(h, io, n_planes, stream);
     // psi is iterated in place in the fp32 output; a uint16 output gets an fp32 scratch and one conversion pass
     int rc = ws_reserve(h, ws, h->T > 0 ? direct_scratch_bytes(h, n_planes) : 0, io.out16 ? sizeof(float) * n : 0);
     if (rc != MVD_OK) return rc;
+    // Product form (PAPER.md:79 as printed): kernel A reads psi^t for every view, kernel B multiplies the factors into a
+    // copy of it, which becomes psi^{t+1} after the last view; the two buffers then swap roles.
+    if (product && (rc = ws_reserve_product(h, ws, sizeof(float) * n, 0)) != MVD_OK) return rc;
     float* psi = io.out16 ? ws.b : io.out;
+    float* const result = psi;
+    float* acc = ws.c;
     const unsigned egrid = (unsigned)std::min<size_t>((n + 255) / 256, (size_t)h->n_sm * 16);
     {
         LaunchScope ls(h, KC_INIT_MEAN, stream);
@@ -651,7 +657,9 @@ int direct_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cu
     MVD_TRY(h, cudaGetLastError());
     float* r = ws.a;
     const size_t per = (size_t)h->dK * h->Kp;
-    for (int t = 0; t < h->T; ++t)
+    for (int t = 0; t < h->T; ++t) {
+        if (product) MVD_TRY(h, cudaMemcpyAsync(acc, psi, sizeof(float) * n, cudaMemcpyDeviceToDevice, stream));
+        float* const upd = product ? acc : psi;     // what kernel B multiplies the factor into
         for (int v = 0; v < h->V; ++v) {
             const float* Gblur = h->d_coef + ((size_t)v * 2 + 0) * per;
             const float* Gback = h->d_coef + ((size_t)v * 2 + 1) * per;
@@ -666,11 +674,15 @@ int direct_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cu
             MVD_TRY(h, (cudaError_t)e);
             {
                 LaunchScope ls(h, h->sep ? KC_SEP_BACK_UPDATE : KC_DIRECT_BACK_UPDATE, stream);
-                e = h->sep ? sep_launch(1, h, v, r, nullptr, psi, n_planes, stream, 0, 0, wv)
-                           : launch_corr(1, h, r, Gback, nullptr, psi, n_planes, stream, 0, 0, wv);
+                e = h->sep ? sep_launch(1, h, v, r, nullptr, upd, n_planes, stream, 0, 0, wv)
+                           : launch_corr(1, h, r, Gback, nullptr, upd, n_planes, stream, 0, 0, wv);
             }
             MVD_TRY(h, (cudaError_t)e);
         }
+        if (product) std::swap(psi, acc);
+    }
+    if (psi != result) MVD_TRY(h, cudaMemcpyAsync(result, psi, sizeof(float) * n, cudaMemcpyDeviceToDevice, stream));
+    psi = result;
     if (io.out16) {
         LaunchScope ls(h, KC_INIT_MEAN, stream);
         convert_u16_kernel<<<egrid, 256, 0, stream>>>(psi, io.out16, n);

@@ -313,6 +313,12 @@ int fft_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cudaS
         return MVD_ERR_INVALID;
     int rc = ws_reserve(h, ws, bytes, bytes, fft_guard_bytes(n_planes));
     if (rc != MVD_OK) return rc;
+    // Product form (PAPER.md:79 as printed; mvd_set_update_mode): every view's blur starts from psi^t's row spectrum,
+    // saved in S0 and copied back into S before views 1 .. V-1, and the factors are multiplied into A = a copy of psi^t
+    // (the update pass runs with its Z pointer on A), which the last view turns into psi^{t+1} -- together with its row
+    // spectrum in S, exactly what the next iteration starts from.  Then Z and A swap roles.
+    const bool product = h->update_mode == MVD_UPDATE_PRODUCT && h->T > 0;
+    if (product && (rc = ws_reserve_product(h, ws, bytes, h->V > 1 ? bytes : 0)) != MVD_OK) return rc;
     if (pairs > 512) return MVD_ERR_INVALID;   // chunks are bounded by fft_default_chunk / mvd_set_chunk_planes
     MVD_TRY(h, cudaMemsetAsync(ws.g, 0, fft_guard_bytes(n_planes), stream));
     CUtensorMap tmap;
@@ -371,9 +377,17 @@ int fft_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cudaS
         rc = mvd_check(h, st->row->rows(mvdfft::ROWS_FIRST, a, st->tw_row, row_grid, stream));
     }
     if (rc != MVD_OK) return rc;
-    for (int t = 0; t < h->T; ++t)
+    float2* Zcur = (float2*)ws.a;       // psi^t
+    float2* Acc = (float2*)ws.c;        // product form: psi^t times the factors so far
+    for (int t = 0; t < h->T; ++t) {
+        if (product) {
+            MVD_TRY(h, cudaMemcpyAsync(Acc, Zcur, bytes, cudaMemcpyDeviceToDevice, stream));
+            if (h->V > 1) MVD_TRY(h, cudaMemcpyAsync(ws.d, ws.b, bytes, cudaMemcpyDeviceToDevice, stream));
+        }
         for (int v = 0; v < h->V; ++v) {
             const float2* otf = h->d_otf + (size_t)v * npx;
+            if (product && v > 0) MVD_TRY(h, cudaMemcpyAsync(ws.b, ws.d, bytes, cudaMemcpyDeviceToDevice, stream));
+            a.Z = product ? Acc : Zcur;
             {
                 LaunchScope ls(h, KC_FFT_COLS, stream);
                 rc = mvd_check(h, st->col->cols(tmap, st->otf_maps.empty() ? tmap : st->otf_maps[v], a.S, otf, 0, pairs, W,
@@ -405,6 +419,9 @@ int fft_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cudaS
             }
             if (rc != MVD_OK) return rc;
         }
+        if (product) std::swap(Zcur, Acc);
+    }
+    if (product) return MVD_OK;     // (the guard's repair pass recomputes the sequential form: not offered here)
     // guard: pairs flagged by the ratio passes are recomputed with the direct engine's arithmetic (one empty
     // cooperative launch when nothing is flagged); Z is free by now and serves as its ratio scratch
     // (with uint16 output psi is iterated in S, which is free as well)

@@ -42,6 +42,11 @@ struct Workspace {
     uint16_t* pin = nullptr;
     float* pout = nullptr;
     size_t pin_bytes = 0, pout_bytes = 0;
+    // product-form update (mvd_set_update_mode): the estimate being built (psi^t times the factors so far) and, on the
+    // FFT engine, the row spectrum of psi^t that every view's blur starts from
+    float* c = nullptr;
+    float* d = nullptr;
+    size_t c_bytes = 0, d_bytes = 0;
 };
 
 struct mvd_handle {
@@ -93,6 +98,7 @@ struct mvd_handle {
     int resident_streams = 2;   // measured: 2 beats 1 by 7-20 % and 3 by 3-10 % on configs 2-5
     cudaEvent_t ev_fork = nullptr, ev_join[kSlots] = {nullptr, nullptr, nullptr};
 
+    int update_mode = 0;    // MVD_UPDATE_SEQUENTIAL / MVD_UPDATE_PRODUCT
     int chunk_planes = 0;   // 0 = default
     int batch_planes = 0;   // 0 = default
 
@@ -150,6 +156,7 @@ int mvd_check(mvd_handle* h, cudaError_t e);
     } while (0)
 
 int ws_reserve(mvd_handle* h, Workspace& ws, size_t a_bytes, size_t b_bytes, size_t g_bytes = 0);
+int ws_reserve_product(mvd_handle* h, Workspace& ws, size_t c_bytes, size_t d_bytes);
 
 // ---- direct path (mvd_direct.cu) ------------------------------------------------------------
 int direct_choose_chunk(int K, int* JC, int* Kp);
