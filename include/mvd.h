@@ -50,7 +50,8 @@ enum {
     MVD_ERR_UNSUPPORTED = -2, /* a forced path cannot handle this shape (e.g. FFT on a non-smooth size)  */
     MVD_ERR_CUDA = -3,        /* a CUDA call failed; mvd_last_cuda_error() has the cudaError_t           */
     MVD_ERR_NOMEM = -4,       /* device or pinned-staging allocation failed                              */
-    MVD_ERR_BUSY = -5         /* reserved                                                                */
+    MVD_ERR_BUSY = -5,        /* reserved                                                                */
+    MVD_ERR_IO = -6           /* mvd_deconvolve_files: a file could not be opened, is too short, or a read / write failed */
 };
 
 /* Convolution engine used for steps a1 and a3 (both engines fuse a2 and a4 into their kernels). */
@@ -213,6 +214,19 @@ MVD_API int mvd_deconvolve_host_weighted(mvd_handle* h, const uint16_t* host_vie
 MVD_API int mvd_deconvolve_planes_u16(mvd_handle* h, const uint16_t* dev_views_u16, uint16_t* dev_out_u16,
                                       int n_planes, void* stream);
 MVD_API int mvd_deconvolve_host_u16(mvd_handle* h, const uint16_t* host_views_u16, uint16_t* host_out_u16, int n_planes);
+
+/*
+ * mvd_deconvolve_files -- the paper's whole workflow (Algorithm 1): loading from and saving to disk
+ * overlap the GPU pipeline.  view_paths[v] names a raw little-endian uint16 file holding view v as
+ * [n_planes][plane_h][plane_w] (the first n_planes planes of a longer file are used); out_path is created / truncated
+ * and receives [n_planes][plane_h][plane_w] as float (MVD_OUT_F32) or uint16 (MVD_OUT_U16).  Slabs of planes (a whole
+ * number of pipeline batches, ~256 MiB of input) cycle through three pinned buffer sets: a reader thread loads slab
+ * k + 1 and a writer thread saves slab k - 1 while slab k runs through mvd_deconvolve_host_ex.  Blocks until the output
+ * file is complete; the bytes written are those mvd_deconvolve_host produces.  Errors: MVD_ERR_INVALID, MVD_ERR_IO,
+ * MVD_ERR_NOMEM (pinned buffers), and everything mvd_deconvolve_host returns.
+ */
+MVD_API int mvd_deconvolve_files(mvd_handle* h, const char* const* view_paths, const char* out_path, int n_planes,
+                                 int out_type);
 
 /*
  * mvd_reserve -- size everything a later call on up to max_planes planes needs (scratch of the engine, the

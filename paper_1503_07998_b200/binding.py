@@ -15,7 +15,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmvd.so")
 
-MVD_OK, MVD_ERR_INVALID, MVD_ERR_UNSUPPORTED, MVD_ERR_CUDA, MVD_ERR_NOMEM, MVD_ERR_BUSY = 0, -1, -2, -3, -4, -5
+MVD_OK, MVD_ERR_INVALID, MVD_ERR_UNSUPPORTED, MVD_ERR_CUDA, MVD_ERR_NOMEM, MVD_ERR_BUSY, MVD_ERR_IO = 0, -1, -2, -3, -4, -5, -6
 PATH_AUTO, PATH_DIRECT, PATH_FFT = 0, 1, 2
 N_KERNEL_CLASSES = 12
 PATH_NAMES = {PATH_AUTO: "auto", PATH_DIRECT: "direct", PATH_FFT: "fft"}
@@ -73,6 +73,7 @@ SIGNATURES.update({
     "mvd_deconvolve_host_weighted": (_i, [_vp, _vp, _vp, _vp, _i]),
     "mvd_deconvolve_planes_u16": (_i, [_vp, _vp, _vp, _i, _vp]),
     "mvd_deconvolve_host_u16": (_i, [_vp, _vp, _vp, _i]),
+    "mvd_deconvolve_files": (_i, [_vp, ctypes.POINTER(ctypes.c_char_p), ctypes.c_char_p, _i, _i]),
 })
 
 _lib: Optional[ctypes.CDLL] = None
@@ -207,6 +208,14 @@ class Mvd:
     def deconvolve_host_u16(self, host_views_u16, host_out_u16, n_planes: int) -> None:
         self._raise(lib().mvd_deconvolve_host_u16(self._h, _ptr(host_views_u16), _ptr(host_out_u16), n_planes),
                     "mvd_deconvolve_host_u16")
+
+    def deconvolve_files(self, view_paths, out_path: str, n_planes: int, out_u16: bool = False) -> None:
+        """mvd_deconvolve_files: raw uint16 view files in, raw float / uint16 file out, disk I/O overlapped.  Blocks."""
+        if len(view_paths) != self.n_views:
+            raise ValueError("one file per view")
+        arr = (ctypes.c_char_p * len(view_paths))(*[os.fsencode(p) for p in view_paths])
+        self._raise(lib().mvd_deconvolve_files(self._h, arr, os.fsencode(out_path), n_planes,
+                                               OUT_U16 if out_u16 else OUT_F32), "mvd_deconvolve_files")
 
     def deconvolve_host(self, host_views_u16, host_out_f32, n_planes: int) -> None:
         """host buffers: pinned torch tensors, numpy arrays or raw host pointers.  Blocks."""

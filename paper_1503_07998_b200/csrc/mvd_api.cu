@@ -701,6 +701,7 @@ const char* mvd_strerror(int code) {
         case MVD_ERR_CUDA: return "CUDA error (see mvd_last_cuda_error)";
         case MVD_ERR_NOMEM: return "out of device or pinned memory";
         case MVD_ERR_BUSY: return "handle busy";
+        case MVD_ERR_IO: return "file could not be opened, is too short, or a read / write failed";
         default: return "unknown mvd error code";
     }
 }
