@@ -537,8 +537,8 @@ static int default_batch(const mvd_handle* h, int n_planes, int min_batches) {
     // ~64 MiB of uint16 input per batch
     const size_t per_plane = (size_t)h->uW * h->uH * sizeof(uint16_t) * h->V;
     size_t b = std::max<size_t>(1, ((size_t)64 << 20) / per_plane);
-    if (min_batches < 16 && h->path == MVD_PATH_FFT) {
-        // Device-resident stacks on the FFT engine: two batches are in flight, each cycling its Z and S (8 B per
+    if (h->path == MVD_PATH_FFT) {
+        // FFT engine (device-resident stacks and the host pipeline alike): two batches are in flight, each cycling its Z and S (8 B per
         // plane-pixel together) through all T x V passes.  When two such working sets fit the 126 MB L2 with at
         // least five planes per batch the passes run largely from L2 (measured: configs 2 / 3 / 5 best
         // at 64 / 8-16 / 4-6 planes); when they cannot (config 4: 13 MB per plane), long launches win instead
