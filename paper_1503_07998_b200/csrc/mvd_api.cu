@@ -44,6 +44,7 @@ LaunchScope::~LaunchScope() {
 
 static int grow(mvd_handle* h, float** p, size_t* have, size_t want) {
     if (want <= *have) return MVD_OK;
+    if (h) h->graph_epoch++;      // captured launch sequences hold the old pointer
     if (*p) {
         // the buffer may still be in use by work enqueued earlier on this handle's stream
         MVD_TRY(h, cudaDeviceSynchronize());
@@ -78,6 +79,76 @@ static void ws_free(Workspace& ws) {
     if (ws.c) cudaFree(ws.c);
     if (ws.d) cudaFree(ws.d);
     ws = Workspace();
+}
+
+// Replay `body`'s launch sequence as a CUDA graph: captured the first time a key is seen (stream capture on `st`;
+// everything body enqueues, including work forked to the internal streams, becomes one graph), launched with one call
+// afterwards.  Falls back to running body directly when the stream is already being captured by the caller, while
+// profiling, or when capture fails.  body must only enqueue (everything it needs is reserved beforehand).
+template <class F>
+static int run_graphed(mvd_handle* h, const uint64_t (&key)[8], cudaStream_t st, F&& body) {
+    if (!h->use_graphs || h->profiling) return body();
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone) {
+        (void)cudaGetLastError();
+        return body();
+    }
+    for (size_t i = 0; i < h->graphs.size();) {       // drop what an epoch change invalidated
+        if (h->graphs[i].epoch != h->graph_epoch) {
+            cudaGraphExecDestroy(h->graphs[i].exec);
+            h->graphs[i] = h->graphs.back();
+            h->graphs.pop_back();
+        } else {
+            ++i;
+        }
+    }
+    for (auto& e : h->graphs)
+        if (!memcmp(e.key, key, sizeof key)) {
+            e.last_use = ++h->graph_clock;
+            h->launches += e.launches;
+            return mvd_check(h, cudaGraphLaunch(e.exec, st));
+        }
+    const uint64_t epoch0 = h->graph_epoch;
+    const long long launches0 = h->launches;
+    if (cudaStreamBeginCapture(st, cudaStreamCaptureModeRelaxed) != cudaSuccess) {
+        (void)cudaGetLastError();
+        return body();
+    }
+    const int rc = body();
+    cudaGraph_t g = nullptr;
+    const cudaError_t ee = cudaStreamEndCapture(st, &g);
+    cudaGraphExec_t exec = nullptr;
+    if (h->graph_epoch != epoch0 && rc == MVD_OK && ee == cudaSuccess) {
+        // body had to allocate (first use of some scratch): nothing ran, the pointers are new -- run it plainly now,
+        // the next call captures
+        if (g) cudaGraphDestroy(g);
+        h->launches = launches0;
+        return body();
+    }
+    if (rc != MVD_OK || ee != cudaSuccess || !g || cudaGraphInstantiate(&exec, g, 0) != cudaSuccess) {
+        if (g) cudaGraphDestroy(g);
+        (void)cudaGetLastError();
+        h->launches = launches0;
+        h->use_graphs = false;        // this plan's sequence cannot be captured: plain launches from now on
+        return body();
+    }
+    cudaGraphDestroy(g);
+    if (h->graphs.size() >= 16) {     // bounded: evict the least recently used
+        size_t lru = 0;
+        for (size_t i = 1; i < h->graphs.size(); ++i)
+            if (h->graphs[i].last_use < h->graphs[lru].last_use) lru = i;
+        cudaGraphExecDestroy(h->graphs[lru].exec);
+        h->graphs[lru] = h->graphs.back();
+        h->graphs.pop_back();
+    }
+    GraphEntry e;
+    memcpy(e.key, key, sizeof key);
+    e.epoch = epoch0;
+    e.exec = exec;
+    e.launches = h->launches - launches0;
+    e.last_use = ++h->graph_clock;
+    h->graphs.push_back(e);
+    return mvd_check(h, cudaGraphLaunch(exec, st));
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -265,6 +336,7 @@ void mvd_destroy(mvd_handle* h) {
     cudaDeviceSynchronize();
     for (auto& r : h->prof) { cudaEventDestroy(r.e0); cudaEventDestroy(r.e1); }
     for (auto& e : h->event_pool) cudaEventDestroy(e);
+    for (auto& g : h->graphs) cudaGraphExecDestroy(g.exec);
     ws_free(h->ws_main);
     for (int s = 0; s < mvd_handle::kSlots; ++s) {
         ws_free(h->ws_slot[s]);
@@ -275,6 +347,7 @@ void mvd_destroy(mvd_handle* h) {
         if (h->ev_join[s]) cudaEventDestroy(h->ev_join[s]);
     }
     if (h->ev_fork) cudaEventDestroy(h->ev_fork);
+    if (h->ev_last) cudaEventDestroy(h->ev_last);
     if (h->d_coef) cudaFree(h->d_coef);
     if (h->d_sep) cudaFree(h->d_sep);
     if (h->d_guard_total) cudaFree(h->d_guard_total);
@@ -308,13 +381,15 @@ static int pad_reserve(mvd_handle* h, Workspace& ws, int n) {
     const size_t npx = (size_t)h->W * h->H;
     const size_t in_b = sizeof(uint16_t) * npx * n * h->V, out_b = sizeof(float) * npx * n;
     if (in_b > ws.pin_bytes) {
-        if (ws.pin) { MVD_TRY(h, cudaDeviceSynchronize()); MVD_TRY(h, cudaFree(ws.pin)); ws.pin = nullptr; ws.pin_bytes = 0; }
+        if (ws.pin) { MVD_TRY(h, cudaDeviceSynchronize()); MVD_TRY(h, cudaFree(ws.pin)); ws.pin = nullptr; ws.pin_bytes = 0; h->graph_epoch++; }
+        h->graph_epoch++;
         MVD_TRY(h, cudaMalloc((void**)&ws.pin, in_b));
         ws.pin_bytes = in_b;
     }
     // the layout [V][n][H][W] depends on n: the corners move, so the whole buffer is cleared for every new n
     if (out_b > ws.pout_bytes) {
-        if (ws.pout) { MVD_TRY(h, cudaDeviceSynchronize()); MVD_TRY(h, cudaFree(ws.pout)); ws.pout = nullptr; ws.pout_bytes = 0; }
+        if (ws.pout) { MVD_TRY(h, cudaDeviceSynchronize()); MVD_TRY(h, cudaFree(ws.pout)); ws.pout = nullptr; ws.pout_bytes = 0; h->graph_epoch++; }
+        h->graph_epoch++;
         MVD_TRY(h, cudaMalloc((void**)&ws.pout, out_b));
         ws.pout_bytes = out_b;
     }
@@ -377,6 +452,7 @@ static int default_batch(const mvd_handle* h, int n_planes, int min_batches = 16
 // Streams and events of the host pipeline / the forked device-resident batches, created once.
 static int ensure_streams(mvd_handle* h) {
     if (!h->ev_fork) MVD_TRY(h, cudaEventCreateWithFlags(&h->ev_fork, cudaEventDisableTiming));
+    if (!h->ev_last) MVD_TRY(h, cudaEventCreateWithFlags(&h->ev_last, cudaEventDisableTiming));
     for (int s = 0; s < mvd_handle::kSlots; ++s) {
         if (!h->streams[s]) MVD_TRY(h, cudaStreamCreateWithFlags(&h->streams[s], cudaStreamNonBlocking));
         if (!h->ev_join[s]) MVD_TRY(h, cudaEventCreateWithFlags(&h->ev_join[s], cudaEventDisableTiming));
@@ -406,6 +482,7 @@ static int reserve_slots(mvd_handle* h, int B) {
         if (h->d_out[s]) { cudaFree(h->d_out[s]); h->d_out[s] = nullptr; }
     }
     h->slot_planes = 0;
+    h->graph_epoch++;
     for (int s = 0; s < mvd_handle::kSlots; ++s) {
         MVD_TRY(h, cudaMalloc((void**)&h->d_in[s], sizeof(uint16_t) * npx * B * h->V));
         MVD_TRY(h, cudaMalloc((void**)&h->d_out[s], sizeof(float) * npx * B));
@@ -493,13 +570,61 @@ static int io_from(const mvd_handle* h, const mvd_io* io, int n_planes, PlaneIO*
     return MVD_OK;
 }
 
+// Scratch of a device-resident call, sized before anything is enqueued (so that the call can be captured).
+static int reserve_resident(mvd_handle* h, int n_planes) {
+    const int B = default_batch(h, n_planes, 4), chunk = default_chunk(h);
+    const int ns = std::min(h->resident_streams, mvd_handle::kSlots);
+    const bool forked = !(ns <= 1 || h->profiling || n_planes < 2 * B);
+    const bool product = h->update_mode == MVD_UPDATE_PRODUCT;
+    size_t a, b, g;
+    int rc = MVD_OK;
+    if (forked) {
+        rc = ensure_streams(h);
+        const int n = std::min(chunk, B);
+        scratch_bytes(h, n, &a, &b, &g);
+        for (int s = 0; s < ns && rc == MVD_OK; ++s) {
+            rc = ws_reserve(h, h->ws_slot[s], a, b, g);
+            if (rc == MVD_OK) rc = pad_reserve(h, h->ws_slot[s], n);
+            if (rc == MVD_OK && product) rc = ws_reserve_product(h, h->ws_slot[s], a, h->path == MVD_PATH_FFT ? b : 0);
+        }
+    } else {
+        const int n = std::min(chunk, n_planes);
+        scratch_bytes(h, n, &a, &b, &g);
+        rc = ws_reserve(h, h->ws_main, a, b, g);
+        if (rc == MVD_OK) rc = pad_reserve(h, h->ws_main, n);
+        if (rc == MVD_OK && product) rc = ws_reserve_product(h, h->ws_main, a, h->path == MVD_PATH_FFT ? b : 0);
+    }
+    return rc;
+}
+
 int mvd_deconvolve_planes_ex(mvd_handle* h, const mvd_io* io, int n_planes, void* stream) {
     if (!h || n_planes < 0) return MVD_ERR_INVALID;
     if (n_planes == 0) return MVD_OK;
     PlaneIO p;
-    const int rc = io_from(h, io, n_planes, &p);
+    int rc = io_from(h, io, n_planes, &p);
     if (rc != MVD_OK) return rc;
-    return run_resident(h, p, n_planes, (cudaStream_t)stream);
+    cudaStream_t st = (cudaStream_t)stream;
+    // Launch-bound calls (small planes, few planes: up to ~4000 launches of a few microseconds) are replayed as one
+    // CUDA graph when the same buffers come again -- the typical loop over time points.  Larger calls gain nothing.
+    const long long est = (long long)((n_planes + default_batch(h, n_planes, 4) - 1) / default_batch(h, n_planes, 4)) *
+                          (4LL * h->T * h->V + 3);
+    const size_t mvox = (size_t)h->W * h->H * (size_t)std::min(n_planes, default_batch(h, n_planes, 4));
+    auto mark_last = [&](int r) {     // order a later host-pipeline call after this one (not while the caller captures)
+        cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+        if (r == MVD_OK && ensure_streams(h) == MVD_OK && cudaStreamIsCapturing(st, &cs) == cudaSuccess &&
+            cs == cudaStreamCaptureStatusNone && cudaEventRecord(h->ev_last, st) == cudaSuccess)
+            h->have_last = true;
+        (void)cudaGetLastError();
+        return r;
+    };
+    if (est > 4096 || mvox > ((size_t)24 << 20) || h->path != MVD_PATH_FFT) return mark_last(run_resident(h, p, n_planes, st));
+    // the direct engine's row-chunk scratch `b` of a uint16 call etc. is covered by ws_reserve inside; for the graph
+    // everything is sized now
+    if ((rc = reserve_resident(h, n_planes)) != MVD_OK) return rc;
+    const uint64_t key[8] = {1u, (uint64_t)(uintptr_t)p.views, (uint64_t)p.lay.view, (uint64_t)p.lay.plane ^ ((uint64_t)p.lay.row << 32),
+                             (uint64_t)(uintptr_t)p.weights, (uint64_t)(uintptr_t)(p.out ? (void*)p.out : (void*)p.out16),
+                             (uint64_t)(p.out16 ? 1 : 0), (uint64_t)n_planes};
+    return mark_last(run_graphed(h, key, st, [&] { return run_resident(h, p, n_planes, st); }));
 }
 
 int mvd_deconvolve_planes(mvd_handle* h, const uint16_t* dev_views_u16, float* dev_out_f32,
@@ -582,13 +707,19 @@ int mvd_deconvolve_host_ex(mvd_handle* h, const mvd_io* io, int n_planes) {
                 if (h->d_w[s]) { cudaFree(h->d_w[s]); h->d_w[s] = nullptr; }
             }
             h->slot_w_planes = 0;
+            h->graph_epoch++;
             for (int s = 0; s < mvd_handle::kSlots && rc0 == MVD_OK; ++s)
                 rc0 = mvd_check(h, cudaMalloc((void**)&h->d_w[s], sizeof(float) * npx * B * h->V));
             if (rc0 == MVD_OK) h->slot_w_planes = (size_t)B;
         }
         size_t a, b, g;
         scratch_bytes(h, std::min(default_chunk(h), B), &a, &b, &g);
-        for (int s = 0; s < mvd_handle::kSlots && rc0 == MVD_OK; ++s) rc0 = ws_reserve(h, h->ws_slot[s], a, b, g);
+        for (int s = 0; s < mvd_handle::kSlots && rc0 == MVD_OK; ++s) {
+            rc0 = ws_reserve(h, h->ws_slot[s], a, b, g);
+            if (rc0 == MVD_OK) rc0 = pad_reserve(h, h->ws_slot[s], std::min(default_chunk(h), B));
+            if (rc0 == MVD_OK && h->update_mode == MVD_UPDATE_PRODUCT)
+                rc0 = ws_reserve_product(h, h->ws_slot[s], a, h->path == MVD_PATH_FFT ? b : 0);
+        }
         if (rc0 != MVD_OK) return rc0;
     }
 
@@ -601,6 +732,8 @@ int mvd_deconvolve_host_ex(mvd_handle* h, const mvd_io* io, int n_planes) {
     // counted from the start of its batch, so a batch that started on an odd plane would pair differently
     // from mvd_deconvolve_planes and the output bits would differ.  An odd stack is split as if it had one
     // plane less and the last plane joins the last batch (or forms a batch of its own when that one is full).
+    if (h->have_last)       // device-resident work enqueued earlier on this handle shares the slots' scratch
+        for (int s = 0; s < mvd_handle::kSlots; ++s) MVD_TRY(h, cudaStreamWaitEvent(h->streams[s], h->ev_last, 0));
     std::vector<int> sizes;
     {
         std::vector<int> ramp;
@@ -653,7 +786,11 @@ int mvd_deconvolve_host_ex(mvd_handle* h, const mvd_io* io, int n_planes) {
         // at most two batches compute at a time (measured: two concurrent batches fill each other's kernel
         // tails, a third only adds contention), while the copies of all three streams overlap freely
         if (rc == MVD_OK && k >= 2) rc = mvd_check(h, cudaStreamWaitEvent(st, h->ev_join[(k - 2) % mvd_handle::kSlots], 0));
-        if (rc == MVD_OK) rc = run_core(h, h->ws_slot[s], p, n, st);
+        if (rc == MVD_OK) {     // the batch's launch sequence depends on the slot and the batch size only: replayed as a graph
+            const uint64_t key[8] = {2u, (uint64_t)s, (uint64_t)n, (uint64_t)B, (uint64_t)(u16 ? 1 : 0) | (host_w ? 2u : 0u) | (camera_order ? 4u : 0u),
+                                     0, 0, 0};
+            rc = run_graphed(h, key, st, [&] { return run_core(h, h->ws_slot[s], p, n, st); });
+        }
         if (rc == MVD_OK) rc = mvd_check(h, cudaEventRecord(h->ev_join[s], st));
         if (rc == MVD_OK)
             rc = mvd_check(h, cudaMemcpyAsync(static_cast<char*>(io->out) + (size_t)p0 * npx * out_elem, h->d_out[s],
@@ -721,24 +858,28 @@ int mvd_get_path(const mvd_handle* h) { return h ? h->path : MVD_ERR_INVALID; }
 int mvd_set_update_mode(mvd_handle* h, int mode) {
     if (!h || (mode != MVD_UPDATE_SEQUENTIAL && mode != MVD_UPDATE_PRODUCT)) return MVD_ERR_INVALID;
     h->update_mode = mode;
+    h->graph_epoch++;
     return MVD_OK;
 }
 
 int mvd_set_chunk_planes(mvd_handle* h, int planes) {
     if (!h || planes < 0) return MVD_ERR_INVALID;
     h->chunk_planes = planes;
+    h->graph_epoch++;
     return MVD_OK;
 }
 
 int mvd_set_resident_streams(mvd_handle* h, int n) {
     if (!h || n < 1 || n > mvd_handle::kSlots) return MVD_ERR_INVALID;
     h->resident_streams = n;
+    h->graph_epoch++;
     return MVD_OK;
 }
 
 int mvd_set_batch_planes(mvd_handle* h, int planes) {
     if (!h || planes < 0) return MVD_ERR_INVALID;
     h->batch_planes = planes;
+    h->graph_epoch++;
     return MVD_OK;
 }
 

@@ -25,6 +25,17 @@ enum KernelClass {
 };
 static_assert(KC_SEP_BACK_UPDATE + 1 == MVD_N_KERNEL_CLASSES, "kernel class table and mvd.h disagree");
 
+// One captured launch sequence (CUDA graph) and what it was captured for.  An entry is valid while the handle's
+// graph_epoch is unchanged: every reallocation of scratch or slots and every setting that changes the launch sequence
+// bumps the epoch.
+struct GraphEntry {
+    uint64_t key[8];
+    uint64_t epoch;
+    cudaGraphExec_t exec;
+    long long launches;     // kernels in the graph (for mvd_launch_count)
+    uint64_t last_use;
+};
+
 struct ProfRecord {
     int kc;
     cudaEvent_t e0, e1;
@@ -97,10 +108,20 @@ struct mvd_handle {
     // joined to the caller's stream, so that one batch's kernel tails overlap the next batch's kernels
     int resident_streams = 2;   // measured: 2 beats 1 by 7-20 % and 3 by 3-10 % on configs 2-5
     cudaEvent_t ev_fork = nullptr, ev_join[kSlots] = {nullptr, nullptr, nullptr};
+    // recorded on the caller's stream at the end of every device-resident call: the host pipeline's streams wait for
+    // it, so that a later mvd_deconvolve_host never touches the slots' scratch while that work is still running
+    cudaEvent_t ev_last = nullptr;
+    bool have_last = false;
 
     int update_mode = 0;    // MVD_UPDATE_SEQUENTIAL / MVD_UPDATE_PRODUCT
     int chunk_planes = 0;   // 0 = default
     int batch_planes = 0;   // 0 = default
+
+    // launch sequences replayed as CUDA graphs (mvd_api.cu: run_graphed): a batch of the host pipeline, or a whole
+    // device-resident call of at most ~4000 launches on the same buffers as an earlier one
+    std::vector<GraphEntry> graphs;
+    uint64_t graph_epoch = 0, graph_clock = 0;
+    bool use_graphs = true;
 
     int last_cuda = 0;
     long long launches = 0;
