@@ -138,7 +138,10 @@ MVD_API int mvd_build_backprojectors(int variant, int n_views, const float* psfs
  *   stream         a cudaStream_t (NULL = legacy default stream).  The call ENQUEUES and returns; it does
  *                  not synchronise -- except that scratch is per handle and grown on demand: a call that needs
  *                  more than is reserved allocates first (see mvd_reserve).  Calls on one handle must all be
- *                  ordered on one stream.
+ *                  ordered on one stream; a later mvd_deconvolve_host* on the handle waits for them by itself.
+ *                  Launch-bound calls (small stacks: at most ~4000 short launches) on the same buffers as an earlier
+ *                  call are replayed as one CUDA graph captured on `stream` the first time; a `stream` that the caller
+ *                  is capturing himself is never captured again.
  * n_planes == 0 is a no-op.  Errors: MVD_ERR_INVALID, MVD_ERR_CUDA, MVD_ERR_NOMEM.
  */
 MVD_API int mvd_deconvolve_planes(mvd_handle* h, const uint16_t* dev_views_u16, float* dev_out_f32,
