@@ -353,6 +353,7 @@ void mvd_destroy(mvd_handle* h) {
     if (h->d_guard_total) cudaFree(h->d_guard_total);
     if (h->d_otf) cudaFree(h->d_otf);
     if (h->d_otf_b) cudaFree(h->d_otf_b);
+    if (h->d_otf_real) cudaFree(h->d_otf_real);
     fft_teardown(h);
     (void)cudaGetLastError();
     delete h;

@@ -75,7 +75,7 @@ __global__ void otf_rows_kernel(const float* __restrict__ P, int K, int W, doubl
 
 // OTF, phase 2: O[ky][kx] = (1 / (W H)) sum_j G[j][kx] exp(-2 pi i ky (j - c) / H)   -> fp32
 __global__ void otf_cols_kernel(const double2* __restrict__ G, int K, int W, int H, float2* __restrict__ O,
-                                int tile_major) {
+                                int tile_major, float* __restrict__ Oreal) {
     const int kx = blockIdx.x * blockDim.x + threadIdx.x, ky = blockIdx.y;
     if (kx >= W) return;
     const int c = (K - 1) / 2;
@@ -91,7 +91,8 @@ __global__ void otf_cols_kernel(const double2* __restrict__ G, int K, int W, int
     }
     const double sc = 1.0 / ((double)W * (double)H);
     const size_t idx = tile_major ? ((size_t)(kx >> 4) * H + ky) * 16 + (kx & 15) : (size_t)ky * W + kx;
-    O[idx] = make_float2((float)(re * sc), (float)(im * sc));
+    if (Oreal) Oreal[idx] = (float)(re * sc);     // centro-symmetric PSF: the imaginary part is round-off only
+    else O[idx] = make_float2((float)(re * sc), (float)(im * sc));
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
@@ -134,6 +135,22 @@ int make_otf_tensor_map(mvd_handle* h, const FftState* st, const float2* otf, CU
     const cuuint64_t dims[2] = {32, (cuuint64_t)(h->W / 16) * h->H};
     const cuuint64_t strides[1] = {128};
     const cuuint32_t box[2] = {(cuuint32_t)st->col->col_box_w, (cuuint32_t)st->col->col_box_h};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = st->encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)otf, dims, strides, box, estr,
+                                  CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+                                  CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        h->last_cuda = (int)cudaErrorInvalidValue;
+        return MVD_ERR_CUDA;
+    }
+    return MVD_OK;
+}
+
+// Tensor map of one view's REAL tile-major OTF, float [(W/16) * H][16]: half the box width of the complex one.
+int make_otf_real_tensor_map(mvd_handle* h, const FftState* st, const float* otf, CUtensorMap* map) {
+    const cuuint64_t dims[2] = {16, (cuuint64_t)(h->W / 16) * h->H};
+    const cuuint64_t strides[1] = {64};
+    const cuuint32_t box[2] = {(cuuint32_t)st->col->col_box_w / 2, (cuuint32_t)st->col->col_box_h};
     const cuuint32_t estr[2] = {1, 1};
     const CUresult r = st->encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, (void*)otf, dims, strides, box, estr,
                                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
@@ -236,10 +253,22 @@ int fft_setup(mvd_handle* h, const float* host_psfs, const float* host_xs) {
     const int W = h->W, H = h->H;
     const size_t npx = (size_t)W * H;
     const bool tile_major = st.row->generation == 2;
+    // Real transfer functions: every PSF centro-symmetric (P[j][i] == P[K-1-j][K-1-i]) and a3 = correlation with P_v
+    // (no explicit back-projector): O_v is real, a1 and a3 use the same array, stored as float (4 B per element
+    // through the column kernels instead of 8, one packed multiply instead of a complex one).
+    bool real_otf = st.col->col_real_otf && !host_xs;
+    for (int v = 0; v < h->V && real_otf; ++v)
+        for (int j = 0; j < h->K && real_otf; ++j)
+            for (int i = 0; i < h->K; ++i)
+                if (host_psfs[((size_t)v * h->K + j) * h->K + i] != host_psfs[((size_t)v * h->K + (h->K - 1 - j)) * h->K + (h->K - 1 - i)]) {
+                    real_otf = false;
+                    break;
+                }
     auto build_otfs = [&](const float* host_k, int K, float2** dst) -> int {
         float* d_k = nullptr;
         double2* d_G = nullptr;
-        MVD_TRY(h, cudaMalloc((void**)dst, sizeof(float2) * npx * h->V));
+        if (real_otf) MVD_TRY(h, cudaMalloc((void**)&h->d_otf_real, sizeof(float) * npx * h->V));
+        else MVD_TRY(h, cudaMalloc((void**)dst, sizeof(float2) * npx * h->V));
         MVD_TRY(h, cudaMalloc((void**)&d_k, sizeof(float) * (size_t)h->V * K * K));
         int r = mvd_check(h, cudaMalloc((void**)&d_G, sizeof(double2) * (size_t)K * W));
         if (r == MVD_OK)
@@ -252,7 +281,8 @@ int fft_setup(mvd_handle* h, const float* host_psfs, const float* host_xs) {
             }
             {
                 LaunchScope ls(h, KC_SETUP, 0);
-                otf_cols_kernel<<<g2, block>>>(d_G, K, W, H, *dst + (size_t)v * npx, tile_major);
+                otf_cols_kernel<<<g2, block>>>(d_G, K, W, H, real_otf ? nullptr : *dst + (size_t)v * npx, tile_major,
+                                               real_otf ? h->d_otf_real + (size_t)v * npx : nullptr);
             }
             r = mvd_check(h, cudaGetLastError());
         }
@@ -267,7 +297,8 @@ int fft_setup(mvd_handle* h, const float* host_psfs, const float* host_xs) {
         FftState* fs = state_of(h);
         fs->otf_maps.resize(h->V);
         for (int v = 0; v < h->V && rc == MVD_OK; ++v)
-            rc = make_otf_tensor_map(h, fs, h->d_otf + (size_t)v * npx, &fs->otf_maps[v]);
+            rc = real_otf ? make_otf_real_tensor_map(h, fs, h->d_otf_real + (size_t)v * npx, &fs->otf_maps[v])
+                          : make_otf_tensor_map(h, fs, h->d_otf + (size_t)v * npx, &fs->otf_maps[v]);
         if (h->d_otf_b) {
             fs->otf_b_maps.resize(h->V);
             for (int v = 0; v < h->V && rc == MVD_OK; ++v)
@@ -385,12 +416,13 @@ int fft_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cudaS
             if (h->V > 1) MVD_TRY(h, cudaMemcpyAsync(ws.d, ws.b, bytes, cudaMemcpyDeviceToDevice, stream));
         }
         for (int v = 0; v < h->V; ++v) {
-            const float2* otf = h->d_otf + (size_t)v * npx;
+            const bool real_otf = h->d_otf_real != nullptr;       // mode 2 of the column kernels; a1 and a3 alike
+            const float2* otf = real_otf ? reinterpret_cast<const float2*>(h->d_otf_real + (size_t)v * npx) : h->d_otf + (size_t)v * npx;
             if (product && v > 0) MVD_TRY(h, cudaMemcpyAsync(ws.b, ws.d, bytes, cudaMemcpyDeviceToDevice, stream));
             a.Z = product ? Acc : Zcur;
             {
                 LaunchScope ls(h, KC_FFT_COLS, stream);
-                rc = mvd_check(h, st->col->cols(tmap, st->otf_maps.empty() ? tmap : st->otf_maps[v], a.S, otf, 0, pairs, W,
+                rc = mvd_check(h, st->col->cols(tmap, st->otf_maps.empty() ? tmap : st->otf_maps[v], a.S, otf, real_otf ? 2 : 0, pairs, W,
                                                 st->tw_col, col_grid, stream));   // a1
             }
             if (rc != MVD_OK) return rc;
@@ -406,7 +438,7 @@ int fft_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cudaS
                 rc = h->d_otf_b      // a3: explicit back-projector B_v, or conj O_v (X = P_v^*)
                          ? mvd_check(h, st->col->cols(tmap, st->otf_b_maps.empty() ? tmap : st->otf_b_maps[v], a.S,
                                                       h->d_otf_b + (size_t)v * npx, 0, pairs, W, st->tw_col, col_grid, stream))
-                         : mvd_check(h, st->col->cols(tmap, st->otf_maps.empty() ? tmap : st->otf_maps[v], a.S, otf, 1, pairs, W,
+                         : mvd_check(h, st->col->cols(tmap, st->otf_maps.empty() ? tmap : st->otf_maps[v], a.S, otf, real_otf ? 2 : 1, pairs, W,
                                                       st->tw_col, col_grid, stream));
             }
             if (rc != MVD_OK) return rc;

@@ -930,6 +930,7 @@ struct SizeOps {
     int row_cps = 0, col_cps = 0;    // generation 2: resident CTAs per SM the persistent grids are sized for
     int row_cps_w = 0;               // ... of the weighted update kernel (twice the landing zone)
     int generation = 1;              // 1: CTA-synchronous TMA-staged kernels (this file); 2: team kernels (mvd_fft_v2.cuh)
+    int col_real_otf = 0;            // the column kernel takes conj_otf == 2: a REAL transfer function stored as float (and its float tensor map)
     int col_tw_custom = 0;           // 1: the column kernel's twiddle table is [R0][N / R0]: exp(-2 pi i t k / N) at [k][t] (two-stage plans with unequal thread counts)
 };
 

@@ -393,7 +393,8 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
     const int c4 = l % CPT, t = l / CPT;
     const ColAddr2<P, CPT> addr{team * H * CPT + c4};
     const TeamSync<TEAM> sync{team};
-    const float sgn = conj_otf ? -1.f : 1.f;
+    const float sgn = conj_otf == 1 ? -1.f : 1.f;
+    const bool real_otf = conj_otf == 2;         // omap / otf describe a float array (mvd_fft.cu: real transfer functions)
     float2* land = buf + team * H * CPT;
     float2* outz = obuf + team * H * CPT;
     uint64_t* full = &bars[team];
@@ -416,10 +417,16 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
     float2 o[OTF_REGS ? E : 1];
     if (OTF_REGS && item < items) {   // the OTF is written once in mvd_create: no dependency on the previous kernel
         const int xg = first_col(item) + c4;
+        if (real_otf) {
+            const float* of = reinterpret_cast<const float*>(otf);
 #pragma unroll
-        for (int e = 0; e < E; ++e) {
-            o[e] = __ldg(otf + plane_off(xg) + (size_t)(t + TPF * e) * 16);
-            o[e].y *= sgn;
+            for (int e = 0; e < E; ++e) o[e] = make_float2(__ldg(of + plane_off(xg) + (size_t)(t + TPF * e) * 16), 0.f);
+        } else {
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                o[e] = __ldg(otf + plane_off(xg) + (size_t)(t + TPF * e) * 16);
+                o[e].y *= sgn;
+            }
         }
     }
     pdl_wait();
@@ -439,22 +446,43 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
             // left by now; it has the whole forward transform's time to arrive.
             bulk_wait_read();
             fence_proxy_async();
-            mbar_arrive_expect_tx(full_otf, (uint32_t)(sizeof(float2) * H * CPT));
             const int oy = (first_col(item) >> 4) * H;
+            if (real_otf) {     // a REAL transfer function (centro-symmetric PSF): one float per element, half the box
+                mbar_arrive_expect_tx(full_otf, (uint32_t)(sizeof(float) * H * CPT));
 #pragma unroll
-            for (int b = 0; b < H / BOXH; ++b) tma_2d_g2s(outz + b * BOXH * CPT, &omap, box_x(item), oy + b * BOXH, full_otf);
+                for (int b = 0; b < H / BOXH; ++b)
+                    tma_2d_g2s(reinterpret_cast<float*>(outz) + b * BOXH * CPT, &omap, box_x(item) >> 1, oy + b * BOXH, full_otf);
+            } else {
+                mbar_arrive_expect_tx(full_otf, (uint32_t)(sizeof(float2) * H * CPT));
+#pragma unroll
+                for (int b = 0; b < H / BOXH; ++b) tma_2d_g2s(outz + b * BOXH * CPT, &omap, box_x(item), oy + b * BOXH, full_otf);
+            }
         }
         fft_run<P, -1>(x, buf, tw, t, addr, sync);
         if (OTF_REGS) {
+            if (real_otf) {
 #pragma unroll
-            for (int e = 0; e < E; ++e) x[e] = cmul(x[e], o[e]);
+                for (int e = 0; e < E; ++e) x[e] = mul2(x[e], make_float2(o[e].x, o[e].x));
+            } else {
+#pragma unroll
+                for (int e = 0; e < E; ++e) x[e] = cmul(x[e], o[e]);
+            }
         } else {
             mbar_wait(full_otf, phase ^ 1);      // same parity sequence as `full`: one completion per item
+            if (real_otf) {
+                const float* of = reinterpret_cast<const float*>(outz);
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    const float w = of[(t + TPF * e) * CPT + c4];
+                    x[e] = mul2(x[e], make_float2(w, w));
+                }
+            } else {
 #pragma unroll
             for (int e = 0; e < E; ++e) {
                 float2 w = outz[(t + TPF * e) * CPT + c4];
                 w.y *= sgn;
                 x[e] = cmul(x[e], w);
+            }
             }
             // no barrier here: the inverse transform's exchanges (team barriers) lie between these
             // reads of the out region and the next writes to it
@@ -512,7 +540,8 @@ fft2_cols_nu_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_const
     const int team = threadIdx.x / TEAM, l = threadIdx.x % TEAM;
     const int c = l % CPT, t = l / CPT;
     const TeamSync<TEAM> sync{team};
-    const float sgn = conj_otf ? -1.f : 1.f;
+    const float sgn = conj_otf == 1 ? -1.f : 1.f;
+    const bool real_otf = conj_otf == 2;         // omap describes a float array (real transfer functions)
     float2* land = buf + team * H * CPT;
     float2* outz = obuf + team * H * CPT;
     uint64_t* full = &bars[team];
@@ -547,10 +576,17 @@ fft2_cols_nu_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_const
         if (l == 0) {   // this item's OTF slice -> the out region, which the previous item's results have left by now
             bulk_wait_read();
             fence_proxy_async();
-            mbar_arrive_expect_tx(full_otf, (uint32_t)(sizeof(float2) * H * CPT));
             const int oy = (first_col(item) >> 4) * H;
+            if (real_otf) {
+                mbar_arrive_expect_tx(full_otf, (uint32_t)(sizeof(float) * H * CPT));
 #pragma unroll
-            for (int b = 0; b < H / BOXH; ++b) tma_2d_g2s(outz + b * BOXH * CPT, &omap, box_x(item), oy + b * BOXH, full_otf);
+                for (int b = 0; b < H / BOXH; ++b)
+                    tma_2d_g2s(reinterpret_cast<float*>(outz) + b * BOXH * CPT, &omap, box_x(item) >> 1, oy + b * BOXH, full_otf);
+            } else {
+                mbar_arrive_expect_tx(full_otf, (uint32_t)(sizeof(float2) * H * CPT));
+#pragma unroll
+                for (int b = 0; b < H / BOXH; ++b) tma_2d_g2s(outz + b * BOXH * CPT, &omap, box_x(item), oy + b * BOXH, full_otf);
+            }
         }
         Bfly<RA, -1>::run(xa);
 #pragma unroll
@@ -564,11 +600,20 @@ fft2_cols_nu_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_const
             for (int j = 0; j < RB; ++j) xb[j] = *slot(t, j);
             Bfly<RB, -1>::run(xb);
             mbar_wait(full_otf, phase ^ 1);      // same parity sequence as `full`: one completion per item
+            if (real_otf) {
+                const float* of = reinterpret_cast<const float*>(outz);
 #pragma unroll
-            for (int k2 = 0; k2 < RB; ++k2) {
-                float2 w = outz[(t + RA * k2) * CPT + c];
-                w.y *= sgn;
-                xb[k2] = cmul(xb[k2], w);
+                for (int k2 = 0; k2 < RB; ++k2) {
+                    const float w = of[(t + RA * k2) * CPT + c];
+                    xb[k2] = mul2(xb[k2], make_float2(w, w));
+                }
+            } else {
+#pragma unroll
+                for (int k2 = 0; k2 < RB; ++k2) {
+                    float2 w = outz[(t + RA * k2) * CPT + c];
+                    w.y *= sgn;
+                    xb[k2] = cmul(xb[k2], w);
+                }
             }
             Bfly<RB, +1>::run(xb);
 #pragma unroll
@@ -667,6 +712,7 @@ struct OpsFor2 {
         o.row_cps_w = kRowCpsW;
         o.col_cps = MINB;
         o.col_otf_regs = OTF_REGS ? 1 : 0;
+        o.col_real_otf = TMA ? 1 : 0;
         return o;
     }
 };
@@ -692,7 +738,7 @@ struct ColsNu2 {
         o.row_threads = 0; o.row_smem = 0;
         o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = kBoxH; o.col_box_w = 8;
         o.rows = nullptr; o.cols = &cols; o.prepare_rows = nullptr; o.prepare_cols = &prepare_cols;
-        o.generation = 2; o.row_cps = 0; o.col_cps = MINB; o.col_otf_regs = 0; o.col_tw_custom = 1;
+        o.generation = 2; o.row_cps = 0; o.col_cps = MINB; o.col_otf_regs = 0; o.col_tw_custom = 1; o.col_real_otf = 1;
         return o;
     }
 };

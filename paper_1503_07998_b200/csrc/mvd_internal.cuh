@@ -86,6 +86,7 @@ struct mvd_handle {
     // fft path: optical transfer functions, float2 [V][H][W], pre-scaled by 1/(W*H)
     float2* d_otf = nullptr;
     float2* d_otf_b = nullptr;   // explicit back-projectors' transfer functions (nullptr: a3 uses conj d_otf)
+    float* d_otf_real = nullptr; // real transfer functions (centro-symmetric PSFs on generation-2 column kernels): replaces d_otf
     int KX = 0;                  // size of the caller's back-projectors (0: Independent variant, X = P_v^*)
     void* fft = nullptr;   // FftState (mvd_fft.cu)
     // fft path, guard: plane pairs with a pixel phi_v > 0 whose blur is below guard_rel x max(psi_0)
