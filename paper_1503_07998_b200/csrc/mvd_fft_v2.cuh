@@ -213,16 +213,22 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
             if (MODE == ROWS_RATIO) {
                 const uint16_t* lu = reinterpret_cast<const uint16_t*>(land);
                 const float tau = a.guard_rel * __uint_as_float(a.gmax[pair]);
-                float bmin = 3.0e38f;    // smallest blur at a pixel that holds photons (guard)
+                // guard: some pixel holds photons (phi >= 1) where the blur is below tau
+                //   <=>  max over the pixels of phi (tau - b) > 0     (two packed operations and one 3-input maximum)
+                float gpos = 0.f;
+                const float2 tau2 = make_float2(tau, tau);
 #pragma unroll
                 for (int e = 0; e < E; ++e) {                                 // a2
                     const int pos = t + TPF * e;
-                    const float fa = (float)lu[pos], fb = (float)lu[W + pos];
-                    bmin = fminf(bmin, fminf(fa > 0.f ? x[e].x : 3.0e38f, fb > 0.f ? x[e].y : 3.0e38f));
-                    x[e].x = __fdividef(fa, fmaxf(x[e].x, a.eps));
-                    x[e].y = __fdividef(fb, fmaxf(x[e].y, a.eps));
+                    // uint16 -> float on the FP32 pipe: 2^23 + u is exact, subtract 2^23 (no conversion-unit trip)
+                    const float2 f = sub2(make_float2(__uint_as_float(0x4B000000u | lu[pos]), __uint_as_float(0x4B000000u | lu[W + pos])),
+                                          make_float2(8388608.f, 8388608.f));
+                    const float2 g = mul2(f, sub2(tau2, x[e]));
+                    gpos = fmaxf(gpos, fmaxf(g.x, g.y));
+                    x[e].x = __fdividef(f.x, fmaxf(x[e].x, a.eps));
+                    x[e].y = __fdividef(f.y, fmaxf(x[e].y, a.eps));
                 }
-                if (valid && bmin < tau) a.gflag[pair] = 1u;
+                if (valid && gpos > 0.f) a.gflag[pair] = 1u;
                 sync();
             } else {
                 if (WT) {
