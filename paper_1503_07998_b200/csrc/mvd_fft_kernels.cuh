@@ -91,13 +91,22 @@ __device__ __forceinline__ float2 fma2(float2 a, float2 b, float2 c) {
     return r;
 }
 __device__ __forceinline__ float2 scale2(float2 a, float s) { return mul2(a, make_float2(s, s)); }
-// a * w
+// a * w = a w.x + (i a) w.y: the two halves of w enter as broadcast scalars and i a = (-a.y, a.x) as a swapped, half-negated
+// view of a -- operand modifiers of FFMA2 / FMUL2 in SASS, so a twiddle loaded from shared memory needs no extra
+// instruction to build (-w.y, w.x)
 __device__ __forceinline__ float2 cmul(float2 a, float2 w) {
-    return fma2(make_float2(a.y, a.y), make_float2(-w.y, w.x), mul2(make_float2(a.x, a.x), w));
+    return fma2(a, make_float2(w.x, w.x), mul2(make_float2(-a.y, a.x), make_float2(w.y, w.y)));
 }
-// a * conj(w)
+// a * conj(w) = a w.x + (-i a) w.y
 __device__ __forceinline__ float2 cmulc(float2 a, float2 w) {
-    return fma2(make_float2(a.y, a.y), make_float2(w.y, w.x), mul2(make_float2(a.x, a.x), make_float2(w.x, -w.y)));
+    return fma2(a, make_float2(w.x, w.x), mul2(make_float2(a.y, -a.x), make_float2(w.y, w.y)));
+}
+// x / d for d in [eps, 2^126): reciprocal on the special-function unit and one multiply (2 ulp), without the range
+// handling __fdividef carries for huge denominators
+__device__ __forceinline__ float div_approx(float x, float d) {
+    float r;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(d));
+    return x * r;
 }
 // a * (-i) for the forward transform (DIR < 0), a * (+i) for the inverse
 template <int DIR>
@@ -777,8 +786,8 @@ __global__ void __launch_bounds__(NT) fft_rows_tma_kernel(RowArgs a, const float
                 const float fa = valid ? (float)pa[pos] : 0.f;
                 const float fb = (valid && has_b) ? (float)pa[W + pos] : 0.f;
                 bmin = fminf(bmin, fminf(fa > 0.f ? x[e].x : 3.0e38f, fb > 0.f ? x[e].y : 3.0e38f));
-                x[e].x = __fdividef(fa, fmaxf(x[e].x, a.eps));
-                x[e].y = __fdividef(fb, fmaxf(x[e].y, a.eps));
+                x[e].x = div_approx(fa, fmaxf(x[e].x, a.eps));
+                x[e].y = div_approx(fb, fmaxf(x[e].y, a.eps));
             }
             if (bmin < tau) a.gflag[pair] = 1u;
         } else {

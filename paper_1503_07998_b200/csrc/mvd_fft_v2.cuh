@@ -225,8 +225,8 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
                                           make_float2(8388608.f, 8388608.f));
                     const float2 g = mul2(f, sub2(tau2, x[e]));
                     gpos = fmaxf(gpos, fmaxf(g.x, g.y));
-                    x[e].x = __fdividef(f.x, fmaxf(x[e].x, a.eps));
-                    x[e].y = __fdividef(f.y, fmaxf(x[e].y, a.eps));
+                    x[e].x = div_approx(f.x, fmaxf(x[e].x, a.eps));
+                    x[e].y = div_approx(f.y, fmaxf(x[e].y, a.eps));
                 }
                 if (valid && gpos > 0.f) a.gflag[pair] = 1u;
                 sync();
