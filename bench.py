@@ -465,6 +465,24 @@ def run_config(cfg, args, steps, warmup, world, local, peaks, traffic_table, fp3
                "h2d_bytes_per_step": int(views.nbytes), "d2h_bytes_per_step": int(host_out.numel() * 4),
                "ms_per_step": dt * 1e3 / e2e_steps, "steps": e2e_steps}
         e2e["ratio_to_device_resident"] = e2e["value"] / value
+        # context: what the PCIe link alone allows -- the step's input copied host -> device and its output device -> host
+        # at the same time on two streams, nothing else running (an upper bound for any host-to-host figure)
+        s_up, s_dn = torch.cuda.Stream(), torch.cuda.Stream()
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(2)]
+        torch.cuda.synchronize()
+        ev[0].record()
+        s_up.wait_event(ev[0]); s_dn.wait_event(ev[0])
+        with torch.cuda.stream(s_up):
+            dev_in.copy_(host_in, non_blocking=True)
+        with torch.cuda.stream(s_dn):
+            host_out.copy_(dev_out, non_blocking=True)
+        torch.cuda.current_stream().wait_stream(s_up); torch.cuda.current_stream().wait_stream(s_dn)
+        ev[1].record()
+        torch.cuda.synchronize()
+        link_ms = ev[0].elapsed_time(ev[1])
+        e2e["pcie_copies_alone_ms"] = link_ms
+        e2e["pcie_bound_value"] = units / (link_ms * 1e-3) / 1e6
+        e2e["ratio_to_min_of_resident_and_pcie_bound"] = e2e["value"] / min(value, e2e["pcie_bound_value"])
         same = True
         for p0 in range(0, N, 256):                          # compare in slices: no second 13 GB host copy
             same = same and bool(torch.equal(host_out[p0:p0 + 256], dev_out[p0:p0 + 256].cpu()))
