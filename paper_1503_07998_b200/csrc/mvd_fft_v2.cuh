@@ -40,12 +40,18 @@ __device__ __forceinline__ int swz(int p) {
     static_assert(R0 == 16 || R0 == 32, "the XOR swizzle is derived for first radices 16 and 32");
     return p ^ ((p / R0) & 15);
 }
-// one FFT per region of N slots
+// One FFT per region of N + N / R0 slots, position p in slot p + p / R0 (one spare slot per R0).  For the ROW kernels this
+// padding does what the XOR swizzle does -- stage 0's stores (positions R0 t + m: slots (R0 + 1) t + m) and the loads
+// (positions t + TPF e: consecutive slots) are both conflict-free for 8-byte elements -- and, unlike the XOR, it leaves
+// every address an immediate offset from one per-thread base: no LOP3 / IADD3 per access (9 % of the row kernels'
+// instructions).
 template <class P>
 struct RowAddr2 {
     int base;
-    __device__ __forceinline__ int operator()(int pos) const { return base + swz<P>(pos); }
+    __device__ __forceinline__ int operator()(int pos) const { return base + pos + pos / P::radix(0); }
 };
+template <class P>
+__host__ __device__ constexpr int row_pitch(int slots) { return slots + slots / P::radix(0); }
 // CPT FFTs (adjacent columns) interleaved: [slot][CPT]
 template <class P, int CPT = 4>
 struct ColAddr2 {
@@ -90,12 +96,13 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
     // ShflTail plans: threads t and t ^ 32 of an FFT sit in lanes l and l ^ 16 of one warp
     const int t = shfl_tail<P>() ? ((int)(threadIdx.x & 16) << 1) | ((int)(threadIdx.x & 32) >> 1) | (int)(threadIdx.x & 15)
                                  : (int)threadIdx.x % TPF;
-    const RowAddr2<P> addr{team * RW};
+    constexpr int RWP = row_pitch<P>(RW);   // pitch of a team's region
+    const RowAddr2<P> addr{team * RWP};
     const TeamSync<TPF> sync{team};
     const size_t npx = (size_t)a.H * W;
     const int stride = gridDim.x * RP;
     const uint16_t* vp = a.views + (size_t)a.v * a.view_stride;
-    float2* land = buf + team * RW;                           // the team's region, used linearly as landing zone
+    float2* land = buf + team * RWP;                          // the team's region, used linearly as landing zone
     const float* wv = WT ? a.weights + (size_t)a.v * a.w_view : nullptr;
     const int last_row = a.total_rows - 1;
 
@@ -667,8 +674,8 @@ inline cudaError_t launch_pdl(Kern kern, dim3 grid, dim3 block, size_t smem, cud
 template <class P, int NT, class PC, int NTC, bool OTF_REGS, int MINB, bool TMA = true, int CPT = 4, int RMINB = 2>
 struct OpsFor2 {
     static_assert(P::N == PC::N, "row and column plan of one entry describe the same length");
-    static constexpr size_t kRowSmem = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * P::N);
-    static constexpr size_t kRowSmemW = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * 2 * P::N);
+    static constexpr size_t kRowSmem = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * row_pitch<P>(P::N));
+    static constexpr size_t kRowSmemW = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * row_pitch<P>(2 * P::N));
     static constexpr int kRowCpsW = (int)((228u * 1024u) / (kRowSmemW + 1024)) < RMINB ? (int)((228u * 1024u) / (kRowSmemW + 1024)) : RMINB;
     static_assert(kRowSmemW <= 227u * 1024u && kRowCpsW >= 1, "the weighted update kernel fits one CTA");
     static constexpr int kTeam = CPT * PC::TPF, kNTeam = NTC / kTeam, kTC = CPT * kNTeam;
