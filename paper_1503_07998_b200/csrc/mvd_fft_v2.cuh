@@ -59,6 +59,15 @@ struct ColAddr2 {
     __device__ __forceinline__ int operator()(int pos) const { return base + CPT * swz<P>(pos); }
 };
 
+// The same with padding instead of the XOR (TMA-fed column kernels): position p in slot p + p / R0 of a region of
+// H + H / R0 slots.  Stage 0's stores ((R0 + 1) t + m: four consecutive t fall into the four 32-byte groups of a line) and
+// the loads (consecutive slots) stay conflict-free, and every address is an immediate offset from one base.
+template <class P, int CPT = 4>
+struct ColAddrPad {
+    int base;   // team region + column within the team
+    __device__ __forceinline__ int operator()(int pos) const { return base + CPT * (pos + pos / P::radix(0)); }
+};
+
 // 16-byte asynchronous copy global -> shared (SASS LDGSTS), no registers in between
 __device__ __forceinline__ void cp_async16(void* dst, const void* src) {
     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
@@ -393,10 +402,12 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
     constexpr int TW = (P::S - 1) * E * TPF;                  // a multiple of 16 float2: regions stay 128-byte aligned
     static_assert(TW % 16 == 0, "twiddle table keeps the regions aligned");
     float2* tw = smem_cols3;                                  // [(S-1) E][TPF]
-    // the exchange region is the landing zone of the next item
-    float2* buf = smem_cols3 + TW;                            // [NTEAM][H][CPT]  exchange regions / landing zones
-    float2* obuf = buf + NTEAM * H * CPT;                     // [NTEAM][H][CPT]  OTF slices, then results on their way out
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_cols3 + TW + 2 * NTEAM * H * CPT);   // [2][NTEAM]
+    // the exchange region (padded: H + H / R0 slots per column) is the landing zone of the next item
+    constexpr int HP = H + H / P::radix(0);
+    static_assert((HP * CPT) % 16 == 0, "regions stay 128-byte aligned");
+    float2* buf = smem_cols3 + TW;                            // [NTEAM][HP][CPT]  exchange regions / landing zones
+    float2* obuf = buf + NTEAM * HP * CPT;                    // [NTEAM][H][CPT]  OTF slices, then results on their way out
+    uint64_t* bars = reinterpret_cast<uint64_t*>(obuf + NTEAM * H * CPT);   // [2][NTEAM]
     if (threadIdx.x < 2 * NTEAM) mbar_init(&bars[threadIdx.x], 1);
     if (threadIdx.x == 0) fence_mbar_init();
     for (int k = threadIdx.x; k < TW; k += NT) tw[k] = tw_g[k];
@@ -404,11 +415,11 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
     pdl_launch_dependents();
     const int team = threadIdx.x / TEAM, l = threadIdx.x % TEAM;
     const int c4 = l % CPT, t = l / CPT;
-    const ColAddr2<P, CPT> addr{team * H * CPT + c4};
+    const ColAddrPad<P, CPT> addr{team * HP * CPT + c4};
     const TeamSync<TEAM> sync{team};
     const float sgn = conj_otf == 1 ? -1.f : 1.f;
     const bool real_otf = conj_otf == 2;         // omap / otf describe a float array (mvd_fft.cu: real transfer functions)
-    float2* land = buf + team * H * CPT;
+    float2* land = buf + team * HP * CPT;
     float2* outz = obuf + team * H * CPT;
     uint64_t* full = &bars[team];
     uint64_t* full_otf = &bars[NTEAM + team];   // !OTF_REGS: the team's OTF slice lands in the out region
@@ -542,8 +553,9 @@ fft2_cols_nu_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_const
     constexpr int TW = RA * RB;
     static_assert(TW % 16 == 0, "twiddle table keeps the regions aligned");
     float2* tw = smem_cols5;                                  // [RA][RB]
-    float2* buf = smem_cols5 + TW;                            // [NTEAM][H][CPT]  exchange regions / landing zones
-    float2* obuf = buf + NTEAM * H * CPT;                     // [NTEAM][H][CPT]  OTF slices, then results on their way out
+    constexpr int PB = (RA * (RB + 1) * CPT + 15) / 16 * 16;  // exchange region: slot (k1, t) at k1 (RB + 1) + t, 128-byte aligned
+    float2* buf = smem_cols5 + TW;                            // [NTEAM][PB]  exchange regions / landing zones ([H][CPT] linear)
+    float2* obuf = buf + NTEAM * PB;                          // [NTEAM][H][CPT]  OTF slices, then results on their way out
     uint64_t* bars = reinterpret_cast<uint64_t*>(obuf + NTEAM * H * CPT);   // [2][NTEAM]
     if (threadIdx.x < 2 * NTEAM) mbar_init(&bars[threadIdx.x], 1);
     if (threadIdx.x == 0) fence_mbar_init();
@@ -555,13 +567,14 @@ fft2_cols_nu_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_const
     const TeamSync<TEAM> sync{team};
     const float sgn = conj_otf == 1 ? -1.f : 1.f;
     const bool real_otf = conj_otf == 2;         // omap describes a float array (real transfer functions)
-    float2* land = buf + team * H * CPT;
+    float2* land = buf + team * PB;
     float2* outz = obuf + team * H * CPT;
     uint64_t* full = &bars[team];
     uint64_t* full_otf = &bars[NTEAM + team];
-    // exchange slot of (k1, t): four consecutive t (stage A stores) and four consecutive k1 (stage B loads) both
-    // spread over the four 32-byte groups of a 128-byte line
-    auto slot = [&](int k1, int tt) { return land + ((k1 * RB + (tt ^ (k1 & 3))) * CPT + c); };
+    // exchange slot of (k1, t) = k1 (RB + 1) + t: four consecutive t (stage A stores) and four consecutive k1 (stage B,
+    // RB + 1 = 1 mod 4) both spread over the four 32-byte groups of a 128-byte line, and every address is an immediate
+    // offset from one per-thread base
+    auto slot = [&](int k1, int tt) { return land + ((k1 * (RB + 1) + tt) * CPT + c); };
     const int tiles = W / TC;
     const int items = tiles * pairs;
     auto first_col = [&](int item) { return (item % tiles) * TC + team * CPT; };
@@ -679,7 +692,8 @@ struct OpsFor2 {
     static constexpr int kRowCpsW = (int)((228u * 1024u) / (kRowSmemW + 1024)) < RMINB ? (int)((228u * 1024u) / (kRowSmemW + 1024)) : RMINB;
     static_assert(kRowSmemW <= 227u * 1024u && kRowCpsW >= 1, "the weighted update kernel fits one CTA");
     static constexpr int kTeam = CPT * PC::TPF, kNTeam = NTC / kTeam, kTC = CPT * kNTeam;
-    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF + (size_t)(TMA ? 2 : 1) * kNTeam * PC::N * CPT) +
+    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF +
+                                                         (size_t)kNTeam * CPT * (TMA ? 2 * PC::N + PC::N / PC::radix(0) : PC::N)) +
                                        (TMA ? 2 * sizeof(uint64_t) * kNTeam : 0);
 
     static cudaError_t rows(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st) {
@@ -735,7 +749,8 @@ template <int RA, int RB, int NTC, int MINB>
 struct ColsNu2 {
     static constexpr int kN = RA * RB, kNTeam = NTC / (4 * RB), kTC = 4 * kNTeam;
     static constexpr int kBoxH = kN <= 256 ? kN : (kN % 256 == 0 ? 256 : 200);
-    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)RA * RB + (size_t)2 * kNTeam * kN * 4) + 2 * sizeof(uint64_t) * kNTeam;
+    static constexpr size_t kColSmem = sizeof(float2) * ((size_t)RA * RB + (size_t)kNTeam * ((RA * (RB + 1) * 4 + 15) / 16 * 16 + kN * 4)) +
+                                       2 * sizeof(uint64_t) * kNTeam;
     static cudaError_t cols(const CUtensorMap& tmap, const CUtensorMap& otf_map, float2*, const float2*, int conj_otf, int pairs, int W,
                             const float2* tw, dim3 grid, cudaStream_t st) {
         return launch_pdl(fft2_cols_nu_kernel<RA, RB, NTC, MINB>, grid, dim3(NTC), kColSmem, st, tmap, otf_map, conj_otf, pairs, W, tw);
