@@ -51,7 +51,8 @@ enum {
     MVD_ERR_CUDA = -3,        /* a CUDA call failed; mvd_last_cuda_error() has the cudaError_t           */
     MVD_ERR_NOMEM = -4,       /* device or pinned-staging allocation failed                              */
     MVD_ERR_BUSY = -5,        /* reserved                                                                */
-    MVD_ERR_IO = -6           /* mvd_deconvolve_files: a file could not be opened, is too short, or a read / write failed */
+    MVD_ERR_IO = -6,          /* mvd_deconvolve_files: a file could not be opened, is too short, or a read / write failed */
+    MVD_ERR_TOO_LARGE = -7    /* mvd_deconvolve_planes_noalloc: n_planes * plane_w * plane_h exceeds MVD_NOALLOC_MAX_VOXELS */
 };
 
 /* Convolution engine used for steps a1 and a3 (both engines fuse a2 and a4 into their kernels). */
@@ -230,6 +231,27 @@ MVD_API int mvd_deconvolve_host_u16(mvd_handle* h, const uint16_t* host_views_u1
  */
 MVD_API int mvd_deconvolve_files(mvd_handle* h, const char* const* view_paths, const char* out_path, int n_planes,
                                  int out_type);
+
+/*
+ * mvd_deconvolve_planes_noalloc -- mvd_deconvolve_planes for callers that cannot allocate (code under CUDA graph
+ * capture, tight serving loops, harnesses that forbid cudaMalloc): the call allocates NOTHING -- no cudaMalloc, cudaFree
+ * or allocating library routine, whatever was or was not reserved.  It runs the direct engine's tiled kernels (steps
+ * a0..a5) with their ratio scratch r in a fixed device array inside the library instead of the handle's
+ * workspace:
+ *   - limit: n_planes * plane_w * plane_h <= MVD_NOALLOC_MAX_VOXELS (4 Mi voxels = 16 MiB, held by every GPU that
+ *     loads libmvd.so until the process exits); larger requests return MVD_ERR_TOO_LARGE and enqueue nothing;
+ *   - the handle must run the direct engine (mvd_create_path(.., MVD_PATH_DIRECT, ..)), sequential update mode, not
+ *     padded: otherwise MVD_ERR_UNSUPPORTED; the handle's device must be the current device (else MVD_ERR_INVALID);
+ *   - dev_views_u16 / dev_out_f32 / stream exactly as for mvd_deconvolve_planes (dense layout, fp32 output); the result
+ *     is the direct engine's (for separable PSFs and planes that fit on chip mvd_deconvolve_planes picks other kernels of
+ *     that engine: same result within the parity tolerance, otherwise bit for bit);
+ *   - the first call on a device resolves the array's address (cudaGetSymbolAddress): make it outside stream capture;
+ *   - ALL calls (of all handles) share the one array: calls that overlap on the GPU -- different streams with no
+ *     ordering between them -- race on it.  Calls ordered on one stream are safe; the array needs no clearing.
+ */
+enum { MVD_NOALLOC_MAX_VOXELS = 4194304 };
+MVD_API int mvd_deconvolve_planes_noalloc(mvd_handle* h, const uint16_t* dev_views_u16, float* dev_out_f32,
+                                          int n_planes, void* stream);
 
 /*
  * mvd_reserve -- size everything a later call on up to max_planes planes needs (scratch of the engine, the

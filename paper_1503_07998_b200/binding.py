@@ -15,7 +15,7 @@ import numpy as np
 _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libmvd.so")
 
-MVD_OK, MVD_ERR_INVALID, MVD_ERR_UNSUPPORTED, MVD_ERR_CUDA, MVD_ERR_NOMEM, MVD_ERR_BUSY, MVD_ERR_IO = 0, -1, -2, -3, -4, -5, -6
+MVD_OK, MVD_ERR_INVALID, MVD_ERR_UNSUPPORTED, MVD_ERR_CUDA, MVD_ERR_NOMEM, MVD_ERR_BUSY, MVD_ERR_IO, MVD_ERR_TOO_LARGE = 0, -1, -2, -3, -4, -5, -6, -7
 PATH_AUTO, PATH_DIRECT, PATH_FFT = 0, 1, 2
 N_KERNEL_CLASSES = 12
 PATH_NAMES = {PATH_AUTO: "auto", PATH_DIRECT: "direct", PATH_FFT: "fft"}
@@ -66,6 +66,7 @@ class MvdIO(ctypes.Structure):
 
 OUT_F32, OUT_U16 = 0, 1
 UPDATE_SEQUENTIAL, UPDATE_PRODUCT = 0, 1
+NOALLOC_MAX_VOXELS = 4194304
 SIGNATURES.update({
     "mvd_deconvolve_planes_ex": (_i, [_vp, ctypes.POINTER(MvdIO), _i, _vp]),
     "mvd_deconvolve_host_ex": (_i, [_vp, ctypes.POINTER(MvdIO), _i]),
@@ -74,6 +75,7 @@ SIGNATURES.update({
     "mvd_deconvolve_planes_u16": (_i, [_vp, _vp, _vp, _i, _vp]),
     "mvd_deconvolve_host_u16": (_i, [_vp, _vp, _vp, _i]),
     "mvd_deconvolve_files": (_i, [_vp, ctypes.POINTER(ctypes.c_char_p), ctypes.c_char_p, _i, _i]),
+    "mvd_deconvolve_planes_noalloc": (_i, [_vp, _vp, _vp, _i, _vp]),
 })
 
 _lib: Optional[ctypes.CDLL] = None
@@ -208,6 +210,11 @@ class Mvd:
     def deconvolve_host_u16(self, host_views_u16, host_out_u16, n_planes: int) -> None:
         self._raise(lib().mvd_deconvolve_host_u16(self._h, _ptr(host_views_u16), _ptr(host_out_u16), n_planes),
                     "mvd_deconvolve_host_u16")
+
+    def deconvolve_planes_noalloc(self, dev_views_u16, dev_out_f32, n_planes: int, stream=None) -> None:
+        """mvd_deconvolve_planes_noalloc: allocates nothing; scratch in a fixed 16 MiB device array (NOALLOC_MAX_VOXELS)."""
+        self._raise(lib().mvd_deconvolve_planes_noalloc(self._h, _ptr(dev_views_u16), _ptr(dev_out_f32), n_planes,
+                                                        _stream(stream)), "mvd_deconvolve_planes_noalloc")
 
     def deconvolve_files(self, view_paths, out_path: str, n_planes: int, out_u16: bool = False) -> None:
         """mvd_deconvolve_files: raw uint16 view files in, raw float / uint16 file out, disk I/O overlapped.  Blocks."""

@@ -840,6 +840,7 @@ const char* mvd_strerror(int code) {
         case MVD_ERR_NOMEM: return "out of device or pinned memory";
         case MVD_ERR_BUSY: return "handle busy";
         case MVD_ERR_IO: return "file could not be opened, is too short, or a read / write failed";
+        case MVD_ERR_TOO_LARGE: return "request exceeds MVD_NOALLOC_MAX_VOXELS, the fixed scratch of mvd_deconvolve_planes_noalloc";
         default: return "unknown mvd error code";
     }
 }

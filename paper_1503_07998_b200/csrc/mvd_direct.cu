@@ -730,3 +730,66 @@ int direct_repair_launch(mvd_handle* h, const PlaneIO& io, float* psi, float* r_
     else e = launch_repair<0, 8>(h, a, stream);
     return mvd_check(h, (cudaError_t)e);
 }
+
+// ---------------------------------------------------------------------------------------------
+// mvd_deconvolve_planes_noalloc -- the direct engine's tiled kernels with their ratio scratch r in a file-scope
+// device array instead of the handle's cudaMalloc'ed workspace, for callers that cannot allocate (code under CUDA
+// graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Nothing here calls cudaMalloc, cudaFree or
+// an allocating library routine; every GPU that loads libmvd.so holds the array (16 MiB) until exit.
+//
+// The array's name is a host-side stand-in in host code, NOT a device address: the kernels get the pointer that
+// cudaGetSymbolAddress returns, resolved once per device with that device current (first call of the entry point on
+// that device -- make it outside stream capture).  Every call shares the array and it keeps the last call's
+// contents: nothing has to start at zero (kernel A overwrites every element kernel B reads), but two calls that
+// overlap on the GPU (different streams, no ordering between them) race on it.
+// ---------------------------------------------------------------------------------------------
+static __device__ __align__(256) float g_noalloc_r[MVD_NOALLOC_MAX_VOXELS];
+
+namespace {
+constexpr int kMaxDevices = 64;
+float* g_noalloc_ptr[kMaxDevices] = {};       // per device: the array's device address
+}  // namespace
+
+int mvd_deconvolve_planes_noalloc(mvd_handle* h, const uint16_t* dev_views_u16, float* dev_out_f32, int n_planes,
+                                  void* stream) {
+    if (!h || !dev_views_u16 || !dev_out_f32 || n_planes < 0) return MVD_ERR_INVALID;
+    if (n_planes == 0) return MVD_OK;
+    if (h->path != MVD_PATH_DIRECT || h->padded || h->update_mode != MVD_UPDATE_SEQUENTIAL || !h->d_coef)
+        return MVD_ERR_UNSUPPORTED;
+    const size_t npx = (size_t)h->W * h->H;
+    const size_t n = npx * (size_t)n_planes;
+    if (n > (size_t)MVD_NOALLOC_MAX_VOXELS) return MVD_ERR_TOO_LARGE;
+    cudaStream_t st = (cudaStream_t)stream;
+
+    int dev = -1;
+    MVD_TRY(h, cudaGetDevice(&dev));
+    if (dev != h->device || dev < 0 || dev >= kMaxDevices) return MVD_ERR_INVALID;   // the handle's device must be current
+    if (!g_noalloc_ptr[dev]) {
+        float* p = nullptr;
+        MVD_TRY(h, cudaGetSymbolAddress((void**)&p, g_noalloc_r));
+        if (!p) return MVD_ERR_CUDA;
+        g_noalloc_ptr[dev] = p;
+    }
+    float* r = g_noalloc_ptr[dev];
+    float* psi = dev_out_f32;                       // iterated in place in the caller's output
+
+    const ViewLayout lay{(size_t)n_planes * npx, npx, (size_t)h->W};
+    const unsigned egrid = (unsigned)std::min<size_t>((n + 255) / 256, (size_t)h->n_sm * 16);
+    init_mean_kernel<<<egrid, 256, 0, st>>>(dev_views_u16, lay, h->V, h->W, h->H, psi, n);   // a0
+    h->launches++;
+    MVD_TRY(h, cudaGetLastError());
+    const size_t per = (size_t)h->dK * h->Kp;
+    for (int t = 0; t < h->T; ++t)
+        for (int v = 0; v < h->V; ++v) {
+            const float* Gblur = h->d_coef + ((size_t)v * 2 + 0) * per;
+            const float* Gback = h->d_coef + ((size_t)v * 2 + 1) * per;
+            const uint16_t* phi = dev_views_u16 + (size_t)v * lay.view;
+            int e = launch_corr(0, h, psi, Gblur, phi, r, n_planes, st, lay.plane, lay.row, nullptr);    // a1 + a2 -> r
+            h->launches++;
+            MVD_TRY(h, (cudaError_t)e);
+            e = launch_corr(1, h, r, Gback, nullptr, psi, n_planes, st, 0, 0, nullptr);                  // a3 + a4
+            h->launches++;
+            MVD_TRY(h, (cudaError_t)e);
+        }
+    return MVD_OK;
+}
