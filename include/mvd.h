@@ -150,7 +150,7 @@ MVD_API int mvd_deconvolve_planes(mvd_handle* h, const uint16_t* dev_views_u16, 
 
 /*
  * mvd_deconvolve_host -- the same result for host-resident stacks, streamed through the GPU in batches
- * of planes on three CUDA streams so that H2D copies, the RL iterations and D2H copies of different
+ * of planes on CUDA streams (four by default, the paper's three with mvd_set_pipeline_streams) so that H2D copies, the RL iterations and D2H copies of different
  * batches overlap (Algorithm 1, with pinned host buffers standing in for disk IO).
  *   host_views_u16  HOST (pinned for overlap; pageable memory works but serialises), same layout as above.
  *   host_out_f32    HOST, float [n_planes][plane_h][plane_w].
@@ -313,10 +313,14 @@ MVD_API int mvd_set_update_mode(mvd_handle* h, int mode);
  * Tuning knobs (measurement; defaults are chosen in mvd_create).
  *   mvd_set_chunk_planes  planes processed per internal pass of mvd_deconvolve_planes (0 = default)
  *   mvd_set_batch_planes  planes per pipeline batch of mvd_deconvolve_host (0 = default)
+ *   mvd_set_pipeline_streams  3 or 4 (default 4): streams = batch slots that mvd_deconvolve_host* cycles through.  Algorithm 1
+ *                          has three; with two batches computing at a time a stream spends ~40 % of its cycle in
+ *                         its own H2D / D2H copies, so a fourth keeps two batches computing (config 2: +4 %); bit-identical
  *   mvd_set_resident_streams  1..3: mvd_deconvolve_planes deals batches of planes (the pipeline's batch size)
  *                         to this many internal streams forked from / joined to the caller's stream, so that
  *                         kernel tails of one batch overlap the next batch; results are bit-identical
  */
+MVD_API int mvd_set_pipeline_streams(mvd_handle* h, int n);
 MVD_API int mvd_set_resident_streams(mvd_handle* h, int n);
 MVD_API int mvd_set_chunk_planes(mvd_handle* h, int planes);
 MVD_API int mvd_set_batch_planes(mvd_handle* h, int planes);

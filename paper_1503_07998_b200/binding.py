@@ -46,6 +46,7 @@ SIGNATURES = {
     "mvd_set_chunk_planes": (_i, [_vp, _i]),
     "mvd_set_batch_planes": (_i, [_vp, _i]),
     "mvd_set_resident_streams": (_i, [_vp, _i]),
+    "mvd_set_pipeline_streams": (_i, [_vp, _i]),
     "mvd_launch_count": (_ll, [_vp]),
     "mvd_launch_count_reset": (None, [_vp]),
     "mvd_profile_enable": (_i, [_vp, _i]),
@@ -266,6 +267,9 @@ class Mvd:
 
     def set_resident_streams(self, n: int) -> None:
         self._raise(lib().mvd_set_resident_streams(self._h, n), "mvd_set_resident_streams")
+
+    def set_pipeline_streams(self, n: int) -> None:
+        self._raise(lib().mvd_set_pipeline_streams(self._h, n), "mvd_set_pipeline_streams")
 
     def set_batch_planes(self, planes: int) -> None:
         self._raise(lib().mvd_set_batch_planes(self._h, planes), "mvd_set_batch_planes")

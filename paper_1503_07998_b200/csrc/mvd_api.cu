@@ -733,8 +733,6 @@ int mvd_deconvolve_host_ex(mvd_handle* h, const mvd_io* io, int n_planes) {
     // counted from the start of its batch, so a batch that started on an odd plane would pair differently
     // from mvd_deconvolve_planes and the output bits would differ.  An odd stack is split as if it had one
     // plane less and the last plane joins the last batch (or forms a batch of its own when that one is full).
-    if (h->have_last)       // device-resident work enqueued earlier on this handle shares the slots' scratch
-        for (int s = 0; s < mvd_handle::kSlots; ++s) MVD_TRY(h, cudaStreamWaitEvent(h->streams[s], h->ev_last, 0));
     std::vector<int> sizes;
     {
         std::vector<int> ramp;
@@ -751,10 +749,16 @@ int mvd_deconvolve_host_ex(mvd_handle* h, const mvd_io* io, int n_planes) {
             else sizes.push_back(1);
         }
     }
+    const int P = h->pipeline_slots;
+    const int used = std::min<int>(P, (int)sizes.size());      // streams this call touches (small stacks: one)
+    if (h->have_last) {     // device-resident work enqueued earlier on this handle shares the slots' scratch
+        for (int s = 0; s < used; ++s) MVD_TRY(h, cudaStreamWaitEvent(h->streams[s], h->ev_last, 0));
+        h->have_last = false;   // ... and everything enqueued here is complete when this call returns
+    }
     int rc = MVD_OK;
     int k = 0, p0 = 0;
     for (size_t bi = 0; bi < sizes.size() && rc == MVD_OK; p0 += sizes[bi], ++bi, ++k) {
-        const int s = k % mvd_handle::kSlots;
+        const int s = k % P;
         const int n = sizes[bi];
         cudaStream_t st = h->streams[s];
         PlaneIO p;
@@ -786,7 +790,7 @@ int mvd_deconvolve_host_ex(mvd_handle* h, const mvd_io* io, int n_planes) {
         else p.out = h->d_out[s];
         // at most two batches compute at a time (measured: two concurrent batches fill each other's kernel
         // tails, a third only adds contention), while the copies of all three streams overlap freely
-        if (rc == MVD_OK && k >= 2) rc = mvd_check(h, cudaStreamWaitEvent(st, h->ev_join[(k - 2) % mvd_handle::kSlots], 0));
+        if (rc == MVD_OK && k >= 2) rc = mvd_check(h, cudaStreamWaitEvent(st, h->ev_join[(k - 2) % P], 0));
         if (rc == MVD_OK) {     // the batch's launch sequence depends on the slot and the batch size only: replayed as a graph
             const uint64_t key[8] = {2u, (uint64_t)s, (uint64_t)n, (uint64_t)B, (uint64_t)(u16 ? 1 : 0) | (host_w ? 2u : 0u) | (camera_order ? 4u : 0u),
                                      0, 0, 0};
@@ -797,7 +801,7 @@ int mvd_deconvolve_host_ex(mvd_handle* h, const mvd_io* io, int n_planes) {
             rc = mvd_check(h, cudaMemcpyAsync(static_cast<char*>(io->out) + (size_t)p0 * npx * out_elem, h->d_out[s],
                                              out_elem * npx * n, cudaMemcpyDeviceToHost, st));
     }
-    for (int s = 0; s < mvd_handle::kSlots; ++s) {
+    for (int s = 0; s < used; ++s) {
         int rs = mvd_check(h, cudaStreamSynchronize(h->streams[s]));
         if (rc == MVD_OK) rc = rs;
     }
@@ -872,8 +876,15 @@ int mvd_set_chunk_planes(mvd_handle* h, int planes) {
 }
 
 int mvd_set_resident_streams(mvd_handle* h, int n) {
-    if (!h || n < 1 || n > mvd_handle::kSlots) return MVD_ERR_INVALID;
+    if (!h || n < 1 || n > 3) return MVD_ERR_INVALID;
     h->resident_streams = n;
+    h->graph_epoch++;
+    return MVD_OK;
+}
+
+int mvd_set_pipeline_streams(mvd_handle* h, int n) {
+    if (!h || n < 3 || n > mvd_handle::kSlots) return MVD_ERR_INVALID;
+    h->pipeline_slots = n;
     h->graph_epoch++;
     return MVD_OK;
 }

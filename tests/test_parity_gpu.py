@@ -189,6 +189,27 @@ def test_host_pipeline_with_ramp_and_odd_plane_count_is_bit_identical():
 
 
 @pytest.mark.parametrize("path", PATHS)
+def test_three_and_four_pipeline_streams_are_bit_identical(path):
+    """mvd_set_pipeline_streams: the paper's three streams and the default four give the same bits as the resident call."""
+    import torch
+    V, N, W, H, K, T = 2, 23, 96, 64, 7, 3
+    _need(path, W, H, K)
+    pr = synth.make_problem(V, N, W, H, K, T, seed=99)
+    ref = _run(pr.views, pr.psfs, T, path)
+    hv = torch.from_numpy(pr.views.view(np.int16)).pin_memory()
+    for n in (3, 4):
+        ho = torch.empty((N, H, W), dtype=torch.float32).pin_memory()
+        with binding.Mvd(W, H, V, pr.psfs, K, T, float(synth.EPS), path) as m:
+            m.set_pipeline_streams(n)
+            m.set_batch_planes(2)
+            m.deconvolve_host(hv, ho, N)
+            m.deconvolve_host(hv, ho, N)          # second call: replayed batches
+            with pytest.raises(binding.MvdError):
+                m.set_pipeline_streams(5)
+        assert np.array_equal(ho.numpy(), ref), n
+
+
+@pytest.mark.parametrize("path", PATHS)
 def test_reserved_handle_is_capturable_into_a_cuda_graph(path):
     """After mvd_reserve the device-resident call only enqueues (no allocation, no synchronisation): it can be
     captured into a CUDA graph and replayed, with the same bits as the eager call."""
