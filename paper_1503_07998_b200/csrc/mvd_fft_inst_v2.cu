@@ -10,8 +10,10 @@ const SizeOps* mvd_fft_ops_v2(int N) {
     static const SizeOps o256 = OpsFor2<P256, 256, P256, 128, true, 4>::make();
     static const SizeOps o512 = OpsFor2<P512, 256, P512, 128, false, 3>::make();
     static const SizeOps o1024 = OpsFor2<P1024, 256, P1024, 128, false, 3>::make();
-    // rows: 3 CTAs of 2 teams, 168 registers; the exchange in front of the radix-2 stage goes through warp shuffles
-    static const SizeOps o2048 = OpsFor2<ShflTail<P2048>, 128, P2048, 256, false, 2, false, 4, 3>::make();
+    // rows: the exchange in front of the radix-2 stage goes through warp shuffles; 2 CTAs of 4 teams at 128 registers (since the
+    // instruction diet they fit without spills).  3 CTAs of 2 teams at 168 registers run the update pass 3 % faster ALONE but the
+    // whole step, with two batches in flight, 1.5 % slower (profiles/r2_experiments.md)
+    static const SizeOps o2048 = OpsFor2<ShflTail<P2048>, 256, P2048, 256, false, 2, false, 4, 2>::make();
     // columns only: 800 = 25 x 32 with unequal thread counts per stage, four columns per team of four warps
     static const SizeOps o800 = ColsNu2<25, 32, 256, 2>::make();
     switch (N) {
