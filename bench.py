@@ -355,10 +355,13 @@ def run_config(cfg, args, steps, warmup, world, local, peaks, traffic_table, fp3
     path = {"auto": None, "direct": binding.PATH_DIRECT, "fft": binding.PATH_FFT}[args.path]
     host_in = torch.from_numpy(views.view(np.int16)).pin_memory()
     host_out = torch.empty((N, H, W), dtype=torch.float32).pin_memory()
+    h2d_bytes = int(views.nbytes)
+    if world > 1:
+        views = None            # N ranks on one host: keep only the pinned copy (the oracle sample runs at N = 1 only)
     dev_in = host_in.cuda()
     dev_out = torch.empty((N, H, W), dtype=torch.float32, device="cuda")
     stream = torch.cuda.Stream()
-    small = views.nbytes + N * H * W * 4 <= 126e6           # fits L2: flush between timed steps
+    small = h2d_bytes + N * H * W * 4 <= 126e6              # fits L2: flush between timed steps
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda") if small else None
 
     def barrier():
@@ -462,7 +465,7 @@ def run_config(cfg, args, steps, warmup, world, local, peaks, traffic_table, fp3
         dt = time.perf_counter() - t0
         dt = shard.max_over_ranks(dt, device="cuda")
         e2e = {"value": shard.job_throughput(units * e2e_steps, dt, world) / 1e6, "unit": UNIT,
-               "h2d_bytes_per_step": int(views.nbytes), "d2h_bytes_per_step": int(host_out.numel() * 4),
+               "h2d_bytes_per_step": h2d_bytes, "d2h_bytes_per_step": int(host_out.numel() * 4),
                "ms_per_step": dt * 1e3 / e2e_steps, "steps": e2e_steps}
         e2e["ratio_to_device_resident"] = e2e["value"] / value
         # context: what the PCIe link alone allows -- the step's input copied host -> device and its output device -> host
