@@ -7,7 +7,8 @@ const SizeOps* mvd_fft_ops_v2(int N) {
     using P512 = Plan<512, 32, 32, 16>;
     using P1024 = Plan<1024, 32, 32, 32>;
     using P2048 = Plan<2048, 32, 32, 32, 2>;
-    static const SizeOps o256 = OpsFor2<P256, 256, P256, 128, true, 4>::make();
+    // columns: OTF in registers, two regions per team in ping-pong (the next slice is requested a whole item ahead)
+    static const SizeOps o256 = OpsFor2<P256, 256, P256, 128, true, 4, true, 4, 2, true>::make();
     static const SizeOps o512 = OpsFor2<P512, 256, P512, 128, false, 3>::make();
     static const SizeOps o1024 = OpsFor2<P1024, 256, P1024, 128, false, 3>::make();
     // rows: the exchange in front of the radix-2 stage goes through warp shuffles; 2 CTAs of 4 teams at 128 registers (since the

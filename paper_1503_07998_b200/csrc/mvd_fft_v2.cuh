@@ -532,6 +532,106 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
     if (l == 0) bulk_wait_read();
 }
 
+// Column pass for plans that keep their OTF in registers (256-point columns), two regions per team in PING-PONG: item i
+// transforms in the region its slice landed in and leaves its results there for the box store, while item i + 1's slice
+// is requested into the other region at the TOP of item i (as soon as item i - 1's results have left it) -- a whole item
+// of lead time instead of one register-only stage, at no extra shared memory (fft2_cols_tma_kernel's second region
+// only holds results on their way out).
+template <class P, int NT, int MINB, int CPT = 4>
+__global__ void __launch_bounds__(NT, MINB)
+fft2_cols_pp_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ otf, int conj_otf, int pairs, int W,
+                    const float2* __restrict__ tw_g) {
+    constexpr int E = P::E, TPF = P::TPF, H = P::N, TEAM = CPT * TPF, NTEAM = NT / TEAM, TC = CPT * NTEAM;
+    constexpr int BOXH = H <= 256 ? H : (H % 256 == 0 ? 256 : 200);
+    static_assert(H % BOXH == 0 && NT % TEAM == 0 && TEAM % 32 == 0 && (TEAM == 32 || NTEAM <= 15), "whole boxes, whole-warp teams");
+    extern __shared__ __align__(128) float2 smem_cols6[];
+    constexpr int TW = (P::S - 1) * E * TPF;
+    constexpr int HP = H + H / P::radix(0);
+    static_assert(TW % 16 == 0 && (HP * CPT) % 16 == 0, "regions stay 128-byte aligned");
+    float2* tw = smem_cols6;                                  // [(S-1) E][TPF]
+    float2* buf = smem_cols6 + TW;                            // [NTEAM][2][HP][CPT]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(buf + NTEAM * 2 * HP * CPT);   // [NTEAM]
+    if (threadIdx.x < NTEAM) mbar_init(&bars[threadIdx.x], 1);
+    if (threadIdx.x == 0) fence_mbar_init();
+    for (int k = threadIdx.x; k < TW; k += NT) tw[k] = tw_g[k];
+    __syncthreads();
+    pdl_launch_dependents();
+    const int team = threadIdx.x / TEAM, l = threadIdx.x % TEAM;
+    const int c4 = l % CPT, t = l / CPT;
+    const ColAddrPad<P, CPT> addr{c4};                        // relative to the region in use
+    const TeamSync<TEAM> sync{team};
+    const float sgn = conj_otf == 1 ? -1.f : 1.f;
+    const bool real_otf = conj_otf == 2;
+    float2* reg0 = buf + team * 2 * HP * CPT;
+    uint64_t* full = &bars[team];
+    const int tiles = W / TC;
+    const int items = tiles * pairs;
+    auto first_col = [&](int item) { return (item % tiles) * TC + team * CPT; };
+    auto plane_off = [&](int x) { return (size_t)(x >> 4) * (H * 16) + (x & 15); };
+    auto box_x = [&](int item) { return 2 * (first_col(item) & 15); };
+    auto box_y = [&](int item) { return ((item / tiles) * (W / 16) + (first_col(item) >> 4)) * H; };
+    auto issue = [&](int item, float2* dst) {   // one lane
+        fence_proxy_async();
+        mbar_arrive_expect_tx(full, (uint32_t)(sizeof(float2) * H * CPT));
+#pragma unroll
+        for (int b = 0; b < H / BOXH; ++b) tma_2d_g2s(dst + b * BOXH * CPT, &tmap, box_x(item), box_y(item) + b * BOXH, full);
+    };
+
+    int item = blockIdx.x;
+    float2 o[E];
+    if (item < items) {   // the OTF is written once in mvd_create: no dependency on the previous kernel
+        const int xg = first_col(item) + c4;
+        if (real_otf) {
+            const float* of = reinterpret_cast<const float*>(otf);
+#pragma unroll
+            for (int e = 0; e < E; ++e) o[e] = make_float2(__ldg(of + plane_off(xg) + (size_t)(t + TPF * e) * 16), 0.f);
+        } else {
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                o[e] = __ldg(otf + plane_off(xg) + (size_t)(t + TPF * e) * 16);
+                o[e].y *= sgn;
+            }
+        }
+    }
+    pdl_wait();
+    if (item < items && l == 0) issue(item, reg0);
+    uint32_t phase = 0;
+    int cur = 0;
+    for (; item < items; item += gridDim.x, cur ^= 1) {
+        float2* X = reg0 + cur * HP * CPT;            // this item's slice, exchange region, results
+        float2* Y = reg0 + (cur ^ 1) * HP * CPT;      // the next item's landing zone
+        float2 x[E];
+        mbar_wait(full, phase);
+        phase ^= 1;
+#pragma unroll
+        for (int e = 0; e < E; ++e) x[e] = X[(t + TPF * e) * CPT + c4];
+        sync();
+        if (l == 0 && item + (int)gridDim.x < items) {
+            bulk_wait_read();                         // the previous item's results have left Y
+            issue(item + gridDim.x, Y);
+        }
+        fft_run<P, -1>(x, X, tw, t, addr, sync);
+        if (real_otf) {
+#pragma unroll
+            for (int e = 0; e < E; ++e) x[e] = mul2(x[e], make_float2(o[e].x, o[e].x));
+        } else {
+#pragma unroll
+            for (int e = 0; e < E; ++e) x[e] = cmul(x[e], o[e]);
+        }
+        fft_run<P, +1>(x, X, tw, t, addr, sync);      // (its last exchange ends with a team barrier: X is free)
+#pragma unroll
+        for (int e = 0; e < E; ++e) X[(t + TPF * e) * CPT + c4] = x[e];
+        fence_proxy_async();
+        sync();
+        if (l == 0) {
+#pragma unroll
+            for (int b = 0; b < H / BOXH; ++b) tma_2d_s2g(&tmap, box_x(item), box_y(item) + b * BOXH, X + b * BOXH * CPT);
+            bulk_commit();
+        }
+    }
+    if (l == 0) bulk_wait_read();
+}
+
 // Column pass for lengths H = RA x RB whose two radices differ (800 = 25 x 32): a two-stage transform in which the
 // stages use different numbers of threads.  RB threads (one warp's worth per column) each hold rows t + RB e and
 // run one radix-RA butterfly; after the exchange RA of them hold RB elements each and run one radix-RB butterfly
@@ -684,8 +784,9 @@ inline cudaError_t launch_pdl(Kern kern, dim3 grid, dim3 block, size_t smem, cud
     return cudaLaunchKernelEx(&cfg, kern, args...);
 }
 
-template <class P, int NT, class PC, int NTC, bool OTF_REGS, int MINB, bool TMA = true, int CPT = 4, int RMINB = 2>
+template <class P, int NT, class PC, int NTC, bool OTF_REGS, int MINB, bool TMA = true, int CPT = 4, int RMINB = 2, bool PP = false>
 struct OpsFor2 {
+    static_assert(!PP || (OTF_REGS && TMA), "the ping-pong column kernel keeps its OTF in registers");
     static_assert(P::N == PC::N, "row and column plan of one entry describe the same length");
     static constexpr size_t kRowSmem = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * row_pitch<P>(P::N));
     static constexpr size_t kRowSmemW = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * row_pitch<P>(2 * P::N));
@@ -693,7 +794,8 @@ struct OpsFor2 {
     static_assert(kRowSmemW <= 227u * 1024u && kRowCpsW >= 1, "the weighted update kernel fits one CTA");
     static constexpr int kTeam = CPT * PC::TPF, kNTeam = NTC / kTeam, kTC = CPT * kNTeam;
     static constexpr size_t kColSmem = sizeof(float2) * ((size_t)(PC::S - 1) * PC::E * PC::TPF +
-                                                         (size_t)kNTeam * CPT * (TMA ? 2 * PC::N + PC::N / PC::radix(0) : PC::N)) +
+                                                         (size_t)kNTeam * CPT * (PP ? 2 * (PC::N + PC::N / PC::radix(0))
+                                                                                    : TMA ? 2 * PC::N + PC::N / PC::radix(0) : PC::N)) +
                                        (TMA ? 2 * sizeof(uint64_t) * kNTeam : 0);
 
     static cudaError_t rows(int mode, const RowArgs& a, const float2* tw, int grid, cudaStream_t st) {
@@ -704,7 +806,9 @@ struct OpsFor2 {
     }
     static cudaError_t cols(const CUtensorMap& tmap, const CUtensorMap& otf_map, float2* S, const float2* otf, int conj_otf, int pairs, int W,
                             const float2* tw, dim3 grid, cudaStream_t st) {
-        if constexpr (TMA)
+        if constexpr (PP)
+            return launch_pdl(fft2_cols_pp_kernel<PC, NTC, MINB, CPT>, grid, dim3(NTC), kColSmem, st, tmap, otf, conj_otf, pairs, W, tw);
+        else if constexpr (TMA)
             return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, grid, dim3(NTC), kColSmem, st, tmap, otf_map, otf, conj_otf, pairs, W, tw);
         else
         return launch_pdl(fft2_cols_kernel<PC, NTC, OTF_REGS, MINB>, grid, dim3(NTC), kColSmem, st, S, otf, conj_otf, pairs, W, tw);
@@ -720,7 +824,9 @@ struct OpsFor2 {
         return cudaFuncSetAttribute(fft2_rows_kernel<P, ROWS_UPDATE, NT, RMINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kRowSmem);
     }
     static cudaError_t prepare_cols() {
-        if constexpr (TMA)
+        if constexpr (PP)
+            return cudaFuncSetAttribute(fft2_cols_pp_kernel<PC, NTC, MINB, CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
+        else if constexpr (TMA)
             return cudaFuncSetAttribute(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
         else
         return cudaFuncSetAttribute(fft2_cols_kernel<PC, NTC, OTF_REGS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
