@@ -93,7 +93,8 @@ MVD_API int mvd_create_path(int plane_w, int plane_h, int n_views, const float* 
  * 2048 - psf_size + 1 runs on it), the direct engine to exactly plane + psf_size - 1; mvd_get_engine_plane tells.
  *   path   MVD_PATH_AUTO (FFT whenever a padded size exists) / MVD_PATH_DIRECT / MVD_PATH_FFT.
  * Layouts, ownership and errors as for mvd_create.  Calls on a padded handle take dense or row-strided views (planes a
- * whole number of rows apart); per-view weights and camera-order host stacks return MVD_ERR_UNSUPPORTED.
+ * whole number of rows apart) and per-view weights (embedded like the views, zero in the padding); camera-order host
+ * stacks return MVD_ERR_UNSUPPORTED.
  * Cost: one zero-fill + embed copy of the views and one crop copy of the result per chunk (2 V + 8 bytes per padded
  * pixel against 42 V T for the iterations), plus the iterations on the larger planes.
  */

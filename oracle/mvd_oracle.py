@@ -146,7 +146,8 @@ def deconvolve(views: np.ndarray, psfs: np.ndarray, T: int, eps: float = 1e-6,
 
 
 def deconvolve_padded(views: np.ndarray, psfs: np.ndarray, T: int, eps: float = 1e-6,
-                      n_threads: Optional[int] = None, extra: int = 0) -> np.ndarray:
+                      n_threads: Optional[int] = None, extra: int = 0,
+                      weights: Optional[np.ndarray] = None) -> np.ndarray:
     """The paper's own boundary (Supp. Table 1 caption: the transformed size is "the sum of the
     actual data size and the size of PSF"): every plane of every view is embedded in a plane K - 1 (+ `extra`)
     pixels larger in x and z, the periodic iteration runs on the padded planes, and the result is cropped.
@@ -159,7 +160,11 @@ def deconvolve_padded(views: np.ndarray, psfs: np.ndarray, T: int, eps: float = 
     K = np.asarray(psfs).shape[1]
     padded = np.zeros((V, N, H + K - 1 + extra, W + K - 1 + extra), dtype=np.uint16)
     padded[:, :, :H, :W] = views
-    return np.ascontiguousarray(deconvolve(padded, psfs, T, eps, n_threads)[:, :H, :W])
+    pw = None
+    if weights is not None:      # reading W1 on the padded planes; the weight in the padding is immaterial (psi = 0 there): 0
+        pw = np.zeros(padded.shape, dtype=np.float32)
+        pw[:, :, :H, :W] = weights
+    return np.ascontiguousarray(deconvolve(padded, psfs, T, eps, n_threads, weights=pw)[:, :H, :W])
 
 
 def deconvolve_product(views: np.ndarray, psfs: np.ndarray, T: int, eps: float = 1e-6,

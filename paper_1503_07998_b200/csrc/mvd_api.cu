@@ -76,6 +76,7 @@ static void ws_free(Workspace& ws) {
     if (ws.g) cudaFree(ws.g);
     if (ws.pin) cudaFree(ws.pin);
     if (ws.pout) cudaFree(ws.pout);
+    if (ws.pw) cudaFree(ws.pw);
     if (ws.c) cudaFree(ws.c);
     if (ws.d) cudaFree(ws.d);
     ws = Workspace();
@@ -399,7 +400,6 @@ static int pad_reserve(mvd_handle* h, Workspace& ws, int n) {
 
 // One chunk of a padded plan: embed, run the engine on the padded planes, crop (reading PD1).
 static int run_padded_chunk(mvd_handle* h, Workspace& ws, const PlaneIO& sub, int n, cudaStream_t stream) {
-    if (sub.weights) return MVD_ERR_UNSUPPORTED;
     if (sub.lay.row < (size_t)h->uW || sub.lay.plane % sub.lay.row != 0 || sub.lay.plane / sub.lay.row < (size_t)h->uH)
         return MVD_ERR_UNSUPPORTED;   // one pitched 3D copy per view: planes must be whole numbers of rows apart
     const size_t npx = (size_t)h->W * h->H;
@@ -418,6 +418,26 @@ static int run_padded_chunk(mvd_handle* h, Workspace& ws, const PlaneIO& sub, in
         MVD_TRY(h, cudaMemcpy3DAsync(&c, stream));
     }
     PlaneIO pio;
+    if (sub.weights) {
+        // weights embedded like the views; ZERO in the padding (psi is zero there whatever the weight is, but the weight
+        // must be finite: 0 . NaN would not be 0).  Allocated at the first weighted call of this workspace.
+        rc = grow(h, &ws.pw, &ws.pw_bytes, sizeof(float) * npx * n * h->V);
+        if (rc != MVD_OK) return rc;
+        MVD_TRY(h, cudaMemsetAsync(ws.pw, 0, sizeof(float) * npx * n * h->V, stream));
+        const size_t unpx = (size_t)h->uW * h->uH;
+        for (int v = 0; v < h->V; ++v) {
+            cudaMemcpy3DParms c = {};
+            c.srcPtr = make_cudaPitchedPtr(const_cast<float*>(sub.weights + (size_t)v * sub.w_view), h->uW * sizeof(float),
+                                           h->uW * sizeof(float), h->uH);
+            c.dstPtr = make_cudaPitchedPtr(ws.pw + (size_t)v * n * npx, h->W * sizeof(float), h->W * sizeof(float), h->H);
+            c.extent = make_cudaExtent(h->uW * sizeof(float), h->uH, n);
+            c.kind = cudaMemcpyDeviceToDevice;
+            MVD_TRY(h, cudaMemcpy3DAsync(&c, stream));
+        }
+        (void)unpx;
+        pio.weights = ws.pw;
+        pio.w_view = (size_t)n * npx;
+    }
     pio.views = ws.pin;
     pio.lay = ViewLayout{(size_t)n * npx, npx, (size_t)h->W};
     if (sub.out16) pio.out16 = reinterpret_cast<uint16_t*>(ws.pout);
@@ -692,7 +712,7 @@ int mvd_deconvolve_host_ex(mvd_handle* h, const mvd_io* io, int n_planes) {
     if (io->out_type != MVD_OUT_F32 && io->out_type != MVD_OUT_U16) return MVD_ERR_INVALID;
     if (io->view_stride || io->plane_stride || io->row_stride) return MVD_ERR_INVALID;   // host stacks are dense
     const bool camera_order = io->camera_order != 0, u16 = io->out_type == MVD_OUT_U16;
-    if (h->padded && (camera_order || io->weights)) return MVD_ERR_UNSUPPORTED;
+    if (h->padded && camera_order) return MVD_ERR_UNSUPPORTED;
     const uint16_t* host_views_u16 = io->views;
     const float* host_w = io->weights;
     const size_t npx = (size_t)h->uW * h->uH;

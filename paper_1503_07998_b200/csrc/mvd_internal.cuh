@@ -53,6 +53,8 @@ struct Workspace {
     uint16_t* pin = nullptr;
     float* pout = nullptr;
     size_t pin_bytes = 0, pout_bytes = 0;
+    float* pw = nullptr;     // ... and the chunk's per-view weights embedded the same way (zero in the padding), fp32 [V][n][H][W]
+    size_t pw_bytes = 0;
     // product-form update (mvd_set_update_mode): the estimate being built (psi^t times the factors so far) and, on the
     // FFT engine, the row spectrum of psi^t that every view's blur starts from
     float* c = nullptr;

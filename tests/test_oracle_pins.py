@@ -470,7 +470,7 @@ def test_PW_argument_validation():
 # ---------------------------------------------------------------------------------------------
 # PD: the paper's padded boundary, READING PD1 = zero padding (oracle.deconvolve_padded)
 # ---------------------------------------------------------------------------------------------
-def _rl_zero_boundary_scipy(views, psfs, T, eps):
+def _rl_zero_boundary_scipy(views, psfs, T, eps, weights=None):
     """RL with ZERO boundary conditions written with scipy's non-periodic routines (independent of the oracle's
     periodic loops): b = convolve2d(psi, P, 'same', fill 0), q = correlate2d(r, P, 'same', fill 0)."""
     from scipy.signal import convolve2d, correlate2d
@@ -485,7 +485,11 @@ def _rl_zero_boundary_scipy(views, psfs, T, eps):
                 P = psfs[v].astype(np.float64)
                 b = convolve2d(psi, P, mode="same", boundary="fill", fillvalue=0.0)
                 r = phi[v] / np.maximum(b, e32)
-                psi = psi * correlate2d(r, P, mode="same", boundary="fill", fillvalue=0.0)
+                q = correlate2d(r, P, mode="same", boundary="fill", fillvalue=0.0)
+                if weights is not None:
+                    w = weights[v, n].astype(np.float64)
+                    q = w * q + (1.0 - w)
+                psi = psi * q
         out[n] = psi
     return out
 
@@ -582,3 +586,17 @@ def test_PP3_product_form_with_weights():
         psi = psi * orc.backproject(phi[0] / np.maximum(orc.blur(psi, psfs[0]), float(np.float32(1e-6))), psfs[0])
     np.testing.assert_allclose(got[0], psi, rtol=1e-12)
     assert one_view.shape == (1, H, W)
+
+
+def test_PD4_padded_mode_with_weights():
+    """Weights on a padded plan: the zero-boundary scipy formulation with reading W1's blend; the weight given to the
+    padding is immaterial (psi is zero there)."""
+    V, N, H, W, K = 2, 2, 9, 13, 5
+    rng = np.random.default_rng(17)
+    views = rng.integers(1, 800, size=(V, N, H, W)).astype(np.uint16)
+    psfs = rand_psfs(V, K, 23)
+    wts = rng.random((V, N, H, W)).astype(np.float32)
+    got = orc.deconvolve_padded(views, psfs, 3, weights=wts)
+    np.testing.assert_allclose(got, _rl_zero_boundary_scipy(views, psfs, 3, 1e-6, weights=wts), rtol=1e-11, atol=1e-300)
+    assert np.abs(got - orc.deconvolve_padded(views, psfs, 3)).max() > 1e-3 * got.max()
+    np.testing.assert_allclose(orc.deconvolve_padded(views, psfs, 3, weights=wts, extra=3), got, rtol=1e-12, atol=1e-300)

@@ -67,17 +67,28 @@ def test_padded_host_pipeline_chunks_and_u16_are_consistent(path):
     assert np.array_equal(u[~near_tie], exp[~near_tie].astype(np.uint16))
 
 
-def test_padded_rejects_weights_and_camera_order():
+@pytest.mark.parametrize("path", PATHS)
+def test_padded_with_weights(path):
+    """Per-view weights on a padded plan, device-resident and through the host pipeline (several batches)."""
+    W, H, K, V, T, N = 100, 60, 9, 2, 4, 7
+    views = synth.random_views(V, N, W, H, seed=31, lo=0, hi=2500)
+    psfs = _psfs(V, K, 13)
+    wts = np.random.default_rng(8).random((V, N, H, W)).astype(np.float32)
+    wts[0, :, :20] = 0.0                                  # view 0 does not cover the top of the planes
+    ref = mvd_oracle.deconvolve_padded(views, psfs, T, float(synth.EPS), weights=wts)
+    out = binding.deconvolve(views, psfs, T, float(synth.EPS), path=path, padded=True, weights=wts)
+    assert_parity(out, ref, f"padded, weighted {binding.PATH_NAMES[path]}")
+    again = binding.deconvolve(views, psfs, T, float(synth.EPS), path=path, padded=True, weights=wts, host=True, batch_planes=2)
+    assert np.array_equal(out, again)
+
+
+def test_padded_rejects_camera_order():
     import torch
     W, H, K, V, N = 64, 40, 5, 2, 2
     psfs = _psfs(V, K, 1)
     views = torch.from_numpy(synth.random_views(V, N, W, H, seed=1).view(np.int16)).cuda()
     out = torch.empty((N, H, W), dtype=torch.float32, device="cuda")
-    wts = torch.ones((V, N, H, W), dtype=torch.float32, device="cuda")
     with binding.Mvd(W, H, V, psfs, K, 2, 1e-6, None, None, True) as m:
-        with pytest.raises(binding.MvdError) as e:
-            m.deconvolve_planes_ex(views, out, N, weights=wts)
-        assert e.value.code == binding.MVD_ERR_UNSUPPORTED
         with pytest.raises(binding.MvdError) as e:
             m.deconvolve_host_ex(views.cpu(), out.cpu(), N, camera_order=True)
         assert e.value.code == binding.MVD_ERR_UNSUPPORTED
