@@ -16,8 +16,10 @@
 //     ((x / 16) H + y) 16 + x % 16, i.e. 16-column tiles of H rows with 128 contiguous bytes per row.  A
 //     column team then walks one contiguous tile (DRAM pages stay open) instead of touching 32 bytes in
 //     every 8 W-byte image row, and a row team still reads whole 128-byte lines;
-//   * exchange regions are XOR-swizzled (position p lives in slot p ^ ((p / R0) & 15)) so that both the
-//     stride-R0 stores of stage 0 and the unit-stride loads are bank-conflict free for 8-byte elements.
+//   * exchange regions are conflict-free for 8-byte elements for both the stride-R0 stores of stage 0 and the
+//     unit-stride loads: padded (position p in slot p + p / R0) in the row kernels and the TMA-fed column kernels --
+//     every address an immediate offset from one base -- and XOR-swizzled (p ^ ((p / R0) & 15)) in the cp.async column
+//     kernel of 2048-point columns.
 #pragma once
 
 #include "mvd_fft_kernels.cuh"
