@@ -350,12 +350,15 @@ def test_chunking_and_host_pipeline_are_bit_identical(path):
     assert np.array_equal(base, _run(pr.views, pr.psfs, T, path, host=True, batch_planes=5))
 
 
-def test_generation2_is_deterministic_and_independent_of_batching():
+@pytest.mark.parametrize("W,H,N", [(512, 256, 11),      # ping-pong 256-point columns, 512-point rows
+                                   (2048, 800, 5),      # config 4: 25 x 32 columns, shuffle-exchange rows
+                                   (1024, 1024, 4)])    # config 5: TMA-fed OTF slices
+def test_generation2_is_deterministic_and_independent_of_batching(W, H, N):
     """The team-synchronous kernels (private exchange regions, cp.async / TMA landing zones, persistent
     grids) must give the same bits run after run and for every chunk / batch split: a missing team
     barrier or an early landing shows up here as a flipped bit.  compute-sanitizer is not available
     on the GPU pool, so this is the race check."""
-    V, N, W, H, K, T = 2, 11, 512, 256, 9, 3
+    V, K, T = 2, 9, 3
     pr = synth.make_problem(V, N, W, H, K, T, seed=123)
     base = _run(pr.views, pr.psfs, T, binding.PATH_FFT)
     for _ in range(4):
@@ -368,7 +371,7 @@ def test_generation2_is_deterministic_and_independent_of_batching():
     assert np.array_equal(base, _run(pr.views, pr.psfs, T, binding.PATH_FFT, host=True, batch_planes=2, chunk_planes=2))
     assert np.array_equal(base, _run(pr.views, pr.psfs, T, binding.PATH_FFT, host=True, batch_planes=6))
     ref = mvd_oracle.deconvolve(pr.views, pr.psfs, T, pr.eps)
-    assert_parity(base, ref, "generation 2, 512x256")
+    assert_parity(base, ref, f"generation 2, {W}x{H}")
 
 
 @pytest.mark.parametrize("path", PATHS)
