@@ -18,8 +18,7 @@
 //     every 8 W-byte image row, and a row team still reads whole 128-byte lines;
 //   * exchange regions are conflict-free for 8-byte elements for both the stride-R0 stores of stage 0 and the
 //     unit-stride loads: padded (position p in slot p + p / R0) in the row kernels and the TMA-fed column kernels --
-//     every address an immediate offset from one base -- and XOR-swizzled (p ^ ((p / R0) & 15)) in the cp.async column
-//     kernel of 2048-point columns.
+//     every address an immediate offset from one base (round 1 used an XOR swizzle, p ^ ((p / R0) & 15)).
 #pragma once
 
 #include "mvd_fft_kernels.cuh"
@@ -36,12 +35,6 @@ __device__ __forceinline__ void prefetch_l2(const void* p, uint32_t bytes) {
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
-template <class P>
-__device__ __forceinline__ int swz(int p) {
-    constexpr int R0 = P::radix(0);
-    static_assert(R0 == 16 || R0 == 32, "the XOR swizzle is derived for first radices 16 and 32");
-    return p ^ ((p / R0) & 15);
-}
 // One FFT per region of N + N / R0 slots, position p in slot p + p / R0 (one spare slot per R0).  For the ROW kernels this
 // padding does what the XOR swizzle does -- stage 0's stores (positions R0 t + m: slots (R0 + 1) t + m) and the loads
 // (positions t + TPF e: consecutive slots) are both conflict-free for 8-byte elements -- and, unlike the XOR, it leaves
@@ -54,14 +47,7 @@ struct RowAddr2 {
 };
 template <class P>
 __host__ __device__ constexpr int row_pitch(int slots) { return slots + slots / P::radix(0); }
-// CPT FFTs (adjacent columns) interleaved: [slot][CPT]
-template <class P, int CPT = 4>
-struct ColAddr2 {
-    int base;   // team region + column within the team
-    __device__ __forceinline__ int operator()(int pos) const { return base + CPT * swz<P>(pos); }
-};
-
-// The same with padding instead of the XOR (TMA-fed column kernels): position p in slot p + p / R0 of a region of
+// CPT FFTs (adjacent columns) interleaved, [slot][CPT], with the same padding: position p in slot p + p / R0 of a region of
 // H + H / R0 slots.  Stage 0's stores ((R0 + 1) t + m: four consecutive t fall into the four 32-byte groups of a line) and
 // the loads (consecutive slots) stay conflict-free, and every address is an immediate offset from one base.
 template <class P, int CPT = 4>
@@ -294,89 +280,8 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
 }
 
 // ---------------------------------------------------------------------------------------------
-// column pass: forward column FFT, . OTF (or its conjugate), inverse column FFT, in place
+// column passes: forward column FFT, . OTF (or its conjugate), inverse column FFT, in place
 // ---------------------------------------------------------------------------------------------
-// The team's exchange region doubles as the landing zone of the NEXT item's slice: it is filled by
-// cp.async while the inverse transform runs its register-only last stage and the results are stored.
-template <class P, int NT, bool OTF_REGS, int MINB>
-__global__ void __launch_bounds__(NT, MINB)
-fft2_cols_kernel(float2* __restrict__ S, const float2* __restrict__ otf, int conj_otf, int pairs, int W,
-                 const float2* __restrict__ tw_g) {
-    constexpr int E = P::E, TPF = P::TPF, H = P::N, TEAM = 4 * TPF, NTEAM = NT / TEAM, TC = 4 * NTEAM;
-    static_assert(NT % TEAM == 0 && TEAM % 32 == 0 && (TEAM == 32 || NTEAM <= 15), "column teams are whole warps");
-    static_assert((2 * H) % TEAM == 0, "the landing copy splits evenly over the team");
-    extern __shared__ __align__(16) float2 smem_cols2[];
-    float2* tw = smem_cols2;                                  // [(S-1) E][TPF]
-    float2* buf = smem_cols2 + (P::S - 1) * E * TPF;          // [NTEAM][H][4]  exchange regions / landing zones
-    for (int k = threadIdx.x; k < (P::S - 1) * E * TPF; k += NT) tw[k] = tw_g[k];
-    __syncthreads();
-    pdl_launch_dependents();
-    const int team = threadIdx.x / TEAM, l = threadIdx.x % TEAM;
-    const int c4 = l & 3, t = l >> 2;
-    const ColAddr2<P> addr{team * H * 4 + c4};
-    const TeamSync<TEAM> sync{team};
-    const float sgn = conj_otf ? -1.f : 1.f;
-    float2* land = buf + team * H * 4;
-    // Work items (group of TC columns, pair), column group fastest, dealt round-robin to a persistent
-    // grid.  With OTF_REGS the host makes gridDim.x a multiple of the group count: a CTA keeps its columns.
-    const int tiles = W / TC;
-    const int items = tiles * pairs;
-    auto first_col = [&](int item) { return (item % tiles) * TC + team * 4; };
-    // tile-major offset of (row 0, column x) within a plane: 16-column tiles of H rows, 16 elements per row
-    auto plane_off = [&](int x) { return (size_t)(x >> 4) * (H * 16) + (x & 15); };
-
-    // chunk q of a team's slice: image row q / 2, columns x0 + 2 (q % 2) .. + 1  (16 bytes)
-    auto issue = [&](int item) {
-        const float2* src = S + (size_t)(item / tiles) * H * W + plane_off(first_col(item));
-#pragma unroll
-        for (int k = 0; k < 2 * H / TEAM; ++k) {
-            const int q = l + TEAM * k;
-            cp_async16(land + 2 * q, src + (size_t)(q >> 1) * 16 + 2 * (q & 1));
-        }
-        cp_async_commit();
-    };
-
-    int item = blockIdx.x;
-    float2 o[OTF_REGS ? E : 1];
-    if (OTF_REGS && item < items) {   // the OTF is written once in mvd_create: no dependency on the previous kernel
-        const int xg = first_col(item) + c4;
-#pragma unroll
-        for (int e = 0; e < E; ++e) {
-            o[e] = __ldg(otf + plane_off(xg) + (size_t)(t + TPF * e) * 16);
-            o[e].y *= sgn;
-        }
-    }
-    pdl_wait();
-    if (item < items) issue(item);
-    for (; item < items; item += gridDim.x) {
-        const int xg = first_col(item) + c4;
-        float2* Sp = S + (size_t)(item / tiles) * H * W + plane_off(xg);
-        float2 x[E];
-        cp_async_wait_all();
-        sync();
-#pragma unroll
-        for (int e = 0; e < E; ++e) x[e] = land[(t + TPF * e) * 4 + c4];
-        sync();
-        fft_run<P, -1>(x, buf, tw, t, addr, sync);
-#pragma unroll
-        for (int e = 0; e < E; ++e) {
-            float2 w;
-            if (OTF_REGS) {
-                w = o[e];
-            } else {
-                w = __ldg(otf + plane_off(xg) + (size_t)(t + TPF * e) * 16);
-                w.y *= sgn;
-            }
-            x[e] = cmul(x[e], w);
-        }
-        fft_run_head<P, +1>(x, buf, tw, t, addr, sync);
-        if (item + (int)gridDim.x < items) issue(item + gridDim.x);
-        fft_run_tail<P, +1>(x, buf, tw, t, addr, sync);
-#pragma unroll
-        for (int e = 0; e < E; ++e) Sp[(size_t)(t + TPF * e) * 16] = x[e];
-    }
-}
-
 // 2D tiled tensor copy shared -> global (SASS UTMASTG), bulk-group completion
 __device__ __forceinline__ void tma_2d_s2g(const CUtensorMap* map, int x, int y, const void* src) {
     asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
@@ -788,7 +693,8 @@ inline cudaError_t launch_pdl(Kern kern, dim3 grid, dim3 block, size_t smem, cud
 
 template <class P, int NT, class PC, int NTC, bool OTF_REGS, int MINB, bool TMA = true, int CPT = 4, int RMINB = 2, bool PP = false>
 struct OpsFor2 {
-    static_assert(!PP || (OTF_REGS && TMA), "the ping-pong column kernel keeps its OTF in registers");
+    static_assert(TMA, "every generation-2 column kernel is TMA-fed");
+    static_assert(!PP || OTF_REGS, "the ping-pong column kernel keeps its OTF in registers");
     static_assert(P::N == PC::N, "row and column plan of one entry describe the same length");
     static constexpr size_t kRowSmem = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * row_pitch<P>(P::N));
     static constexpr size_t kRowSmemW = sizeof(float2) * ((size_t)(P::S - 1) * P::E * P::TPF + (size_t)(NT / P::TPF) * row_pitch<P>(2 * P::N));
@@ -810,10 +716,8 @@ struct OpsFor2 {
                             const float2* tw, dim3 grid, cudaStream_t st) {
         if constexpr (PP)
             return launch_pdl(fft2_cols_pp_kernel<PC, NTC, MINB, CPT>, grid, dim3(NTC), kColSmem, st, tmap, otf, conj_otf, pairs, W, tw);
-        else if constexpr (TMA)
-            return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, grid, dim3(NTC), kColSmem, st, tmap, otf_map, otf, conj_otf, pairs, W, tw);
         else
-        return launch_pdl(fft2_cols_kernel<PC, NTC, OTF_REGS, MINB>, grid, dim3(NTC), kColSmem, st, S, otf, conj_otf, pairs, W, tw);
+            return launch_pdl(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, grid, dim3(NTC), kColSmem, st, tmap, otf_map, otf, conj_otf, pairs, W, tw);
     }
     static cudaError_t prepare_rows() {
         cudaError_t e;
@@ -828,10 +732,8 @@ struct OpsFor2 {
     static cudaError_t prepare_cols() {
         if constexpr (PP)
             return cudaFuncSetAttribute(fft2_cols_pp_kernel<PC, NTC, MINB, CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
-        else if constexpr (TMA)
-            return cudaFuncSetAttribute(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
         else
-        return cudaFuncSetAttribute(fft2_cols_kernel<PC, NTC, OTF_REGS, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
+            return cudaFuncSetAttribute(fft2_cols_tma_kernel<PC, NTC, OTF_REGS, MINB, CPT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kColSmem);
     }
     static SizeOps make() {
         SizeOps o;
