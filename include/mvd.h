@@ -57,7 +57,8 @@ enum {
 
 /* Convolution engine used for steps a1 and a3 (both engines fuse a2 and a4 into their kernels). */
 enum {
-    MVD_PATH_AUTO = 0,   /* chosen in mvd_create: FFT whenever the shape is supported (measured) */
+    MVD_PATH_AUTO = 0,   /* chosen in mvd_create from the measured crossover: the FFT engine on every shape its
+                            fast kernels take; on the other supported shapes whichever engine is estimated faster for this K  */
     MVD_PATH_DIRECT = 1, /* shared-memory halo tiles + register-blocked FP32 FMA; any shape               */
     MVD_PATH_FFT = 2     /* hand-written batched 2D FFT with the pointwise steps fused into the passes;
                             plane_w and plane_h must be supported transform lengths (32 ... 2048) within the kernel's

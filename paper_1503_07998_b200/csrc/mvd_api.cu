@@ -170,15 +170,21 @@ int mvd_path_supported(int path, int plane_w, int plane_h, int psf_size) {
     return 0;
 }
 
-// Measured crossover: the FFT engine moves a fixed number of bytes per
-// voxel-view-iteration whatever K is, the direct engine does 4 K^2 flop.
-static int choose_path(int W, int H, int K) {
+// Measured crossover.  The FFT engine moves a fixed number of bytes per voxel-view-iteration whatever K
+// is: ~120 GVoxel/s on shapes its generation-2 kernels take (where it wins at EVERY K, even K = 3), ~31 GVoxel/s on
+// shapes only generation 1 takes.  The direct engine does 4 K^2 flop per unit (88 ... 5.5 GVoxel/s for K = 3 ... 51), or
+// 8 K with separable PSFs (79 / 63 GVoxel/s at K = 21 / 41).  So on generation-1 shapes the direct engine is chosen when its
+// estimate is better -- except for planes small enough for launch overheads to decide (below 256 x 256: config 1's 8 planes
+// of 64 x 64 take 0.22 ms on the FFT engine's replayed launches against 0.50 ms for the direct engine's on-chip kernel).
+static int choose_path(int W, int H, int K, bool separable) {
     const bool fft_ok = mvd_path_supported(MVD_PATH_FFT, W, H, K) != 0;
     const bool dir_ok = mvd_path_supported(MVD_PATH_DIRECT, W, H, K) != 0;
-    // Measured: the FFT engine wins at every K, even K = 3, on large stacks; on config 1 its
-    // 81 short launches (0.41 ms) still beat the direct engine's one-launch on-chip kernel (0.50 ms), which keeps
-    // only one SM per plane pair busy.
-    (void)K;
+    if (fft_ok && dir_ok && fft_generation(W, H) == 1 && (long long)W * H >= 256 * 256) {
+        const double fft_rate = 31.0;
+        const double direct_rate = separable && K >= 3 && K <= 65 ? std::min(85.0, 95.0 - 0.8 * K)
+                                   : K <= 9 ? 75.0 : K <= 13 ? 50.0 : 13000.0 / ((double)K * K);
+        if (direct_rate > 1.1 * fft_rate) return MVD_PATH_DIRECT;
+    }
     if (fft_ok) return MVD_PATH_FFT;
     if (dir_ok) return MVD_PATH_DIRECT;
     return -1;
@@ -217,7 +223,7 @@ static int create_impl(int plane_w, int plane_h, int n_views, const float* psfs,
         else { path = MVD_PATH_DIRECT; eng_w = w_min; eng_h = h_min; }
         if ((long long)eng_w * eng_h > (1LL << 30) || !mvd_path_supported(path, eng_w, eng_h, k_eff)) return MVD_ERR_UNSUPPORTED;
     } else if (path == MVD_PATH_AUTO) {
-        path = choose_path(plane_w, plane_h, k_eff);
+        path = choose_path(plane_w, plane_h, k_eff, !xs && sep_psfs_separable(n_views, psfs, psf_size));
         if (path < 0) return MVD_ERR_UNSUPPORTED;
     } else if (!mvd_path_supported(path, plane_w, plane_h, k_eff)) {
         return MVD_ERR_UNSUPPORTED;

@@ -176,17 +176,21 @@ int fft_supported(int W, int H) {
     return 1;
 }
 
+// 0: not supported, 1: generation-1 kernels, 2: generation-2 (team) kernels
+int fft_generation(int W, int H) { return !fft_supported(W, H) ? 0 : use_v2(W, H) ? 2 : 1; }
+
 int fft_pad_dims(int w_min, int h_min, int* Wp, int* Hp) {
     std::vector<int> lens;
     for (int n = 32; n <= 2048; ++n)
         if (find_ops_v1(n) || mvd_fft_ops_v2(n)) lens.push_back(n);
-    // cost = padded area, x 1.6 for shapes only the generation-1 kernels take (measured ratio of the two generations)
+    // cost = padded area x the measured relative cost per voxel: generation-2 shapes 1 (2048-point columns 1.25: one team
+    // per SM), shapes only the generation-1 kernels take 3.5 (30-42 against 110-150 GVoxel/s, profiles/r2_experiments.md)
     double best = 0.0;
     for (int w : lens) {
         if (w < w_min) continue;
         for (int hh : lens) {
             if (hh < h_min || !fft_supported(w, hh)) continue;
-            const double cost = (double)w * hh * (use_v2(w, hh) ? 1.0 : 1.6);
+            const double cost = (double)w * hh * (use_v2(w, hh) ? (hh == 2048 ? 1.25 : 1.0) : 3.5);
             if (best == 0.0 || cost < best) { best = cost; *Wp = w; *Hp = hh; }
         }
     }

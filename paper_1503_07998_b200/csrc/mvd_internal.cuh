@@ -207,6 +207,7 @@ int direct_repair_launch(mvd_handle* h, const PlaneIO& io, float* psi, float* r_
 
 // ---- fft path (mvd_fft.cu) --------------------------------------------------------------------
 int fft_supported(int W, int H);
+int fft_generation(int W, int H);   // 0: not supported, 1: generation-1 kernels, 2: generation-2 (team) kernels
 // smallest supported W x H (by area) with W >= w_min and H >= h_min; 0 if there is none
 int fft_pad_dims(int w_min, int h_min, int* W, int* H);
 int fft_setup(mvd_handle* h, const float* host_psfs, const float* host_xs);
