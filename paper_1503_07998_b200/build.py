@@ -18,7 +18,7 @@ INCLUDE = os.path.join(os.path.dirname(_HERE), "include")
 LIB = os.path.join(_HERE, "libmvd.so")
 _STAMP = os.path.join(_HERE, "csrc", ".build_stamp")
 SOURCES = ["mvd_api.cu", "mvd_direct.cu", "mvd_sep.cu", "mvd_files.cu", "mvd_fft.cu", "mvd_fft_inst_small.cu", "mvd_fft_inst_mid.cu",
-           "mvd_fft_inst_large.cu", "mvd_fft_inst_v2.cu", "mvd_fft_inst_more_a.cu", "mvd_fft_inst_more_b.cu", "mvd_peak.cu"]
+           "mvd_fft_inst_large.cu", "mvd_fft_inst_v2.cu", "mvd_fft_inst_v2b.cu", "mvd_fft_inst_more_a.cu", "mvd_fft_inst_more_b.cu", "mvd_peak.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC,-O2,-fvisibility=hidden",
               "-Xptxas", "-v", "-shared", "-cudart", "static"]

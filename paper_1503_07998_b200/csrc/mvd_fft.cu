@@ -190,7 +190,7 @@ int fft_pad_dims(int w_min, int h_min, int* Wp, int* Hp) {
         if (w < w_min) continue;
         for (int hh : lens) {
             if (hh < h_min || !fft_supported(w, hh)) continue;
-            const double cost = (double)w * hh * (use_v2(w, hh) ? (hh == 2048 ? 1.25 : 1.0) : 3.5);
+            const double cost = (double)w * hh * (use_v2(w, hh) ? (hh == 2048 || hh == 1536 ? 1.25 : 1.0) : 3.5);
             if (best == 0.0 || cost < best) { best = cost; *Wp = w; *Hp = hh; }
         }
     }

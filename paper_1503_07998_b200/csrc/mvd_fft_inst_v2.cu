@@ -25,6 +25,6 @@ const SizeOps* mvd_fft_ops_v2(int N) {
         case 800: return &o800;
         case 1024: return &o1024;
         case 2048: return &o2048;
-        default: return nullptr;
+        default: return mvd_fft_ops_v2b(N);
     }
 }

@@ -344,6 +344,52 @@ struct Bfly<20, DIR> : BflyTimes5<4, DIR> {};
 template <int DIR>
 struct Bfly<40, DIR> : BflyTimes5<8, DIR> {};
 
+// cos / sin of 2 pi k / 24 as compile-time constants (k any integer)
+__host__ __device__ constexpr float cos24(int k) {
+    constexpr float C[7] = {1.0f, 0.96592582628906828675f, 0.86602540378443864676f, 0.70710678118654752440f, 0.5f,
+                            0.25881904510252076235f, 0.0f};
+    k = ((k % 24) + 24) % 24;
+    if (k > 12) k = 24 - k;
+    return k > 6 ? -C[12 - k] : C[k];
+}
+__host__ __device__ constexpr float sin24(int k) { return cos24(k - 6); }
+
+// 24 = 8 x 3: n = n1 + 3 n2 (n1 < 3, n2 < 8), f = f2 + 8 f1; 8-point transforms over n2, twiddles w24^(n1 f2), 3-point
+// transforms over n1
+template <int DIR>
+struct Bfly<24, DIR> {
+    static __device__ __forceinline__ void run(float2* v) {
+        float2 a[3][8];
+#pragma unroll
+        for (int n1 = 0; n1 < 3; ++n1) {
+            float2 t[8];
+#pragma unroll
+            for (int n2 = 0; n2 < 8; ++n2) t[n2] = v[n1 + 3 * n2];
+            Bfly<8, DIR>::run(t);
+#pragma unroll
+            for (int f2 = 0; f2 < 8; ++f2) a[n1][f2] = t[f2];
+        }
+#pragma unroll
+        for (int n1 = 1; n1 < 3; ++n1) {
+#pragma unroll
+            for (int f2 = 1; f2 < 8; ++f2) {
+                const int k = n1 * f2;
+                if (k % 24 == 6) a[n1][f2] = rot90<DIR>(a[n1][f2]);
+                else if (k % 24 == 3) a[n1][f2] = rot45<DIR>(a[n1][f2]);
+                else if (k % 24 == 9) a[n1][f2] = rot135<DIR>(a[n1][f2]);
+                else a[n1][f2] = cmul(a[n1][f2], make_float2(cos24(k), (DIR < 0 ? -1.f : 1.f) * sin24(k)));
+            }
+        }
+#pragma unroll
+        for (int f2 = 0; f2 < 8; ++f2) {
+            float2 t[3] = {a[0][f2], a[1][f2], a[2][f2]};
+            Bfly<3, DIR>::run(t);
+#pragma unroll
+            for (int f1 = 0; f1 < 3; ++f1) v[f2 + 8 * f1] = t[f1];
+        }
+    }
+};
+
 // cos / sin of 2 pi k / 25 as compile-time constants (k any integer)
 __host__ __device__ constexpr float cos25(int k) {
     constexpr float C[13] = {1.0f, 0.96858316112863107605f, 0.87630668004386358394f, 0.72896862742141155245f,
@@ -995,4 +1041,5 @@ const mvdfft::SizeOps* mvd_fft_ops_mid(int N);
 const mvdfft::SizeOps* mvd_fft_ops_large(int N);
 const mvdfft::SizeOps* mvd_fft_ops_more_a(int N);   // 384, 768, 1536
 const mvdfft::SizeOps* mvd_fft_ops_more_b(int N);   // 640, 1280, 1600
-const mvdfft::SizeOps* mvd_fft_ops_v2(int N);      // power-of-two lengths, team kernels
+const mvdfft::SizeOps* mvd_fft_ops_v2(int N);      // power-of-two lengths (and 800-point columns), team kernels
+const mvdfft::SizeOps* mvd_fft_ops_v2b(int N);     // 384, 768, 1536, 640, 1280, team kernels

@@ -282,6 +282,11 @@ __global__ void __launch_bounds__(NT, RMINB) fft2_rows_kernel(RowArgs a, const f
 // ---------------------------------------------------------------------------------------------
 // column passes: forward column FFT, . OTF (or its conjugate), inverse column FFT, in place
 // ---------------------------------------------------------------------------------------------
+// rows per TMA box of a column slice: the largest supported divisor of H up to 256 (a box dimension is at most 256)
+__host__ __device__ constexpr int col_box_h(int H) {
+    return H <= 256 ? H : H % 256 == 0 ? 256 : H % 200 == 0 ? 200 : H % 192 == 0 ? 192 : H % 160 == 0 ? 160 : 128;
+}
+
 // 2D tiled tensor copy shared -> global (SASS UTMASTG), bulk-group completion
 __device__ __forceinline__ void tma_2d_s2g(const CUtensorMap* map, int x, int y, const void* src) {
     asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.bulk_group [%0, {%1, %2}], [%3];"
@@ -302,7 +307,7 @@ __global__ void __launch_bounds__(NT, MINB)
 fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap omap,
                      const float2* __restrict__ otf, int conj_otf, int pairs, int W, const float2* __restrict__ tw_g) {
     constexpr int E = P::E, TPF = P::TPF, H = P::N, TEAM = CPT * TPF, NTEAM = NT / TEAM, TC = CPT * NTEAM;
-    constexpr int BOXH = H <= 256 ? H : (H % 256 == 0 ? 256 : 200);
+    constexpr int BOXH = col_box_h(H);
     static_assert(H % BOXH == 0 && (CPT == 4 || CPT == 8 || CPT == 16), "whole boxes; a team owns whole 32-byte sectors of a row");
     static_assert(NT % TEAM == 0 && TEAM % 32 == 0 && (TEAM == 32 || NTEAM <= 15), "column teams are whole warps");
     extern __shared__ __align__(128) float2 smem_cols3[];
@@ -449,7 +454,7 @@ __global__ void __launch_bounds__(NT, MINB)
 fft2_cols_pp_kernel(const __grid_constant__ CUtensorMap tmap, const float2* __restrict__ otf, int conj_otf, int pairs, int W,
                     const float2* __restrict__ tw_g) {
     constexpr int E = P::E, TPF = P::TPF, H = P::N, TEAM = CPT * TPF, NTEAM = NT / TEAM, TC = CPT * NTEAM;
-    constexpr int BOXH = H <= 256 ? H : (H % 256 == 0 ? 256 : 200);
+    constexpr int BOXH = col_box_h(H);
     static_assert(H % BOXH == 0 && NT % TEAM == 0 && TEAM % 32 == 0 && (TEAM == 32 || NTEAM <= 15), "whole boxes, whole-warp teams");
     extern __shared__ __align__(128) float2 smem_cols6[];
     constexpr int TW = (P::S - 1) * E * TPF;
@@ -553,7 +558,7 @@ __global__ void __launch_bounds__(NT, MINB)
 fft2_cols_nu_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_constant__ CUtensorMap omap,
                     int conj_otf, int pairs, int W, const float2* __restrict__ tw_g) {
     constexpr int H = RA * RB, TPF = RB, CPT = 4, TEAM = CPT * TPF, NTEAM = NT / TEAM, TC = CPT * NTEAM;
-    constexpr int BOXH = H <= 256 ? H : (H % 256 == 0 ? 256 : 200);
+    constexpr int BOXH = col_box_h(H);
     static_assert(RB == 32 && RA <= RB, "one warp's worth of threads per column");
     static_assert(H % BOXH == 0 && NT % TEAM == 0 && NTEAM <= 15, "whole boxes, whole teams");
     extern __shared__ __align__(128) float2 smem_cols5[];
@@ -742,7 +747,7 @@ struct OpsFor2 {
         o.col = PlanInfo{PC::E, PC::TPF, PC::S, {PC::radix(0), PC::radix(1), PC::radix(2), PC::radix(3), PC::radix(4)}};
         o.row_threads = NT;
         o.row_smem = kRowSmem;
-        o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = TMA ? (PC::N < 256 ? PC::N : 256) : 0; o.col_box_w = 2 * CPT;
+        o.col_smem = kColSmem; o.col_tc = kTC; o.col_box_h = col_box_h(PC::N); o.col_box_w = 2 * CPT;
         o.rows = &rows; o.cols = &cols; o.prepare_rows = &prepare_rows; o.prepare_cols = &prepare_cols;
         o.generation = 2;
         o.row_cps = RMINB;
@@ -758,7 +763,7 @@ struct OpsFor2 {
 template <int RA, int RB, int NTC, int MINB>
 struct ColsNu2 {
     static constexpr int kN = RA * RB, kNTeam = NTC / (4 * RB), kTC = 4 * kNTeam;
-    static constexpr int kBoxH = kN <= 256 ? kN : (kN % 256 == 0 ? 256 : 200);
+    static constexpr int kBoxH = col_box_h(kN);
     static constexpr size_t kColSmem = sizeof(float2) * ((size_t)RA * RB + (size_t)kNTeam * ((RA * (RB + 1) * 4 + 15) / 16 * 16 + kN * 4)) +
                                        2 * sizeof(uint64_t) * kNTeam;
     static cudaError_t cols(const CUtensorMap& tmap, const CUtensorMap& otf_map, float2*, const float2*, int conj_otf, int pairs, int W,
