@@ -352,7 +352,8 @@ def test_chunking_and_host_pipeline_are_bit_identical(path):
 
 @pytest.mark.parametrize("W,H,N", [(512, 256, 11),      # ping-pong 256-point columns, 512-point rows
                                    (2048, 800, 5),      # config 4: 25 x 32 columns, shuffle-exchange rows
-                                   (1024, 1024, 4)])    # config 5: TMA-fed OTF slices
+                                   (1024, 1024, 4),     # config 5: TMA-fed OTF slices
+                                   (768, 640, 6)])      # three-stage plans with radix-24 / radix-40 first stages
 def test_generation2_is_deterministic_and_independent_of_batching(W, H, N):
     """The team-synchronous kernels (private exchange regions, cp.async / TMA landing zones, persistent
     grids) must give the same bits run after run and for every chunk / batch split: a missing team
