@@ -457,7 +457,8 @@ def run_config(cfg, args, steps, warmup, world, local, peaks, traffic_table, fp3
         for _ in range(max(1, min(warmup, 2))):
             m.deconvolve_host(host_in, host_out, N)
         barrier()
-        e2e_steps = max(steps, 50) if small else steps      # sub-millisecond steps: enough of them to time by wall clock
+        # sub-millisecond steps: enough of them to time by wall clock; steps of a few milliseconds: at least 20
+        e2e_steps = max(steps, 50) if small else (max(steps, 20) if ms_max / steps < 50.0 else steps)
         t0 = time.perf_counter()
         for _ in range(e2e_steps):
             m.deconvolve_host(host_in, host_out, N)

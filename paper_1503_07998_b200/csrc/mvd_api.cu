@@ -134,7 +134,9 @@ static int run_graphed(mvd_handle* h, const uint64_t (&key)[8], cudaStream_t st,
         return body();
     }
     cudaGraphDestroy(g);
-    if (h->graphs.size() >= 16) {     // bounded: evict the least recently used
+    // bounded: evict the least recently used.  One host-pipeline call alone needs up to 4 slots x 4 batch sizes (ramp, full,
+    // remainder) = 16 entries; a cache of that size thrashed as soon as a device-resident capture joined them.
+    if (h->graphs.size() >= 64) {
         size_t lru = 0;
         for (size_t i = 1; i < h->graphs.size(); ++i)
             if (h->graphs[i].last_use < h->graphs[lru].last_use) lru = i;
