@@ -51,6 +51,8 @@ def parse():
     ap.add_argument("--per-config", default="1,2,3,4,5", help="configs reported in `per_config` (N = 1 only; '' = none)")
     ap.add_argument("--per-config-steps", type=int, default=5, help="timed steps of the per_config entries")
     ap.add_argument("--planes", type=int, default=0, help="override the number of planes (0 = the config's)")
+    ap.add_argument("--shape", default="", help="WxH: the config's views, PSFs and iteration count on planes of another size "
+                                                "(measurement of other shapes; the headline stays the config's own)")
     ap.add_argument("--path", default="auto", choices=["auto", "direct", "fft"])
     ap.add_argument("--chunk", type=int, default=0, help="mvd_set_chunk_planes (0 = library default)")
     ap.add_argument("--batch", type=int, default=0, help="mvd_set_batch_planes (0 = library default)")
@@ -505,6 +507,10 @@ def main():
     cfg = synth.config(args.config)
     if args.planes:
         cfg = cfg.with_planes(args.planes)
+    if args.shape:
+        import dataclasses
+        w, h = (int(x) for x in args.shape.lower().split("x"))
+        cfg = dataclasses.replace(cfg, W=w, H=h, name=f"{cfg.name} on {w}x{h} planes")
     if args.impl == "reference":
         return run_reference(args, cfg)
 
@@ -530,7 +536,7 @@ def main():
             peaks = json.load(f)
     except OSError:
         peaks = {}
-    traffic_table = load_traffic_table()
+    traffic_table = {} if args.shape else load_traffic_table()      # the ncu captures belong to the configs' own shapes
     fp32_peak = binding.measure_fp32_peak()
 
     main_rec, psfs, views = run_config(cfg, args, args.steps, args.warmup, world, local, peaks, traffic_table,
@@ -544,7 +550,7 @@ def main():
 
     # ---- every config, shorter (N = 1 only): value, e2e, per-class roofline, clocks ---------------
     per_config = None
-    if world == 1 and args.per_config and not args.planes:
+    if world == 1 and args.per_config and not args.planes and not args.shape:
         per_config = []
         for cid in [int(c) for c in args.per_config.split(",") if c]:
             if cid == cfg.cid:
@@ -559,7 +565,7 @@ def main():
     # ---- the direct engine (FP32-bound; the fallback for shapes the FFT engine does not take), driver-measured on
     # config 2's shape with 128 planes: value and the FFMA-pipe roofline of its two kernels ----------------------
     direct = None
-    if world == 1 and args.per_config and not args.planes and args.path == "auto":
+    if world == 1 and args.per_config and not args.planes and not args.shape and args.path == "auto":
         import copy
         a2 = copy.copy(args)
         a2.path = "direct"
