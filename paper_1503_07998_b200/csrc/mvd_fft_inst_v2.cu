@@ -15,8 +15,9 @@ const SizeOps* mvd_fft_ops_v2(int N) {
     // instruction diet they fit without spills).  3 CTAs of 2 teams at 168 registers run the update pass 3 % faster ALONE but the
     // whole step, with two batches in flight, 1.5 % slower (profiles/r2_experiments.md).
     // columns: one 256-thread team per SM (166 KB: both regions of 2048 rows and a 32 KB twiddle table); the cp.async kernel
-    // it replaces fitted two CTAs but ran at 0.28 of the copy peak against 0.41 (2048 x 2048 planes: 75 -> 88 GVoxel/s)
-    static const SizeOps o2048 = OpsFor2<ShflTail<P2048>, 256, P2048, 256, false, 1, true, 4, 2>::make();
+    // it replaces fitted two CTAs but ran at 0.28 of the copy peak against 0.44 (2048 x 2048 planes: 75 -> 92 GVoxel/s);
+    // the shuffle exchange serves the columns too (lanes l and l ^ 16 hold threads t and t ^ 32 of a column)
+    static const SizeOps o2048 = OpsFor2<ShflTail<P2048>, 256, ShflTail<P2048>, 256, false, 1, true, 4, 2>::make();
     // columns only: 800 = 25 x 32 with unequal thread counts per stage, four columns per team of four warps
     static const SizeOps o800 = ColsNu2<25, 32, 256, 2>::make();
     switch (N) {

@@ -326,7 +326,12 @@ fft2_cols_tma_kernel(const __grid_constant__ CUtensorMap tmap, const __grid_cons
     __syncthreads();
     pdl_launch_dependents();
     const int team = threadIdx.x / TEAM, l = threadIdx.x % TEAM;
-    const int c4 = l % CPT, t = l / CPT;
+    // ShflTail plans (2048 points): threads t and t ^ 32 of a column sit in lanes l and l ^ 16 of one warp, so that the
+    // exchange in front of the radix-2 stage goes through shuffles (fft_stage); a half-warp still covers 4 consecutive t
+    // x CPT = 4 columns = one 128-byte line of the regions
+    static_assert(!shfl_tail<P>() || (CPT == 4 && TPF == 64), "shuffle exchange: four columns, 64 threads per column");
+    const int c4 = l % CPT;
+    const int t = shfl_tail<P>() ? (((l >> 4) & 1) << 5) | (((l >> 5) & 7) << 2) | ((l >> 2) & 3) : l / CPT;
     const ColAddrPad<P, CPT> addr{team * HP * CPT + c4};
     const TeamSync<TEAM> sync{team};
     const float sgn = conj_otf == 1 ? -1.f : 1.f;
