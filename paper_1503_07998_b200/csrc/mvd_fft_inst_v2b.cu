@@ -12,7 +12,7 @@ const SizeOps* mvd_fft_ops_v2b(int N) {
     using P1280 = Plan<1280, 40, 40, 8, 4>;
     static const SizeOps o384 = OpsFor2<P384, 256, P384, 128, false, 3>::make();
     static const SizeOps o768 = OpsFor2<P768, 256, P768, 128, false, 3>::make();
-    static const SizeOps o1536 = OpsFor2<P1536, 256, P1536, 256, false, 1>::make();
+    static const SizeOps o1536 = OpsFor2<P1536, 256, P1536, 512, false, 1>::make();     // columns: two 256-thread teams share one twiddle table (225 KB)
     static const SizeOps o640 = OpsFor2<P640, 128, P640, 128, false, 2, true, 4, 3>::make();     // E = 40: 168 registers, 3 CTAs
     static const SizeOps o1280 = OpsFor2<P1280, 128, P1280, 128, false, 2, true, 4, 3>::make();
     switch (N) {
