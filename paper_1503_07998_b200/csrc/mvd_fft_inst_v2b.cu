@@ -11,7 +11,7 @@ const SizeOps* mvd_fft_ops_v2b(int N) {
     using P640 = Plan<640, 40, 40, 4, 4>;
     using P1280 = Plan<1280, 40, 40, 8, 4>;
     static const SizeOps o384 = OpsFor2<P384, 256, P384, 128, false, 3>::make();
-    static const SizeOps o768 = OpsFor2<P768, 256, P768, 128, false, 3>::make();
+    static const SizeOps o768 = OpsFor2<P768, 256, P768, 512, false, 1>::make();       // columns: four teams share one twiddle table (16 warps per SM)
     static const SizeOps o1536 = OpsFor2<P1536, 256, P1536, 512, false, 1>::make();     // columns: two 256-thread teams share one twiddle table (225 KB)
     static const SizeOps o640 = OpsFor2<P640, 128, P640, 128, false, 2, true, 4, 3>::make();     // E = 40: 168 registers, 3 CTAs
     static const SizeOps o1280 = OpsFor2<P1280, 128, P1280, 128, false, 2, true, 4, 3>::make();
