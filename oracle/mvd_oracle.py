@@ -3,6 +3,11 @@
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
 this module.  It never imports the CUDA package, and the CUDA package never imports it.
 
+Parity unpinned (no value in the paper fixes the READING; the arithmetic under the reading is pinned in
+tests/test_oracle_pins.py): the per-view weights of `deconvolve(weights=)` (reading W1), the zero fill of
+`deconvolve_padded` (reading PD1), the variant builders of `backprojectors()` (readings B1-B4).  Everything else --
+`deconvolve`, `deconvolve_product`, `blur`, `backproject`, `trace` -- is pinned (P1-P11, PX1-PX4, PP1-PP3).
+
 The shared object is compiled with gcc on the machine that uses it (seconds), keyed by the source
 hash and the host's CPU flags, so a copy built on another box is never executed with the wrong ISA.
 """
@@ -151,7 +156,8 @@ def deconvolve_padded(views: np.ndarray, psfs: np.ndarray, T: int, eps: float = 
     """The paper's own boundary (Supp. Table 1 caption: the transformed size is "the sum of the
     actual data size and the size of PSF"): every plane of every view is embedded in a plane K - 1 (+ `extra`)
     pixels larger in x and z, the periodic iteration runs on the padded planes, and the result is cropped.
-    READING PD1 (the paper does not say what the padding holds): the padding is ZERO.
+    READING PD1 (the paper does not say what the padding holds; parity of the reading unpinned,
+    arithmetic pinned by PD1-PD4): the padding is ZERO.
     Then psi_0 and every later psi are zero in it (the update is multiplicative) and so is r (phi = 0), i.e. the
     result on the plane is the RL iteration with zero boundary conditions -- whatever `extra` is (pin PD1).
     """
