@@ -116,3 +116,19 @@ def test_product_does_not_import_the_oracle():
                 src = f.read()
             assert not re.search(r"^\s*(import|from)\s+paper_1503_07998_b200\b", src, flags=re.M), fn
             assert "libmvd.so" not in src and "csrc/" not in src and "mvd.h\"" not in src, fn
+
+
+def test_header_constants_match_the_binding():
+    with open(os.path.join(ROOT, "include", "mvd.h")) as f:
+        text = f.read()
+    def const(name):
+        m = re.search(name + r"\s*=\s*(-?\d+)", text)
+        assert m, name
+        return int(m.group(1))
+    assert const("MVD_NOALLOC_MAX_VOXELS") == binding.NOALLOC_MAX_VOXELS
+    assert const("MVD_N_KERNEL_CLASSES") == binding.N_KERNEL_CLASSES
+    for name, val in (("MVD_ERR_INVALID", binding.MVD_ERR_INVALID), ("MVD_ERR_UNSUPPORTED", binding.MVD_ERR_UNSUPPORTED),
+                      ("MVD_ERR_CUDA", binding.MVD_ERR_CUDA), ("MVD_ERR_NOMEM", binding.MVD_ERR_NOMEM),
+                      ("MVD_ERR_IO", binding.MVD_ERR_IO), ("MVD_ERR_TOO_LARGE", binding.MVD_ERR_TOO_LARGE),
+                      ("MVD_UPDATE_PRODUCT", binding.UPDATE_PRODUCT), ("MVD_OUT_U16", binding.OUT_U16)):
+        assert const(name) == val, name
