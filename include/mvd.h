@@ -305,7 +305,9 @@ MVD_API int mvd_path_supported(int path, int plane_w, int plane_h, int psf_size)
  *                                    with the kernels of the sequential form: the factors are multiplied into a copy of psi^t
  *                                    that becomes psi^{t+1} after the last view (FFT engine: every view's blur restarts
  *                                    from a saved copy of psi^t's row spectrum; 8 (1 + 2 / V) extra bytes per unit).  The FFT
- *                                    engine's guard (mvd_guard_flagged) does not repair plane pairs in this mode.
+ *                                    engine's guard repairs flagged plane pairs with the direct engine's arithmetic in this
+ *                                    mode as well (plans whose PSF is too large for the repair kernel only count them:
+ *                                    mvd_guard_flagged).
  * Call it before mvd_reserve.  Errors: MVD_ERR_INVALID.
  */
 enum { MVD_UPDATE_SEQUENTIAL = 0, MVD_UPDATE_PRODUCT = 1 };

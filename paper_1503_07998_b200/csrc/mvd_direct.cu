@@ -277,6 +277,8 @@ struct RepairArgs {
     const float* weights;       // nullptr or [V][n][H][W] (a4w)
     size_t w_view;
     uint16_t* out16;            // nullptr, or the uint16 output that receives the repaired planes (out is then scratch)
+    float* acc;                 // nullptr: sequential update; else product form (PAPER.md:79 as printed): scratch like out, in
+                                // which psi^t times the factors so far is built while kernel A keeps reading psi^t
     int n_planes, W, H, K, Kp, V, T;
     float eps;
 };
@@ -321,8 +323,23 @@ __global__ void __launch_bounds__(BX* BY) direct_repair_kernel(RepairArgs a) {
     }
     grid_barrier(a.barrier, ++epoch * gridDim.x);
 
+    // dst <- src on the flagged pairs (every CTA takes a share; the caller puts a grid barrier behind it)
+    auto copy_flagged = [&](float* dst, const float* src) {
+        for (int k = 0; k < nf; ++k) {
+            const int pa = 2 * s_list[k];
+            const int np = pa + 1 < a.n_planes ? 2 : 1;
+            for (size_t q = (size_t)blockIdx.x * (BX * BY) + tid; q < np * npx; q += (size_t)gridDim.x * (BX * BY))
+                dst[(size_t)pa * npx + q] = __ldcg(src + (size_t)pa * npx + q);
+        }
+    };
     const size_t per = (size_t)a.K * a.Kp;
-    for (int t = 0; t < a.T; ++t)
+    float* psi = a.out;     // psi^t
+    float* acc = a.acc;     // product form: the estimate being built (the two swap roles after every iteration)
+    for (int t = 0; t < a.T; ++t) {
+        if (acc) {
+            copy_flagged(acc, psi);
+            grid_barrier(a.barrier, ++epoch * gridDim.x);
+        }
         for (int v = 0; v < a.V; ++v) {
             const float* Gblur = a.coef + ((size_t)v * 2 + 0) * per;
             const float* Gback = a.coef + ((size_t)v * 2 + 1) * per;
@@ -330,19 +347,27 @@ __global__ void __launch_bounds__(BX* BY) direct_repair_kernel(RepairArgs a) {
             for (int w = blockIdx.x; w < nf * tiles; w += gridDim.x) {
                 const int pa = 2 * s_list[w / tiles], tl = w % tiles;
                 __syncthreads();   // the previous tile's shared memory is no longer read
-                corr2_tile<KT, JC, 0, true>(smem, a.out, Gblur, phi, a.r, a.W, a.H, a.K, a.Kp, a.eps, tl % tiles_x,
+                corr2_tile<KT, JC, 0, true>(smem, psi, Gblur, phi, a.r, a.W, a.H, a.K, a.Kp, a.eps, tl % tiles_x,
                                       tl / tiles_x, pa, pa + 1 < a.n_planes, a.lay.plane, a.lay.row, true);
             }
             grid_barrier(a.barrier, ++epoch * gridDim.x);
             for (int w = blockIdx.x; w < nf * tiles; w += gridDim.x) {
                 const int pa = 2 * s_list[w / tiles], tl = w % tiles;
                 __syncthreads();
-                corr2_tile<KT, JC, 1, true>(smem, a.r, Gback, nullptr, a.out, a.W, a.H, a.K, a.Kp, a.eps, tl % tiles_x,
+                corr2_tile<KT, JC, 1, true>(smem, a.r, Gback, nullptr, acc ? acc : psi, a.W, a.H, a.K, a.Kp, a.eps, tl % tiles_x,
                                       tl / tiles_x, pa, pa + 1 < a.n_planes, 0, 0, true,
                                       a.weights ? a.weights + (size_t)v * a.w_view : nullptr);
             }
             grid_barrier(a.barrier, ++epoch * gridDim.x);
         }
+        if (acc) {
+            float* tmp = psi; psi = acc; acc = tmp;
+        }
+    }
+    if (psi != a.out) {     // product form, odd iteration count: the result sits in the scratch
+        copy_flagged(a.out, psi);
+        grid_barrier(a.barrier, ++epoch * gridDim.x);
+    }
     if (a.out16)
         for (int k = 0; k < nf; ++k) {
             const int pa = 2 * s_list[k];
@@ -714,8 +739,9 @@ int launch_repair(const mvd_handle* h, RepairArgs& a, cudaStream_t st) {
 bool direct_repair_available(const mvd_handle* h) { return h->d_coef != nullptr && h->direct_pair; }
 
 int direct_repair_launch(mvd_handle* h, const PlaneIO& io, float* psi, float* r_scratch,
-                         const unsigned* flags, unsigned* barrier, int n_planes, cudaStream_t stream) {
+                         const unsigned* flags, unsigned* barrier, int n_planes, cudaStream_t stream, float* acc) {
     RepairArgs a;
+    a.acc = acc;
     a.views = io.views; a.lay = io.lay; a.out = psi; a.r = r_scratch; a.coef = h->d_coef; a.flags = flags;
     a.barrier = barrier; a.total = h->d_guard_total;
     a.weights = io.weights; a.w_view = io.w_view; a.out16 = io.out16;

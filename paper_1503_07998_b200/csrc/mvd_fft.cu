@@ -95,6 +95,15 @@ __global__ void otf_cols_kernel(const double2* __restrict__ G, int K, int W, int
     else O[idx] = make_float2((float)(re * sc), (float)(im * sc));
 }
 
+// Product-form runs are not repaired (the repair kernel implements the sequential update): the flagged plane pairs are
+// only counted, so that mvd_guard_flagged tells the caller which stacks to rerun on the direct engine.
+__global__ void guard_count_kernel(const unsigned* __restrict__ flags, int pairs, unsigned* __restrict__ total) {
+    unsigned n = 0;
+    for (int p = threadIdx.x; p < pairs; p += blockDim.x) n += flags[p] ? 1u : 0u;
+    n = __reduce_add_sync(0xffffffffu, n);
+    if ((threadIdx.x & 31) == 0 && n) atomicAdd(total, n);
+}
+
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
                                   const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
                                   CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
@@ -457,7 +466,15 @@ int fft_run(mvd_handle* h, Workspace& ws, const PlaneIO& io, int n_planes, cudaS
         }
         if (product) std::swap(Zcur, Acc);
     }
-    if (product) return MVD_OK;     // (the guard's repair pass recomputes the sequential form: not offered here)
+    if (product) {
+        // the repair pass runs the product form too (psi^t and the estimate being built in two buffers): Z and the
+        // product-form scratch are free by now.  Plans without a repair kernel only count the flagged pairs.
+        if (direct_repair_available(h))
+            return direct_repair_launch(h, io, io.out ? io.out : ws.b, ws.a, ws.g + pairs, ws.g + 2 * pairs, n_planes, stream, ws.c);
+        LaunchScope ls(h, KC_GUARD_REPAIR, stream);
+        guard_count_kernel<<<1, 256, 0, stream>>>(ws.g + pairs, pairs, h->d_guard_total);
+        return mvd_check(h, cudaGetLastError());
+    }
     // guard: pairs flagged by the ratio passes are recomputed with the direct engine's arithmetic (one empty
     // cooperative launch when nothing is flagged); Z is free by now and serves as its ratio scratch
     // (with uint16 output psi is iterated in S, which is free as well)

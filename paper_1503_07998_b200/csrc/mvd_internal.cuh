@@ -202,8 +202,9 @@ int sep_launch(int mode, const mvd_handle* h, int v, const float* src, const uin
 bool direct_small_available(const mvd_handle* h);
 bool direct_repair_available(const mvd_handle* h);
 // psi: fp32 [n][H][W] iteration buffer of the repair (io.out itself, or scratch when the output is uint16)
+// acc: nullptr (sequential update) or fp32 [n][H][W] scratch for the product form (mvd_set_update_mode)
 int direct_repair_launch(mvd_handle* h, const PlaneIO& io, float* psi, float* r_scratch,
-                         const unsigned* flags, unsigned* barrier, int n_planes, cudaStream_t stream);
+                         const unsigned* flags, unsigned* barrier, int n_planes, cudaStream_t stream, float* acc = nullptr);
 
 // ---- fft path (mvd_fft.cu) --------------------------------------------------------------------
 int fft_supported(int W, int H);

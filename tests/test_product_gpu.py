@@ -65,3 +65,24 @@ def test_product_form_weights_pipeline_chunks_u16(path):
     u = binding.deconvolve(pr.views, pr.psfs, T, pr.eps, path=path, product=True, out_u16=True)
     near_tie = np.abs(a - np.floor(a) - 0.5) < 1e-3
     assert np.array_equal(u[~near_tie], np.clip(np.rint(a.astype(np.float64)), 0, 65535)[~near_tie].astype(np.uint16))
+
+
+def test_product_form_guard_repairs_collapsed_estimates():
+    """A scalar 'PSF' (K = 1) in the product form: psi^{t+1} = phi_0 phi_1 / psi^t drives the estimate towards zero where one
+    view is dark, the blur falls below the transforms' round-off and a2 divides noise.  The FFT engine flags those plane
+    pairs and hands them to the direct engine's arithmetic -- in the product form too."""
+    import torch
+    V, N, W, H, K, T = 2, 5, 512, 512, 1, 2
+    pr = synth.make_problem(V, N, W, H, K, T, seed=228, psf="sparse")
+    ref = mvd_oracle.deconvolve_product(pr.views, pr.psfs, T, pr.eps)
+    with binding.Mvd(W, H, V, pr.psfs, K, T, pr.eps, binding.PATH_FFT) as m:
+        m.set_update_mode(binding.UPDATE_PRODUCT)
+        dv = torch.from_numpy(pr.views.view(np.int16)).cuda()
+        do = torch.empty((N, H, W), dtype=torch.float32, device="cuda")
+        m.deconvolve_planes(dv, do, N)
+        torch.cuda.synchronize()
+        flagged = m.guard_flagged()
+        out = do.cpu().numpy()
+    direct = binding.deconvolve(pr.views, pr.psfs, T, pr.eps, path=binding.PATH_DIRECT, product=True)
+    assert_parity(direct, ref, "product form, K = 1, direct engine")
+    assert_parity(out, ref, f"product form, K = 1, FFT engine ({flagged} pairs repaired)")
